@@ -1,0 +1,168 @@
+/* bs.h — C-ABI boundary of the B200-native phononic band-structure hot path.
+ *
+ * Method: mixed-variational plane-wave formulation of arXiv:1310.6380 ("PAPER.md" below), 2-D plane strain
+ * (eq. 13-14), plane waves alpha,beta in [-Mt,Mt] (eq. 15), matrices Phi, Psi(=paper's
+ * Omega), H of PAPER.md:140-173 (eq. 17-20), eigenproblem PAPER.md:94-104 (eq. 10-11) solved as the Hermitian pencil
+ * K(k) U = lambda Psi U, K(k) = H(k)^dagger Phi^{-1} H(k), lambda = omega^2.  Readings of ambiguous passages: DESIGN.md
+ * section 3.
+ *
+ * Conventions common to every call
+ *   - All matrices are column-major complex128 stored as interleaved (re,im) doubles, leading dimension = order.
+ *   - N = (2Mt+1)^2 plane waves; plane wave g <-> (a1,a2), g = (a1+Mt)(2Mt+1) + (a2+Mt)  (PAPER.md:150, 0-based).
+ *   - Entry (row alpha = test function, column beta = trial function) uses q = G_beta - G_alpha.
+ *   - "host" / "device" is stated per pointer.  Inputs are copied at bs_create_cell (the caller keeps its arrays).
+ *   - Every call returns a bs_status; bs_last_error() gives a thread-local message for the last failure.
+ *   - A handle is not thread-safe; distinct handles are independent.  `stream` is a cudaStream_t passed as void*
+ *     (NULL = the legacy default stream).  All kernels of a call are launched on that stream.
+ *   - There is NO CPU fallback: without a CUDA device every compute call returns BS_ERR_CUDA.
+ */
+#ifndef BS_H_
+#define BS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bs_cell bs_cell; /* opaque; owns small device buffers (geometry), borrows the big workspace */
+
+typedef enum {
+  BS_OK = 0,
+  BS_ERR_ARG = -1,      /* null pointer, negative size, nbands > 2N, ... */
+  BS_ERR_GEOMETRY = -2, /* polygon with non-positive signed area, or sum of areas != |det lattice| (1e-10 relative) */
+  BS_ERR_NOT_PD = -3,   /* a Cholesky pivot of Phi or of R (Psi = diag(R,R)) was not positive */
+  BS_ERR_STATE = -4,    /* call order violated (e.g. bs_bands before bs_assemble) */
+  BS_ERR_CUDA = -5,     /* CUDA runtime error, or no device */
+  BS_ERR_NOMEM = -6     /* workspace missing or too small */
+} bs_status;
+
+/* Options for bs_set_option. */
+typedef enum {
+  BS_OPT_PENCIL_MODE = 0, /* 0 = BS_PENCIL_POLY (default), 1 = BS_PENCIL_DIRECT; see bs_bands */
+  BS_OPT_PANEL = 1,       /* Householder panel width nb of the tridiagonalisation, 4..32, multiple of 4 (default 32) */
+  BS_OPT_TIMING = 2       /* 1 = record CUDA events around the stages (read back with bs_get_timings) */
+} bs_option;
+enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
+
+/* Stage indices of bs_get_timings (milliseconds, CUDA events on the call's stream). */
+enum {
+  BS_T_TABLE = 0,   /* S1 shape-integral table               */
+  BS_T_EXPAND = 1,  /* S2 expansion to Phi, R                */
+  BS_T_FACTOR = 2,  /* S3 Cholesky(Phi), Phi^{-1}, Cholesky(R), L_R^{-1} */
+  BS_T_COEF = 3,    /* S4+S5 on the six k-polynomial coefficient matrices (POLY mode, inside bs_assemble) */
+  BS_T_PENCIL = 4,  /* S4(+S5 in DIRECT mode): per-k formation of A(k)   */
+  BS_T_TRIDIAG = 5, /* S6 Householder tridiagonalisation     */
+  BS_T_BISECT = 6,  /* S7 Sturm bisection                    */
+  BS_T_COUNT = 8
+};
+
+/* PAPER.md:121 (eq. 14): isotropic plane-strain compliance D_jkmn from Young's modulus E and Poisson ratio nu.
+ * E, nu: host, n doubles each.  compliance_out: host, n x 6 doubles, row = [D1111 D2222 D1122 D1112 D2212 D1212]
+ * (the component order of PAPER.md:167-171, eq. 20).  Pure host arithmetic.  BS_ERR_ARG on null / n<0 / E<=0 / nu>=0.5. */
+bs_status bs_isotropic_plane_strain(int32_t n, const double *E, const double *nu, double *compliance_out);
+
+/* PAPER.md:21-37 (section II: lattice vectors h^1,h^2, phases with their own compliance D and density rho).
+ *   lattice     host, 4 doubles [h1x h1y h2x h2y]: rows of [A]_{jk} = h^j . e^k.
+ *   nphase      number of phases P >= 1; each phase is one simple polygon.
+ *   vert_offset host, P+1 int32, CSR offsets into verts (vert_offset[0] = 0, >= 3 vertices per polygon).
+ *   verts       host, 2*vert_offset[P] doubles, Cartesian (x,y) pairs, counter-clockwise.  Polygons may stick out of
+ *               the cell (lattice-translated pieces); together they must tile the cell area exactly.
+ *   compliance  host, P x 6 doubles [D1111 D2222 D1122 D1112 D2212 D1212] per phase (eq. 20).
+ *   density     host, P doubles, > 0.
+ *   out         receives the handle (free with bs_destroy_cell).
+ * Does S0 (reciprocal basis eq. 1, fractional coordinates, per-edge arrays) on the host and copies them to the device.
+ * Errors: BS_ERR_ARG, BS_ERR_GEOMETRY, BS_ERR_CUDA. */
+bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
+                         const double *compliance, const double *density, bs_cell **out);
+
+void bs_destroy_cell(bs_cell *cell);
+
+bs_status bs_set_option(bs_cell *cell, int32_t option, int32_t value);
+
+/* Device workspace the handle needs for truncation Mt and up to nk k-points per bs_bands call (depends on the
+ * options set so far).  The caller allocates it (e.g. a torch uint8 tensor), 256-byte aligned, and lends it with
+ * bs_set_workspace; it must stay alive and untouched until bs_destroy_cell or the next bs_set_workspace. */
+bs_status bs_workspace_bytes(const bs_cell *cell, int32_t truncation, int32_t nk, size_t *bytes);
+bs_status bs_set_workspace(bs_cell *cell, void *dev_ptr, size_t bytes);
+
+/* S1+S2+S3 (+ the k-independent part of S4/S5 in POLY mode), PAPER.md:140-173:
+ *   S1  T_c(D) = sum_p w_{c,p} I_p(D1 q^1 + D2 q^2) for every index difference D in [-2Mt,2Mt]^2, with the closed-form
+ *       polygon integral I_p(q) = int_{Omega_p} exp(i q.x) dx (exact version of the centroid rule eq. 12/22);
+ *   S2  Phi (3N x 3N, eq. 20 with its factors 1/2/4) and R (N x N, eq. 19; Psi = diag(R,R));
+ *   S3  Phi = L L^dagger, Y = Phi^{-1} explicitly, R = L_R L_R^dagger, L_R^{-1}.
+ * Asynchronous on `stream` except for one final synchronise that reads the Cholesky status.
+ * Errors: BS_ERR_ARG (Mt < 0 or 2N > 2048), BS_ERR_NOMEM, BS_ERR_NOT_PD, BS_ERR_CUDA. */
+bs_status bs_assemble(bs_cell *cell, int32_t truncation, void *stream);
+
+/* The same for ncells handles in one set of launches (config 4: optimisation-loop batch).  All cells must have a
+ * workspace set for the same truncation. */
+bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t truncation, void *stream);
+
+/* Parity access after bs_assemble: copies Phi (3N x 3N) and Psi (2N x 2N) to HOST buffers (either may be NULL). */
+bs_status bs_get_matrices(bs_cell *cell, void *phi_host, void *psi_host);
+/* Parity access: the table T_c(D), host, 7 x (4Mt+1) x (4Mt+1) complex128, index [c][D1+2Mt][D2+2Mt];
+ * channels c = Dv11 Dv22 Dv12 Dv13 Dv23 Dv33 (Voigt weights of eq. 20) then rho. */
+bs_status bs_get_table(bs_cell *cell, void *table_host);
+/* Parity access: K(k) = H^dagger Phi^{-1} H (2N x 2N, HOST out) at one reduced k-point (S4 only). */
+bs_status bs_get_pencil(bs_cell *cell, const double kred[2], void *K_host, void *stream);
+
+/* S4..S8 for nk k-points:
+ *   kpts        HOST, nk x 2 doubles, reduced coordinates (Q1,Q2), k = Q1 q^1 + Q2 q^2.
+ *   nbands      1 <= nbands <= 2N.
+ *   omega2_out  nk x nbands doubles, row-major, ascending lambda = omega^2 per k; HOST or DEVICE pointer
+ *               (detected); a host pointer implies a final stream synchronise.
+ * All k-points are in flight on the device at once; there is no host round-trip between k-points.
+ * POLY mode: A(k) = L_Psi^{-1} K(k) L_Psi^{-dagger} is evaluated as the quadratic polynomial in (kx,ky) whose six
+ * coefficient matrices bs_assemble prepared; DIRECT mode forms K(k) by the scaling kernel and reduces it per k.
+ * Errors: BS_ERR_STATE, BS_ERR_ARG, BS_ERR_NOMEM (nk larger than the workspace was sized for), BS_ERR_CUDA. */
+bs_status bs_bands(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *stream);
+
+/* The same k-points for ncells assembled cells in one set of launches.  omega2_out: ncells x nk x nbands. */
+bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, const double *kpts, int32_t nbands,
+                         double *omega2_out, void *stream);
+
+/* Parity access after bs_bands: the tridiagonal T(k) of the last call, HOST out: d (nk x 2N), e (nk x 2N, last unused). */
+bs_status bs_get_tridiagonal(bs_cell *cell, double *d_host, double *e_host);
+
+/* Stage timings of the last bs_assemble / bs_bands on this handle (BS_OPT_TIMING=1), HOST out, BS_T_COUNT doubles (ms).
+ * For a batch call the timings are recorded on cells[0]. */
+bs_status bs_get_timings(bs_cell *cell, double *ms_out);
+
+/* Number of kernel launches issued by the library on behalf of this handle since creation (batch: on cells[0]). */
+int64_t bs_launch_count(const bs_cell *cell);
+
+const char *bs_last_error(void); /* thread-local, valid until the next call on this thread */
+
+/* ---- diagnostics: the dense building blocks, exposed so that tests can check them in isolation ------------------- */
+/* C = alpha op(A) op(B) + beta C on DEVICE column-major complex128 arrays; op: 0 = none, 1 = conjugate transpose.
+ * flags: see DESIGN.md section 5 (BS_GEMM_*).  batch >= 1 matrices with the given element strides. */
+bs_status bs_zgemm(int32_t opA, int32_t opB, int32_t M, int32_t N, int32_t K, const double alpha[2], const void *A,
+                   int32_t lda, int64_t strideA, const void *B, int32_t ldb, int64_t strideB, const double beta[2],
+                   void *C, int32_t ldc, int64_t strideC, int32_t batch, int32_t flags, void *stream);
+/* In-place lower Cholesky of `batch` n x n DEVICE matrices (stride in elements) and X = L^{-1} (lower, zeros above);
+ * tmp: DEVICE scratch of batch*strideA elements; dinv: DEVICE scratch, batch*ceil(n/64)*64*64 elements;
+ * info: DEVICE int32[batch] (0 = ok, else 1-based failing pivot). */
+bs_status bs_zpotrf_trtri(int32_t n, void *A, int32_t lda, int64_t strideA, void *X, void *tmp, void *dinv,
+                          int32_t *info, int32_t batch, void *stream);
+/* Householder tridiagonalisation of `batch` n x n Hermitian DEVICE matrices (lower triangle read, destroyed).
+ * d, e: DEVICE, batch x n doubles.  vw: DEVICE scratch, batch*2*n*nb complex. */
+bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *vw, int32_t nb,
+                    int32_t batch, void *stream);
+/* Lowest nev eigenvalues of `batch` real symmetric tridiagonal matrices (d, e: DEVICE, batch x n) by Sturm bisection;
+ * lam: DEVICE, batch x nev, ascending. */
+bs_status bs_sturm(int32_t n, const double *d, const double *e, int32_t nev, double *lam, int32_t batch, void *stream);
+
+enum {
+  BS_GEMM_LOWER_ONLY = 1, /* compute only tiles that intersect the lower triangle of C */
+  BS_GEMM_KLO_ROW = 2,    /* op(A)[m][k] = 0 for k < m   (start the k loop at the tile's first row)   */
+  BS_GEMM_KHI_ROW = 4,    /* op(A)[m][k] = 0 for k > m   (stop the k loop after the tile's last row)  */
+  BS_GEMM_KLO_COL = 8,    /* op(B)[k][n] = 0 for k < n */
+  BS_GEMM_KHI_COL = 16    /* op(B)[k][n] = 0 for k > n */
+};
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BS_H_ */

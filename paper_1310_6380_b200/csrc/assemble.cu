@@ -1,0 +1,128 @@
+// S1 (shape-integral table) and S2 (expansion to Phi, R).  PAPER.md:140-173 (eq. 17-20) with the exact polygon
+// integral in place of the centroid rule (eq. 12/22); DESIGN.md sections 3 (R1: entries depend only on the index
+// difference) and 5.
+#include "bs_internal.cuh"
+
+namespace bsk {
+
+static constexpr double kPi = 3.14159265358979323846264338327950288;
+
+// One warp per index difference D in the half plane {D1>0} u {D1==0, D2>=0}; lanes stride over the edges.
+//   T_c(D) = (-i/|q|^2) sum_edges w_c[phase(e)] (q x e) exp(i q.m_e) j0(q.e/2),   q = D1 q^1 + D2 q^2,
+// and T_c(0) = sum_p w_c[p] area_p.  The phase q.m and the argument of j0 are evaluated in FRACTIONAL coordinates
+// (q.x = 2 pi (D1 H1 + D2 H2) with integer D), so sincospi/sinpi reduce the argument exactly.
+__global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table) {
+  const int cell = blockIdx.y;
+  const Geometry g = geos[cell];
+  const int L = 4 * Mt + 1;
+  const int L2 = L * L;
+  const int nhalf = (L2 + 1) / 2;
+  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  if (warp >= nhalf) return;
+  const int flat = warp + (L2 - 1) / 2;
+  const int D1 = flat / L - 2 * Mt;
+  const int D2 = flat % L - 2 * Mt;
+  cplx *T = batch_ptr(table, cell, 0);
+
+  double accr[7], acci[7];
+#pragma unroll
+  for (int c = 0; c < 7; ++c) accr[c] = acci[c] = 0.0;
+
+  if (D1 == 0 && D2 == 0) {
+    for (int p = lane; p < g.P; p += 32) {
+      const double a = g.area[p];
+#pragma unroll
+      for (int c = 0; c < 7; ++c) accr[c] = fma(g.w[c * g.P + p], a, accr[c]);
+    }
+  } else {
+    const double qx = D1 * g.Q[0] + D2 * g.Q[2];
+    const double qy = D1 * g.Q[1] + D2 * g.Q[3];
+    const int ne = g.nedge;
+    const double *mh1 = g.edge, *mh2 = g.edge + ne, *eh1 = g.edge + 2 * ne, *eh2 = g.edge + 3 * ne;
+    const double *ex = g.edge + 4 * ne, *ey = g.edge + 5 * ne;
+    for (int e = lane; e < ne; e += 32) {
+      const double phi = fma((double)D1, mh1[e], (double)D2 * mh2[e]);  // q.m / (2 pi)
+      const double u = fma((double)D1, eh1[e], (double)D2 * eh2[e]);    // q.e / (2 pi)  ->  q.e/2 = pi u
+      double sn, cs;
+      sincospi(2.0 * phi, &sn, &cs);
+      const double j0 = (u == 0.0) ? 1.0 : sinpi(u) / (kPi * u);
+      const double f = (qx * ey[e] - qy * ex[e]) * j0;
+      const double tr = f * cs, ti = f * sn;
+      const int p = g.ephase[e];
+#pragma unroll
+      for (int c = 0; c < 7; ++c) {
+        const double w = g.w[c * g.P + p];
+        accr[c] = fma(w, tr, accr[c]);
+        acci[c] = fma(w, ti, acci[c]);
+      }
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 7; ++c) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      accr[c] += __shfl_xor_sync(0xffffffffu, accr[c], o);
+      acci[c] += __shfl_xor_sync(0xffffffffu, acci[c], o);
+    }
+  }
+  if (lane == 0) {
+    if (D1 == 0 && D2 == 0) {
+#pragma unroll
+      for (int c = 0; c < 7; ++c) T[(size_t)c * L2 + flat] = cmake(accr[c], 0.0);
+    } else {
+      const double qx = D1 * g.Q[0] + D2 * g.Q[2];
+      const double qy = D1 * g.Q[1] + D2 * g.Q[3];
+      const double inv = 1.0 / (qx * qx + qy * qy);
+#pragma unroll
+      for (int c = 0; c < 7; ++c) {
+        // (-i) * (ar + i ai) = ai - i ar
+        const double re = acci[c] * inv, im = -accr[c] * inv;
+        T[(size_t)c * L2 + flat] = cmake(re, im);
+        T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);  // T(-D) = conj T(D): Phi, R exactly Hermitian
+      }
+    }
+  }
+}
+
+void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, cudaStream_t s) {
+  const int L = 4 * Mt + 1;
+  const int nhalf = (L * L + 1) / 2;
+  dim3 grid((nhalf + 7) / 8, ncells);
+  table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table);
+}
+
+// S2: one thread per (g_alpha, g_beta): Phi[(a,ga),(b,gb)] = T_{c(a,b)}(D(gb) - D(ga)), R[ga,gb] = T_rho(...).
+// Consecutive threads -> consecutive rows ga (column-major stores coalesce; table reads are nearly contiguous).
+__global__ void __launch_bounds__(256) expand_kernel(int Mt, BatchRef table, BatchRef Phi, BatchRef R) {
+  const int cell = blockIdx.z;
+  const int W = 2 * Mt + 1;
+  const int N = W * W;
+  const int L = 4 * Mt + 1;
+  const int L2 = L * L;
+  const int ga = blockIdx.x * blockDim.x + threadIdx.x;
+  const int gb = blockIdx.y;
+  if (ga >= N) return;
+  const cplx *T = batch_ptr(table, cell, 0);
+  cplx *P = batch_ptr(Phi, cell, 0);
+  cplx *Rm = batch_ptr(R, cell, 0);
+  const int d1 = gb / W - ga / W + 2 * Mt;
+  const int d2 = gb % W - ga % W + 2 * Mt;
+  const int f = d1 * L + d2;
+  const size_t n3 = 3 * (size_t)N;
+  // channel of block (a,b): 11 22 12 13 23 33 -> 0 1 2 3 4 5
+  const int chan[3][3] = {{0, 2, 3}, {2, 1, 4}, {3, 4, 5}};
+#pragma unroll
+  for (int b = 0; b < 3; ++b)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) P[((size_t)b * N + gb) * n3 + (size_t)a * N + ga] = T[(size_t)chan[a][b] * L2 + f];
+  Rm[(size_t)gb * N + ga] = T[(size_t)6 * L2 + f];
+}
+
+void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s) {
+  const int W = 2 * Mt + 1, N = W * W;
+  dim3 grid((N + 255) / 256, N, ncells);
+  expand_kernel<<<grid, 256, 0, s>>>(Mt, table, Phi, R);
+}
+
+}  // namespace bsk

@@ -1,0 +1,108 @@
+// Internal declarations shared by the translation units of libbs.so (sm_100a).  Not part of the C-ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+#include <vector>
+
+#include "bs.h"
+
+typedef double2 cplx;
+
+// ---------------------------------------------------------------- small complex helpers (device)
+__host__ __device__ __forceinline__ cplx cmake(double r, double i) { return make_double2(r, i); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {  // a * conj(b)
+  return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+__device__ __forceinline__ cplx cconj(cplx a) { return make_double2(a.x, -a.y); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
+// acc += a*b
+__device__ __forceinline__ void cfma(cplx &acc, cplx a, cplx b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(-a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(a.y, b.x, acc.y);
+}
+// acc += conj(a)*b
+__device__ __forceinline__ void cfmac(cplx &acc, cplx a, cplx b) {
+  acc.x = fma(a.x, b.x, acc.x);
+  acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(a.x, b.y, acc.y);
+  acc.y = fma(-a.y, b.x, acc.y);
+}
+// acc -= a*b
+__device__ __forceinline__ void cfms(cplx &acc, cplx a, cplx b) {
+  acc.x = fma(-a.x, b.x, acc.x);
+  acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(-a.x, b.y, acc.y);
+  acc.y = fma(-a.y, b.x, acc.y);
+}
+
+// ---------------------------------------------------------------- batched pointer addressing
+// A "batch" is ncells handles (each with its own workspace base) times `inner` equally strided matrices inside each
+// workspace.  blockIdx.z = cell * inner + i  ->  bases[cell] + off + i * stride   (units: complex elements).
+struct BatchRef {
+  const unsigned long long *bases;  // device array [ncells] of workspace base addresses; nullptr -> `single`
+  unsigned long long single;        // used when bases == nullptr
+  long long off;                    // element offset inside the workspace
+  long long stride;                 // element stride between inner matrices
+};
+__device__ __forceinline__ cplx *batch_ptr(const BatchRef &r, int cell, int i) {
+  unsigned long long b = r.bases ? r.bases[cell] : r.single;
+  return reinterpret_cast<cplx *>(b) + r.off + (long long)i * r.stride;
+}
+
+// ---------------------------------------------------------------- kernels' host launchers (one per .cu)
+namespace bsk {
+
+struct Geometry {  // device pointers, per cell
+  const double *edge;   // SoA [6][nedge]: mh1, mh2 (fractional midpoint), eh1, eh2 (fractional edge), ex, ey (Cartesian edge)
+  const int *ephase;    // [nedge] phase of each edge
+  const double *w;      // [7][P] channel weights: Dv11 Dv22 Dv12 Dv13 Dv23 Dv33 rho
+  const double *area;   // [P]
+  int nedge, P;
+  double Q[4];          // rows q^1, q^2 (Cartesian)
+};
+
+// S1: table[c][(D1+2Mt)*(4Mt+1) + (D2+2Mt)], c < 7.  geo: device array [ncells]; table at BatchRef (inner unused).
+void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, cudaStream_t s);
+// S2: Phi (3N x 3N full) and R (N x N full) from the table.
+void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s);
+
+struct GemmDesc {
+  int M, N, K, opA, opB, lda, ldb, ldc, flags, inner, ncells;
+  cplx alpha, beta;
+  BatchRef A, B, C;
+};
+void launch_zgemm(const GemmDesc &g, cudaStream_t s);
+
+// S3 pieces.  A: n x n (lda) lower Cholesky in place; X = L^{-1}; tmp same shape as A; dinv: ceil(n/64) blocks of 64x64.
+// info: device int per (cell*inner).  Returns number of kernel launches issued.
+int potrf_trtri(int n, int lda, BatchRef A, BatchRef X, BatchRef tmp, BatchRef dinv, int *info, long long info_stride_unused,
+                int ncells, int inner, cudaStream_t s);
+void launch_copy_matrix(int rows, int cols, BatchRef src, int lds, BatchRef dst, int ldd, int ncells, int inner,
+                        cudaStream_t s);
+void launch_hermitian_fill_upper(int n, BatchRef A, int lda, int ncells, int inner, cudaStream_t s);
+
+// S4: K = V^2 sum_t Btilde(kL_t)^T Y Btilde(kR_t), nterm <= 2.  kvec: device doubles,
+// per output matrix z (= cell*inner + i): [nterm][2 (L,R)][2 (x,y)][N] at kvec + z*kvec_stride.
+void launch_pencil(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk, const double *kvec, long long kvec_stride,
+                   int nterm, int ncells, int inner, cudaStream_t s);
+// A(k) = sum_i c_i(k) Coef_i, lower triangle (by 64-tiles) only.  coef: [ncells*nk][6] doubles.
+void launch_combine(int n, BatchRef Coef, long long coef_mat_stride, BatchRef Ak, int ld, const double *coefk, int nk,
+                    int ncells, cudaStream_t s);
+
+// S6: tridiagonalisation.  vw: per matrix 2*n*nb complex.  d,e: per matrix n doubles at d + z*n.
+size_t tridiag_smem_bytes(int n, int nb);
+void launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, double *d, double *e, int ncells, int inner,
+                    cudaStream_t s);
+// S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
+void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s);
+
+}  // namespace bsk

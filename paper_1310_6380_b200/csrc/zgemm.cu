@@ -1,0 +1,159 @@
+// Batched complex128 GEMM on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> DMMA on sm_100a; tcgen05 has no f64 kind).
+// C = alpha op(A) op(B) + beta C, column-major interleaved complex.  A complex product is four real DMMAs on the
+// (re,im) parts kept interleaved in shared memory (one LDS.128 fetches both).  DESIGN.md section 5 (zgemm).
+#include "bs_internal.cuh"
+
+namespace bsk {
+
+namespace {
+constexpr int BM = 64, BN = 64, BK = 8, STAGES = 4, LDS = 66;  // LDS: padded row stride (conflict-free fragment loads)
+constexpr int NT = 256;
+constexpr size_t kSmem = (size_t)STAGES * BK * LDS * sizeof(cplx) * 2;
+
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+  const int sz = valid ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+__device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+
+template <int OPA, int OPB>
+__global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx(*As)[BK][LDS] = reinterpret_cast<cplx(*)[BK][LDS]>(smem_raw);
+  cplx(*Bs)[BK][LDS] = reinterpret_cast<cplx(*)[BK][LDS]>(smem_raw + (size_t)STAGES * BK * LDS * sizeof(cplx));
+
+  const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+  if ((g.flags & BS_GEMM_LOWER_ONLY) && n0 >= m0 + BM) return;
+  const int cell = blockIdx.z / g.inner, bi = blockIdx.z % g.inner;
+  const cplx *__restrict__ A = batch_ptr(g.A, cell, bi);
+  const cplx *__restrict__ B = batch_ptr(g.B, cell, bi);
+  cplx *C = batch_ptr(g.C, cell, bi);
+
+  int klo = 0, khi = g.K;
+  if (g.flags & BS_GEMM_KLO_ROW) klo = max(klo, m0);
+  if (g.flags & BS_GEMM_KHI_ROW) khi = min(khi, m0 + BM);
+  if (g.flags & BS_GEMM_KLO_COL) klo = max(klo, n0);
+  if (g.flags & BS_GEMM_KHI_COL) khi = min(khi, n0 + BN);
+  klo &= ~(BK - 1);
+  const int nkt = khi > klo ? (khi - klo + BK - 1) / BK : 0;
+
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int wm = warp & 3, wn = warp >> 2;  // 4 x 2 warps; warp tile 16 x 32
+
+  auto load_tile = [&](int kt, int stage) {
+    const int k0 = klo + kt * BK;
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      int m, k;
+      if (OPA == 0) { m = t & 63; k = (t >> 6) + 4 * r; } else { k = t & 7; m = (t >> 3) + 32 * r; }
+      const bool ok = (m0 + m < g.M) && (k0 + k < khi);
+      const cplx *src = OPA == 0 ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
+                                 : A + (size_t)(k0 + k) + (size_t)(m0 + m) * g.lda;
+      cp_async16(&As[stage][k][m], ok ? src : A, ok);
+    }
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+      int n, k;
+      if (OPB == 0) { k = t & 7; n = (t >> 3) + 32 * r; } else { n = t & 63; k = (t >> 6) + 4 * r; }
+      const bool ok = (n0 + n < g.N) && (k0 + k < khi);
+      const cplx *src = OPB == 0 ? B + (size_t)(k0 + k) + (size_t)(n0 + n) * g.ldb
+                                 : B + (size_t)(n0 + n) + (size_t)(k0 + k) * g.ldb;
+      cp_async16(&Bs[stage][k][n], ok ? src : B, ok);
+    }
+  };
+
+  double cr[2][4][2], ci[2][4][2];
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s) {
+    if (s < nkt) load_tile(s, s);
+    cp_commit();
+  }
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_wait<STAGES - 2>();
+    __syncthreads();
+    if (kt + STAGES - 1 < nkt) load_tile(kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
+    cp_commit();
+    const int st = kt % STAGES;
+#pragma unroll
+    for (int kk = 0; kk < BK; kk += 4) {
+      cplx a[2], b[4];
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) {
+        a[mi] = As[st][kk + (lane & 3)][wm * 16 + mi * 8 + (lane >> 2)];
+        if (OPA) a[mi].y = -a[mi].y;
+      }
+#pragma unroll
+      for (int ni = 0; ni < 4; ++ni) {
+        b[ni] = Bs[st][kk + (lane & 3)][wn * 32 + ni * 8 + (lane >> 2)];
+        if (OPB) b[ni].y = -b[ni].y;
+      }
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) {
+        const double nai = -a[mi].y;
+#pragma unroll
+        for (int ni = 0; ni < 4; ++ni) {
+          dmma(cr[mi][ni][0], cr[mi][ni][1], a[mi].x, b[ni].x);
+          dmma(cr[mi][ni][0], cr[mi][ni][1], nai, b[ni].y);
+          dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].x, b[ni].y);
+          dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].y, b[ni].x);
+        }
+      }
+    }
+  }
+  cp_wait<0>();
+
+  const bool has_beta = (g.beta.x != 0.0 || g.beta.y != 0.0);
+  const bool lower = g.flags & BS_GEMM_LOWER_ONLY;
+#pragma unroll
+  for (int mi = 0; mi < 2; ++mi) {
+    const int row = m0 + wm * 16 + mi * 8 + (lane >> 2);
+    if (row >= g.M) continue;
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
+        if (col >= g.N || (lower && col > row)) continue;
+        cplx v = cmul(g.alpha, cmake(cr[mi][ni][j], ci[mi][ni][j]));
+        cplx *dst = C + (size_t)row + (size_t)col * g.ldc;
+        if (has_beta) v = cadd(v, cmul(g.beta, *dst));
+        *dst = v;
+      }
+    }
+  }
+}
+}  // namespace
+
+void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
+  if (g.M <= 0 || g.N <= 0 || g.ncells * g.inner <= 0) return;
+  dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(zgemm_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    attr_done = true;
+  }
+  if (g.opA == 0 && g.opB == 0) zgemm_kernel<0, 0><<<grid, NT, kSmem, s>>>(g);
+  else if (g.opA == 0 && g.opB == 1) zgemm_kernel<0, 1><<<grid, NT, kSmem, s>>>(g);
+  else if (g.opA == 1 && g.opB == 0) zgemm_kernel<1, 0><<<grid, NT, kSmem, s>>>(g);
+  else zgemm_kernel<1, 1><<<grid, NT, kSmem, s>>>(g);
+}
+
+}  // namespace bsk

@@ -146,9 +146,12 @@ bs_status bs_zgemm(int32_t opA, int32_t opB, int32_t M, int32_t N, int32_t K, co
  * info: DEVICE int32[batch] (0 = ok, else 1-based failing pivot). */
 bs_status bs_zpotrf_trtri(int32_t n, void *A, int32_t lda, int64_t strideA, void *X, void *tmp, void *dinv,
                           int32_t *info, int32_t batch, void *stream);
-/* Householder tridiagonalisation of `batch` n x n Hermitian DEVICE matrices (lower triangle read, destroyed).
- * d, e: DEVICE, batch x n doubles.  vw: DEVICE scratch, batch*2*n*nb complex. */
-bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *vw, int32_t nb,
+/* Householder tridiagonalisation of `batch` n x n Hermitian DEVICE matrices (lower triangle read; trailing blocks are
+ * overwritten), n <= 2048, Q^H A Q = T real symmetric tridiagonal (eigenvalues of the pencil).
+ * d, e: DEVICE, batch x n doubles (e[.][n-1] unused).  scratch: DEVICE, batch * bs_zhetrd_scratch_elems(n, nb) complex128
+ * elements.  nb: panel width (clamped to 4..32).  Synchronises the stream before returning. */
+size_t bs_zhetrd_scratch_elems(int32_t n, int32_t nb);
+bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *scratch, int32_t nb,
                     int32_t batch, void *stream);
 /* Lowest nev eigenvalues of `batch` real symmetric tridiagonal matrices (d, e: DEVICE, batch x n) by Sturm bisection;
  * lam: DEVICE, batch x nev, ascending. */

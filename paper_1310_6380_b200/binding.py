@@ -1,0 +1,274 @@
+"""ctypes binding of ``libbs.so`` (C-ABI in ``include/bs.h``): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C calls.  PyTorch supplies device memory (the workspace
+tensor lent to the handle) and the stream.  There is no CPU fallback: importing this module without a built
+``libbs.so`` raises, and every compute call fails with ``BsError`` when there is no CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libbs.so")
+
+BS_OK, BS_ERR_ARG, BS_ERR_GEOMETRY, BS_ERR_NOT_PD, BS_ERR_STATE, BS_ERR_CUDA, BS_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
+BS_OPT_PENCIL_MODE, BS_OPT_PANEL, BS_OPT_TIMING = 0, 1, 2
+BS_PENCIL_POLY, BS_PENCIL_DIRECT = 0, 1
+BS_T_TABLE, BS_T_EXPAND, BS_T_FACTOR, BS_T_COEF, BS_T_PENCIL, BS_T_TRIDIAG, BS_T_BISECT, BS_T_COUNT = 0, 1, 2, 3, 4, 5, 6, 8
+BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_KHI_COL = 1, 2, 4, 8, 16
+
+# every symbol include/bs.h declares (tests check that the library exports all of them)
+SYMBOLS = [
+    "bs_isotropic_plane_strain", "bs_create_cell", "bs_destroy_cell", "bs_set_option", "bs_workspace_bytes",
+    "bs_set_workspace", "bs_assemble", "bs_assemble_batch", "bs_get_matrices", "bs_get_table", "bs_get_pencil",
+    "bs_bands", "bs_bands_batch", "bs_get_tridiagonal", "bs_get_timings", "bs_launch_count", "bs_last_error",
+    "bs_zgemm", "bs_zpotrf_trtri", "bs_zhetrd_scratch_elems", "bs_zhetrd", "bs_sturm",
+]
+
+
+class BsError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"bs status {status}: {message}")
+        self.status = status
+
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1310_6380_b200.build` "
+                      "(there is no CPU fallback)")
+lib = C.CDLL(LIB_PATH)
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+_vp = C.c_void_p
+lib.bs_last_error.restype = C.c_char_p
+lib.bs_launch_count.restype = C.c_int64
+lib.bs_launch_count.argtypes = [_vp]
+lib.bs_zhetrd_scratch_elems.restype = C.c_size_t
+lib.bs_zhetrd_scratch_elems.argtypes = [C.c_int32, C.c_int32]
+lib.bs_destroy_cell.restype = None
+lib.bs_destroy_cell.argtypes = [_vp]
+lib.bs_isotropic_plane_strain.argtypes = [C.c_int32, _dp, _dp, _dp]
+lib.bs_create_cell.argtypes = [_dp, C.c_int32, _ip, _dp, _dp, _dp, C.POINTER(_vp)]
+lib.bs_set_option.argtypes = [_vp, C.c_int32, C.c_int32]
+lib.bs_workspace_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
+lib.bs_set_workspace.argtypes = [_vp, _vp, C.c_size_t]
+lib.bs_assemble.argtypes = [_vp, C.c_int32, _vp]
+lib.bs_assemble_batch.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int32, _vp]
+lib.bs_get_matrices.argtypes = [_vp, _vp, _vp]
+lib.bs_get_table.argtypes = [_vp, _vp]
+lib.bs_get_pencil.argtypes = [_vp, _dp, _vp, _vp]
+lib.bs_bands.argtypes = [_vp, C.c_int32, _dp, C.c_int32, _vp, _vp]
+lib.bs_bands_batch.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int32, _dp, C.c_int32, _vp, _vp]
+lib.bs_get_tridiagonal.argtypes = [_vp, _dp, _dp]
+lib.bs_get_timings.argtypes = [_vp, _dp]
+lib.bs_zgemm.argtypes = [C.c_int32] * 5 + [_dp, _vp, C.c_int32, C.c_int64, _vp, C.c_int32, C.c_int64, _dp, _vp, C.c_int32,
+                                           C.c_int64, C.c_int32, C.c_int32, _vp]
+lib.bs_zpotrf_trtri.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, _vp, C.c_int32, _vp]
+lib.bs_zhetrd.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, _vp]
+lib.bs_sturm.argtypes = [C.c_int32, _vp, _vp, C.c_int32, _vp, C.c_int32, _vp]
+for _name in SYMBOLS:
+    if _name not in ("bs_last_error", "bs_launch_count", "bs_zhetrd_scratch_elems", "bs_destroy_cell"):
+        getattr(lib, _name).restype = C.c_int
+
+
+def _check(status: int) -> None:
+    if status != BS_OK:
+        raise BsError(status, (lib.bs_last_error() or b"").decode())
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def _ptr(a: np.ndarray, typ=_dp):
+    return a.ctypes.data_as(typ)
+
+
+def _stream(stream) -> Optional[int]:
+    """cudaStream_t of a torch stream (None -> torch's current stream)."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def bs_isotropic_plane_strain(E, nu) -> np.ndarray:
+    """PAPER.md:121 (eq. 14).  Returns (n,6) [D1111 D2222 D1122 D1112 D2212 D1212]."""
+    E, nu = _f64(E).ravel(), _f64(nu).ravel()
+    out = np.empty((E.shape[0], 6))
+    _check(lib.bs_isotropic_plane_strain(E.shape[0], _ptr(E), _ptr(nu), _ptr(out)))
+    return out
+
+
+class Cell:
+    """Owner of one ``bs_cell`` handle and of the torch workspace tensor lent to it."""
+
+    def __init__(self, lattice, vert_offset, verts, compliance, density):
+        lattice = _f64(lattice).reshape(4)
+        off = np.ascontiguousarray(np.asarray(vert_offset, dtype=np.int32))
+        verts = _f64(verts).reshape(-1)
+        compliance = _f64(compliance).reshape(-1)
+        density = _f64(density).reshape(-1)
+        self.nphase = int(off.shape[0] - 1)
+        if compliance.shape[0] != 6 * self.nphase or density.shape[0] != self.nphase or verts.shape[0] != 2 * int(off[-1]):
+            raise BsError(BS_ERR_ARG, "array sizes do not match nphase / vert_offset")
+        h = _vp()
+        _check(lib.bs_create_cell(_ptr(lattice), self.nphase, _ptr(off, _ip), _ptr(verts), _ptr(compliance),
+                                  _ptr(density), C.byref(h)))
+        self.handle = h
+        self.workspace = None
+        self.Mt = None
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib.bs_destroy_cell(self.handle)
+            self.handle = None
+            self.workspace = None
+
+    def __del__(self):
+        self.close()
+
+    @property
+    def N(self) -> int:
+        return (2 * self.Mt + 1) ** 2
+
+
+def bs_create_cell(lattice, vert_offset, verts, compliance, density) -> Cell:
+    return Cell(lattice, vert_offset, verts, compliance, density)
+
+
+def bs_destroy_cell(cell: Cell) -> None:
+    cell.close()
+
+
+def bs_set_option(cell: Cell, option: int, value: int) -> None:
+    _check(lib.bs_set_option(cell.handle, option, value))
+
+
+def bs_workspace_bytes(cell: Cell, truncation: int, nk: int) -> int:
+    b = C.c_size_t(0)
+    _check(lib.bs_workspace_bytes(cell.handle, truncation, nk, C.byref(b)))
+    return int(b.value)
+
+
+def bs_set_workspace(cell: Cell, tensor) -> None:
+    """Lend a torch uint8 CUDA tensor (kept alive by the Cell)."""
+    _check(lib.bs_set_workspace(cell.handle, C.c_void_p(tensor.data_ptr()), tensor.numel() * tensor.element_size()))
+    cell.workspace = tensor
+
+
+def allocate_workspace(cell: Cell, truncation: int, nk: int, device="cuda:0") -> None:
+    import torch
+    nbytes = bs_workspace_bytes(cell, truncation, nk)
+    bs_set_workspace(cell, torch.empty(nbytes, dtype=torch.uint8, device=device))
+
+
+def bs_assemble(cell: Cell, truncation: int, stream=None) -> None:
+    _check(lib.bs_assemble(cell.handle, truncation, _stream(stream)))
+    cell.Mt = truncation
+
+
+def _handles(cells: Sequence[Cell]):
+    arr = (_vp * len(cells))(*[c.handle for c in cells])
+    return arr
+
+
+def bs_assemble_batch(cells: Sequence[Cell], truncation: int, stream=None) -> None:
+    _check(lib.bs_assemble_batch(_handles(cells), len(cells), truncation, _stream(stream)))
+    for c in cells:
+        c.Mt = truncation
+
+
+def bs_get_matrices(cell: Cell):
+    """Phi (3N,3N) and Psi (2N,2N) as NumPy complex128 arrays (row index = test function)."""
+    N = cell.N
+    phi = np.empty((3 * N, 3 * N), dtype=np.complex128, order="F")
+    psi = np.empty((2 * N, 2 * N), dtype=np.complex128, order="F")
+    _check(lib.bs_get_matrices(cell.handle, phi.ctypes.data_as(_vp), psi.ctypes.data_as(_vp)))
+    return phi, psi
+
+
+def bs_get_table(cell: Cell) -> np.ndarray:
+    L = 4 * cell.Mt + 1
+    tab = np.empty((7, L, L), dtype=np.complex128)
+    _check(lib.bs_get_table(cell.handle, tab.ctypes.data_as(_vp)))
+    return tab
+
+
+def bs_get_pencil(cell: Cell, kred, stream=None) -> np.ndarray:
+    n = 2 * cell.N
+    K = np.empty((n, n), dtype=np.complex128, order="F")
+    k = _f64(kred).reshape(2)
+    _check(lib.bs_get_pencil(cell.handle, _ptr(k), K.ctypes.data_as(_vp), _stream(stream)))
+    return K
+
+
+def bs_bands(cell: Cell, kpts, nbands: int, out=None, stream=None):
+    """omega^2 (nk, nbands), ascending.  ``out``: None -> new host NumPy array; a NumPy array (host) or a torch CUDA
+    float64 tensor (device) is filled in place and returned."""
+    k = _f64(kpts).reshape(-1, 2)
+    nk = k.shape[0]
+    if out is None:
+        out = np.empty((nk, nbands))
+    p = C.c_void_p(out.ctypes.data) if isinstance(out, np.ndarray) else C.c_void_p(out.data_ptr())
+    _check(lib.bs_bands(cell.handle, nk, _ptr(k), nbands, p, _stream(stream)))
+    return out
+
+
+def bs_bands_batch(cells: Sequence[Cell], kpts, nbands: int, out=None, stream=None):
+    k = _f64(kpts).reshape(-1, 2)
+    nk = k.shape[0]
+    if out is None:
+        out = np.empty((len(cells), nk, nbands))
+    p = C.c_void_p(out.ctypes.data) if isinstance(out, np.ndarray) else C.c_void_p(out.data_ptr())
+    _check(lib.bs_bands_batch(_handles(cells), len(cells), nk, _ptr(k), nbands, p, _stream(stream)))
+    return out
+
+
+def bs_get_tridiagonal(cell: Cell, nmat: int):
+    n = 2 * cell.N
+    d = np.empty((nmat, n))
+    e = np.empty((nmat, n))
+    _check(lib.bs_get_tridiagonal(cell.handle, _ptr(d), _ptr(e)))
+    return d, e
+
+
+def bs_get_timings(cell: Cell) -> np.ndarray:
+    ms = np.zeros(BS_T_COUNT)
+    _check(lib.bs_get_timings(cell.handle, _ptr(ms)))
+    return ms
+
+
+def bs_launch_count(cell: Cell) -> int:
+    return int(lib.bs_launch_count(cell.handle))
+
+
+# ---- diagnostics on torch CUDA tensors (complex128, column-major = the transpose of a contiguous torch tensor)
+def bs_zgemm(opA, opB, M, N, K, alpha, A, lda, strideA, B, ldb, strideB, beta, Cm, ldc, strideC, batch=1, flags=0, stream=None):
+    al = np.array([complex(alpha).real, complex(alpha).imag])
+    be = np.array([complex(beta).real, complex(beta).imag])
+    _check(lib.bs_zgemm(opA, opB, M, N, K, _ptr(al), C.c_void_p(A.data_ptr()), lda, strideA, C.c_void_p(B.data_ptr()), ldb,
+                        strideB, _ptr(be), C.c_void_p(Cm.data_ptr()), ldc, strideC, batch, flags, _stream(stream)))
+
+
+def bs_zpotrf_trtri(n, A, lda, strideA, X, tmp, dinv, info, batch=1, stream=None):
+    _check(lib.bs_zpotrf_trtri(n, C.c_void_p(A.data_ptr()), lda, strideA, C.c_void_p(X.data_ptr()), C.c_void_p(tmp.data_ptr()),
+                               C.c_void_p(dinv.data_ptr()), C.c_void_p(info.data_ptr()), batch, _stream(stream)))
+
+
+def bs_zhetrd_scratch_elems(n: int, nb: int) -> int:
+    return int(lib.bs_zhetrd_scratch_elems(n, nb))
+
+
+def bs_zhetrd(n, A, lda, strideA, d, e, scratch, nb=32, batch=1, stream=None):
+    _check(lib.bs_zhetrd(n, C.c_void_p(A.data_ptr()), lda, strideA, C.c_void_p(d.data_ptr()), C.c_void_p(e.data_ptr()),
+                         C.c_void_p(scratch.data_ptr()), nb, batch, _stream(stream)))
+
+
+def bs_sturm(n, d, e, nev, lam, batch=1, stream=None):
+    _check(lib.bs_sturm(n, C.c_void_p(d.data_ptr()), C.c_void_p(e.data_ptr()), nev, C.c_void_p(lam.data_ptr()), batch,
+                        _stream(stream)))

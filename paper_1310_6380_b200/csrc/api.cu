@@ -1,0 +1,725 @@
+// C-ABI of libbs.so (include/bs.h): handle, workspace layout and the host-side orchestration of S0..S8.
+// Every arithmetic step of the path runs in the kernels of assemble.cu / factor.cu / zgemm.cu / pencil.cu / tridiag.cu /
+// sturm.cu; the host only does S0 (geometry preparation) and argument marshalling.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "bs_internal.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+bs_status fail(bs_status st, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+#define CU(expr)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (expr);                                                                       \
+    if (e_ != cudaSuccess) return fail(BS_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_));      \
+  } while (0)
+
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+
+// Offsets (complex128 elements, each region 256-byte aligned) inside one cell's workspace.
+struct Layout {
+  int Mt = -1, N = 0, nk = 0, mode = 0, nb = 32;
+  long long table, Phi, R, Lf, X, tmp, dinv, Y, LR, XR, tmpR, dinvR, kvecA, Coef, Tb, kvecK, Kk, Ak, VW, P;
+  long long total;  // elements
+};
+
+long long align16(long long x) { return (x + 15) & ~15LL; }
+
+Layout make_layout(int Mt, int nk, int mode, int nb) {
+  Layout L;
+  L.Mt = Mt; L.nk = nk; L.mode = mode; L.nb = nb;
+  const long long W = 2 * Mt + 1, N = W * W, n3 = 3 * N, n2 = 2 * N, Lt = 4 * Mt + 1;
+  L.N = (int)N;
+  long long o = 0;
+  auto take = [&](long long elems) { long long at = o; o = align16(o + elems); return at; };
+  L.table = take(7 * Lt * Lt);
+  L.Phi = take(n3 * n3);
+  L.R = take(N * N);
+  L.Lf = take(n3 * n3);
+  L.X = take(n3 * n3);
+  L.tmp = take(n3 * n3);
+  L.dinv = take(((n3 + 63) / 64) * 4096);
+  L.Y = take(n3 * n3);
+  L.LR = take(N * N);
+  L.XR = take(N * N);
+  L.tmpR = take(N * N);
+  L.dinvR = take(((N + 63) / 64) * 4096);
+  L.kvecA = take(6 * 2 * 2 * N);      // 6 matrices x 2 terms x [2][2][N] doubles
+  L.Coef = take(mode == BS_PENCIL_POLY ? 6 * n2 * n2 : 0);
+  L.Tb = take((mode == BS_PENCIL_POLY ? 6 : (long long)nk) * N * N);
+  L.kvecK = take((long long)nk * 2 * N);  // nk x [2][2][N] doubles
+  L.Kk = take(mode == BS_PENCIL_DIRECT ? (long long)nk * n2 * n2 : n2 * n2);  // POLY keeps one slot for bs_get_pencil
+  L.Ak = take((long long)nk * n2 * n2);
+  L.VW = take((long long)nk * (long long)bsk::tridiag_vw_elems((int)n2, nb));
+  L.P = take((long long)nk * (long long)bsk::tridiag_p_elems((int)n2));
+  L.total = o;
+  return L;
+}
+
+}  // namespace
+
+struct bs_cell {
+  double A[4], T[4], Q[4], V;
+  int P = 0, nedge = 0;
+  double *d_edge = nullptr, *d_w = nullptr, *d_area = nullptr;
+  int *d_ephase = nullptr;
+  bsk::Geometry geo;
+  bsk::Geometry *d_geo = nullptr;  // [1]
+  int mode = BS_PENCIL_POLY, nb = 32, timing = 0;
+  void *ws = nullptr;
+  size_t ws_bytes = 0;
+  Layout lay;            // layout of the last bs_assemble (lay.Mt < 0: not assembled)
+  int ws_nk = 0;         // nk the caller sized the workspace for (unknown: derived from bytes at assemble time)
+  bool assembled = false;
+  int64_t launches = 0;
+  double ms[BS_T_COUNT] = {0};
+  // batch scratch owned by the handle that leads a call (cells[0])
+  unsigned long long *d_bases = nullptr;
+  bsk::Geometry *d_geos = nullptr;
+  int *d_info = nullptr;
+  int batch_cap = 0;
+  double *d_flat = nullptr;  // d, e, scal, lam, coefk
+  size_t flat_cap = 0;
+  int last_n = 0, last_nmat = 0, last_nk = 0;
+  cudaEvent_t ev[BS_T_COUNT + 1] = {nullptr};
+};
+
+namespace {
+
+BatchRef ref(const bs_cell *lead, int ncells, bs_cell *const *cells, long long off, long long stride) {
+  BatchRef r;
+  r.bases = ncells > 1 ? lead->d_bases : nullptr;
+  r.single = (unsigned long long)cells[0]->ws;
+  r.off = off;
+  r.stride = stride;
+  return r;
+}
+
+bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStream_t s) {
+  if (ncells > lead->batch_cap) {
+    if (lead->d_bases) cudaFree(lead->d_bases);
+    if (lead->d_geos) cudaFree(lead->d_geos);
+    if (lead->d_info) cudaFree(lead->d_info);
+    lead->d_bases = nullptr; lead->d_geos = nullptr; lead->d_info = nullptr; lead->batch_cap = 0;
+    CU(cudaMalloc(&lead->d_bases, sizeof(unsigned long long) * ncells));
+    CU(cudaMalloc(&lead->d_geos, sizeof(bsk::Geometry) * ncells));
+    CU(cudaMalloc(&lead->d_info, sizeof(int) * 2 * ncells));
+    lead->batch_cap = ncells;
+  }
+  std::vector<unsigned long long> b(ncells);
+  std::vector<bsk::Geometry> g(ncells);
+  for (int c = 0; c < ncells; ++c) {
+    b[c] = (unsigned long long)cells[c]->ws;
+    g[c] = cells[c]->geo;
+  }
+  CU(cudaMemcpyAsync(lead->d_bases, b.data(), sizeof(unsigned long long) * ncells, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(lead->d_geos, g.data(), sizeof(bsk::Geometry) * ncells, cudaMemcpyHostToDevice, s));
+  CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
+  return BS_OK;
+}
+
+bs_status ensure_flat(bs_cell *lead, size_t doubles) {
+  if (doubles > lead->flat_cap) {
+    if (lead->d_flat) cudaFree(lead->d_flat);
+    lead->d_flat = nullptr; lead->flat_cap = 0;
+    CU(cudaMalloc(&lead->d_flat, doubles * sizeof(double)));
+    lead->flat_cap = doubles;
+  }
+  return BS_OK;
+}
+
+void tick(bs_cell *c, int idx, cudaStream_t s) {
+  if (!c->timing) return;
+  if (!c->ev[idx]) cudaEventCreate(&c->ev[idx]);
+  cudaEventRecord(c->ev[idx], s);
+}
+double tock(bs_cell *c, int a, int b) {
+  float ms = 0.f;
+  if (c->ev[a] && c->ev[b]) cudaEventElapsedTime(&ms, c->ev[a], c->ev[b]);
+  return ms;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *bs_last_error(void) { return g_err; }
+
+bs_status bs_isotropic_plane_strain(int32_t n, const double *E, const double *nu, double *out) {
+  if (n < 0 || (n > 0 && (!E || !nu || !out))) return fail(BS_ERR_ARG, "bs_isotropic_plane_strain: null pointer or n < 0");
+  for (int i = 0; i < n; ++i) {
+    if (!(E[i] > 0.0) || !(nu[i] < 0.5) || !(nu[i] > -1.0))
+      return fail(BS_ERR_ARG, "bs_isotropic_plane_strain: phase %d has E <= 0 or nu outside (-1, 0.5)", i);
+    // PAPER.md:121 (eq. 14): D_jkmn = (1/2mu) [ (d_jm d_kn + d_jn d_km)/2 - lam/(2(mu+lam)) d_jk d_mn ]
+    const double mu = E[i] / (2.0 * (1.0 + nu[i]));
+    const double lam = E[i] * nu[i] / ((1.0 + nu[i]) * (1.0 - 2.0 * nu[i]));
+    const double c = lam / (2.0 * (mu + lam)), h = 1.0 / (2.0 * mu);
+    double *o = out + 6 * (size_t)i;
+    o[0] = h * (1.0 - c);  // D1111
+    o[1] = o[0];           // D2222
+    o[2] = -h * c;         // D1122
+    o[3] = 0.0;            // D1112
+    o[4] = 0.0;            // D2212
+    o[5] = 0.5 * h;        // D1212
+  }
+  return BS_OK;
+}
+
+bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
+                         const double *compliance, const double *density, bs_cell **out) {
+  if (!lattice || !vert_offset || !verts || !compliance || !density || !out || nphase < 1)
+    return fail(BS_ERR_ARG, "bs_create_cell: null pointer or nphase < 1");
+  *out = nullptr;
+  if (vert_offset[0] != 0) return fail(BS_ERR_ARG, "bs_create_cell: vert_offset[0] != 0");
+  for (int p = 0; p < nphase; ++p)
+    if (vert_offset[p + 1] - vert_offset[p] < 3) return fail(BS_ERR_ARG, "bs_create_cell: phase %d has < 3 vertices", p);
+  const double det = lattice[0] * lattice[3] - lattice[1] * lattice[2];
+  if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return fail(BS_ERR_GEOMETRY, "bs_create_cell: singular lattice");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(BS_ERR_CUDA, "bs_create_cell: no CUDA device");
+
+  bs_cell *c = new (std::nothrow) bs_cell();
+  if (!c) return fail(BS_ERR_NOMEM, "bs_create_cell: host allocation failed");
+  std::memcpy(c->A, lattice, sizeof(double) * 4);
+  // T = A^{-1}; q^j = 2 pi (column j of T)  =>  q^i . h^j = 2 pi delta_ij   (PAPER.md:23-26 eq. 1, :138)
+  c->T[0] = lattice[3] / det;  c->T[1] = -lattice[1] / det;
+  c->T[2] = -lattice[2] / det; c->T[3] = lattice[0] / det;
+  c->Q[0] = kTwoPi * c->T[0]; c->Q[1] = kTwoPi * c->T[2];  // q^1
+  c->Q[2] = kTwoPi * c->T[1]; c->Q[3] = kTwoPi * c->T[3];  // q^2
+  c->V = std::fabs(det);
+  c->P = nphase;
+  const int ne = vert_offset[nphase];
+  c->nedge = ne;
+  std::vector<double> edge((size_t)6 * ne), area(nphase), w((size_t)7 * nphase);
+  std::vector<int> eph(ne);
+  double total = 0.0;
+  for (int p = 0; p < nphase; ++p) {
+    const int s = vert_offset[p], t = vert_offset[p + 1];
+    double a2 = 0.0;
+    for (int i = s; i < t; ++i) {
+      const int k = (i + 1 < t) ? i + 1 : s;
+      const double x0 = verts[2 * i], y0 = verts[2 * i + 1], x1 = verts[2 * k], y1 = verts[2 * k + 1];
+      a2 += x0 * y1 - x1 * y0;
+      const double ex = x1 - x0, ey = y1 - y0, mx = 0.5 * (x0 + x1), my = 0.5 * (y0 + y1);
+      // fractional coordinates H = x T  (x = H_1 h^1 + H_2 h^2)
+      edge[0 * (size_t)ne + i] = mx * c->T[0] + my * c->T[2];
+      edge[1 * (size_t)ne + i] = mx * c->T[1] + my * c->T[3];
+      edge[2 * (size_t)ne + i] = ex * c->T[0] + ey * c->T[2];
+      edge[3 * (size_t)ne + i] = ex * c->T[1] + ey * c->T[3];
+      edge[4 * (size_t)ne + i] = ex;
+      edge[5 * (size_t)ne + i] = ey;
+      eph[i] = p;
+    }
+    area[p] = 0.5 * a2;
+    if (!(area[p] > 0.0)) {
+      delete c;
+      return fail(BS_ERR_GEOMETRY, "bs_create_cell: phase %d has non-positive signed area %g (must be CCW)", p, area[p]);
+    }
+    total += area[p];
+    if (!(density[p] > 0.0)) {
+      delete c;
+      return fail(BS_ERR_ARG, "bs_create_cell: phase %d has density <= 0", p);
+    }
+    // Voigt weights with the factors 1/2/4 of PAPER.md:167-171 (eq. 20)
+    const double *D = compliance + 6 * (size_t)p;
+    w[0 * (size_t)nphase + p] = D[0];
+    w[1 * (size_t)nphase + p] = D[1];
+    w[2 * (size_t)nphase + p] = D[2];
+    w[3 * (size_t)nphase + p] = 2.0 * D[3];
+    w[4 * (size_t)nphase + p] = 2.0 * D[4];
+    w[5 * (size_t)nphase + p] = 4.0 * D[5];
+    w[6 * (size_t)nphase + p] = density[p];
+  }
+  if (std::fabs(total - c->V) > 1e-10 * c->V) {
+    delete c;
+    return fail(BS_ERR_GEOMETRY, "bs_create_cell: phases cover area %.17g, cell area is %.17g", total, c->V);
+  }
+  bs_status st = BS_OK;
+  auto up = [&](void **dst, const void *src, size_t bytes) {
+    if (st != BS_OK) return;
+    if (cudaMalloc(dst, bytes) != cudaSuccess || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess)
+      st = fail(BS_ERR_CUDA, "bs_create_cell: device allocation/copy failed: %s", cudaGetErrorString(cudaGetLastError()));
+  };
+  up((void **)&c->d_edge, edge.data(), sizeof(double) * edge.size());
+  up((void **)&c->d_ephase, eph.data(), sizeof(int) * eph.size());
+  up((void **)&c->d_w, w.data(), sizeof(double) * w.size());
+  up((void **)&c->d_area, area.data(), sizeof(double) * area.size());
+  c->geo.edge = c->d_edge; c->geo.ephase = c->d_ephase; c->geo.w = c->d_w; c->geo.area = c->d_area;
+  c->geo.nedge = ne; c->geo.P = nphase;
+  std::memcpy(c->geo.Q, c->Q, sizeof(double) * 4);
+  up((void **)&c->d_geo, &c->geo, sizeof(bsk::Geometry));
+  if (st != BS_OK) {
+    bs_destroy_cell(c);
+    return st;
+  }
+  *out = c;
+  return BS_OK;
+}
+
+void bs_destroy_cell(bs_cell *c) {
+  if (!c) return;
+  cudaFree(c->d_edge); cudaFree(c->d_ephase); cudaFree(c->d_w); cudaFree(c->d_area); cudaFree(c->d_geo);
+  cudaFree(c->d_bases); cudaFree(c->d_geos); cudaFree(c->d_info); cudaFree(c->d_flat);
+  for (auto &e : c->ev)
+    if (e) cudaEventDestroy(e);
+  delete c;
+}
+
+bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
+  if (!c) return fail(BS_ERR_ARG, "bs_set_option: null handle");
+  switch (option) {
+    case BS_OPT_PENCIL_MODE:
+      if (value != BS_PENCIL_POLY && value != BS_PENCIL_DIRECT) return fail(BS_ERR_ARG, "bs_set_option: bad pencil mode");
+      if (c->mode != value) c->assembled = false;
+      c->mode = value;
+      return BS_OK;
+    case BS_OPT_PANEL:
+      if (value < 4 || value > 32 || value % 4) return fail(BS_ERR_ARG, "bs_set_option: panel must be 4..32, multiple of 4");
+      if (c->nb != value) c->assembled = false;
+      c->nb = value;
+      return BS_OK;
+    case BS_OPT_TIMING:
+      c->timing = value ? 1 : 0;
+      return BS_OK;
+  }
+  return fail(BS_ERR_ARG, "bs_set_option: unknown option %d", option);
+}
+
+bs_status bs_workspace_bytes(const bs_cell *c, int32_t Mt, int32_t nk, size_t *bytes) {
+  if (!c || !bytes || Mt < 0 || nk < 1) return fail(BS_ERR_ARG, "bs_workspace_bytes: bad argument");
+  const long long n2 = 2LL * (2 * Mt + 1) * (2 * Mt + 1);
+  if (n2 > 2048) return fail(BS_ERR_ARG, "bs_workspace_bytes: 2N = %lld exceeds 2048", n2);
+  *bytes = (size_t)make_layout(Mt, nk, c->mode, c->nb).total * sizeof(cplx);
+  return BS_OK;
+}
+
+bs_status bs_set_workspace(bs_cell *c, void *dev_ptr, size_t bytes) {
+  if (!c || !dev_ptr) return fail(BS_ERR_ARG, "bs_set_workspace: null argument");
+  if (((uintptr_t)dev_ptr) & 255) return fail(BS_ERR_ARG, "bs_set_workspace: pointer not 256-byte aligned");
+  c->ws = dev_ptr;
+  c->ws_bytes = bytes;
+  c->assembled = false;
+  return BS_OK;
+}
+
+int64_t bs_launch_count(const bs_cell *c) { return c ? c->launches : 0; }
+
+bs_status bs_get_timings(bs_cell *c, double *ms_out) {
+  if (!c || !ms_out) return fail(BS_ERR_ARG, "bs_get_timings: null argument");
+  std::memcpy(ms_out, c->ms, sizeof(double) * BS_T_COUNT);
+  return BS_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// k-independent direction vectors of the bilinear scaling kernel for the six coefficient matrices of
+//   K(k) = V^2 Bt(G + k)^T Y Bt(G + k) = C0 + kx C1 + ky C2 + kx^2 C3 + kx ky C4 + ky^2 C5     (S4)
+// layout per matrix: [2 terms][L,R][x,y][N] doubles.
+void fill_coef_kvec(const bs_cell *c, int Mt, std::vector<double> &kv) {
+  const int W = 2 * Mt + 1, N = W * W;
+  kv.assign((size_t)6 * 8 * N, 0.0);
+  std::vector<double> Gx(N), Gy(N);
+  for (int a1 = -Mt; a1 <= Mt; ++a1)
+    for (int a2 = -Mt; a2 <= Mt; ++a2) {
+      const int g = (a1 + Mt) * W + (a2 + Mt);  // PAPER.md:150 (0-based)
+      Gx[g] = a1 * c->Q[0] + a2 * c->Q[2];
+      Gy[g] = a1 * c->Q[1] + a2 * c->Q[3];
+    }
+  // vec kinds: 0 = G, 1 = ex (1,0), 2 = ey (0,1)
+  const int terms[6][2][2] = {{{0, 0}, {-1, -1}}, {{0, 1}, {1, 0}}, {{0, 2}, {2, 0}},
+                              {{1, 1}, {-1, -1}}, {{1, 2}, {2, 1}}, {{2, 2}, {-1, -1}}};
+  for (int m = 0; m < 6; ++m)
+    for (int t = 0; t < 2; ++t)
+      for (int side = 0; side < 2; ++side) {
+        const int kind = terms[m][t][side];
+        if (kind < 0) continue;
+        double *x = &kv[(((size_t)m * 2 + t) * 2 + side) * 2 * N], *y = x + N;
+        for (int g = 0; g < N; ++g) {
+          x[g] = kind == 0 ? Gx[g] : (kind == 1 ? 1.0 : 0.0);
+          y[g] = kind == 0 ? Gy[g] : (kind == 2 ? 1.0 : 0.0);
+        }
+      }
+}
+
+// kappa_g = k + G_g for every k-point: [nk][L,R][x,y][N] doubles (L = R).
+void fill_direct_kvec(const bs_cell *c, int Mt, int nk, const double *kpts, std::vector<double> &kv) {
+  const int W = 2 * Mt + 1, N = W * W;
+  kv.assign((size_t)nk * 4 * N, 0.0);
+  for (int k = 0; k < nk; ++k)
+    for (int a1 = -Mt; a1 <= Mt; ++a1)
+      for (int a2 = -Mt; a2 <= Mt; ++a2) {
+        const int g = (a1 + Mt) * W + (a2 + Mt);
+        const double f1 = kpts[2 * k] + a1, f2 = kpts[2 * k + 1] + a2;  // PAPER.md:133-138 (eq. 16): Q + alpha
+        const double kx = f1 * c->Q[0] + f2 * c->Q[2], ky = f1 * c->Q[1] + f2 * c->Q[3];
+        double *b = &kv[(size_t)k * 4 * N];
+        b[g] = kx; b[N + g] = ky; b[2 * N + g] = kx; b[3 * N + g] = ky;
+      }
+}
+
+// S5 on `inner` matrices per cell: A_jl = X_R K_jl X_R^H for the blocks (0,0), (1,0), (1,1) (lower triangle of A).
+int reduce_blocks(bs_cell *lead, bs_cell *const *cells, int ncells, const Layout &L, long long src_off, long long dst_off,
+                  int inner, cudaStream_t s) {
+  const int N = L.N, n2 = 2 * N;
+  int launches = 0;
+  const long long blk[3] = {0, N, (long long)N * n2 + N};
+  for (int b = 0; b < 3; ++b) {
+    bsk::GemmDesc g{};
+    g.ncells = ncells; g.inner = inner;
+    g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+    // T = X_R * K_blk      (X_R lower: op(A)[m][k] = 0 for k > m)
+    g.M = N; g.N = N; g.K = N; g.opA = 0; g.opB = 0;
+    g.A = ref(lead, ncells, cells, L.XR, 0); g.lda = N;
+    g.B = ref(lead, ncells, cells, src_off + blk[b], (long long)n2 * n2); g.ldb = n2;
+    g.C = ref(lead, ncells, cells, L.Tb, (long long)N * N); g.ldc = N;
+    g.flags = BS_GEMM_KHI_ROW;
+    bsk::launch_zgemm(g, s);
+    // A_blk = T * X_R^H    (op(B)[k][n] = conj(X_R[n][k]) = 0 for k > n)
+    g.opB = 1;
+    g.A = g.C; g.lda = N;
+    g.B = ref(lead, ncells, cells, L.XR, 0); g.ldb = N;
+    g.C = ref(lead, ncells, cells, dst_off + blk[b], (long long)n2 * n2); g.ldc = n2;
+    g.flags = BS_GEMM_KHI_COL | (b != 1 ? BS_GEMM_LOWER_ONLY : 0);
+    bsk::launch_zgemm(g, s);
+    launches += 2;
+  }
+  return launches;
+}
+
+bs_status check_batch(bs_cell *const *cells, int ncells, const char *who) {
+  if (!cells || ncells < 1) return fail(BS_ERR_ARG, "%s: no cells", who);
+  for (int c = 0; c < ncells; ++c) {
+    if (!cells[c]) return fail(BS_ERR_ARG, "%s: cells[%d] is null", who, c);
+    if (!cells[c]->ws) return fail(BS_ERR_NOMEM, "%s: cells[%d] has no workspace (bs_set_workspace)", who, c);
+    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb)
+      return fail(BS_ERR_ARG, "%s: cells[%d] has different options than cells[0]", who, c);
+  }
+  return BS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, void *stream) {
+  bs_status st = check_batch(cells, ncells, "bs_assemble");
+  if (st != BS_OK) return st;
+  if (Mt < 0) return fail(BS_ERR_ARG, "bs_assemble: truncation < 0");
+  const long long N = (2LL * Mt + 1) * (2 * Mt + 1);
+  if (2 * N > 2048) return fail(BS_ERR_ARG, "bs_assemble: 2N = %lld exceeds 2048", 2 * N);
+  bs_cell *lead = cells[0];
+  cudaStream_t s = (cudaStream_t)stream;
+  const Layout L = make_layout(Mt, 1, lead->mode, lead->nb);
+  for (int c = 0; c < ncells; ++c) {
+    cells[c]->assembled = false;
+    if ((size_t)L.total * sizeof(cplx) > cells[c]->ws_bytes)
+      return fail(BS_ERR_NOMEM, "bs_assemble: cells[%d] workspace is %zu bytes, need %zu", c, cells[c]->ws_bytes,
+                  (size_t)L.total * sizeof(cplx));
+  }
+  st = ensure_batch(lead, cells, ncells, s);
+  if (st != BS_OK) return st;
+  const int n3 = 3 * (int)N, n2 = 2 * (int)N, Ni = (int)N;
+  auto R = [&](long long off, long long stride = 0) { return ref(lead, ncells, cells, off, stride); };
+  int64_t nl = 0;
+
+  tick(lead, 0, s);
+  bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), s); ++nl;  // S1
+  tick(lead, 1, s);
+  bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2
+  tick(lead, 2, s);
+  // S3: Phi = L L^H, X = L^{-1}, Y = X^H X;  R = L_R L_R^H, X_R = L_R^{-1}
+  CU(cudaMemsetAsync(lead->d_info, 0, sizeof(int) * 2 * ncells, s));
+  bsk::launch_copy_matrix(n3, n3, R(L.Phi), n3, R(L.Lf), n3, ncells, 1, s); ++nl;
+  bsk::launch_copy_matrix(Ni, Ni, R(L.R), Ni, R(L.LR), Ni, ncells, 1, s); ++nl;
+  nl += bsk::potrf_trtri(n3, n3, R(L.Lf), R(L.X), R(L.tmp), R(L.dinv), lead->d_info, 0, ncells, 1, s);
+  nl += bsk::potrf_trtri(Ni, Ni, R(L.LR), R(L.XR), R(L.tmpR), R(L.dinvR), lead->d_info + ncells, 0, ncells, 1, s);
+  {
+    bsk::GemmDesc g{};
+    g.ncells = ncells; g.inner = 1;
+    g.M = n3; g.N = n3; g.K = n3; g.opA = 1; g.opB = 0;
+    g.A = R(L.X); g.lda = n3; g.B = R(L.X); g.ldb = n3; g.C = R(L.Y); g.ldc = n3;
+    g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+    g.flags = BS_GEMM_LOWER_ONLY | BS_GEMM_KLO_ROW | BS_GEMM_KLO_COL;
+    bsk::launch_zgemm(g, s); ++nl;
+    bsk::launch_hermitian_fill_upper(n3, R(L.Y), n3, ncells, 1, s); ++nl;
+  }
+  tick(lead, 3, s);
+  if (lead->mode == BS_PENCIL_POLY) {
+    std::vector<double> kv;
+    for (int c = 0; c < ncells; ++c) {
+      fill_coef_kvec(cells[c], Mt, kv);
+      CU(cudaMemcpyAsync((cplx *)cells[c]->ws + L.kvecA, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+      CU(cudaStreamSynchronize(s));
+    }
+    // the cells of one batch may have different areas: V^2 is applied per cell
+    bool sameV = true;
+    for (int c = 1; c < ncells; ++c) sameV = sameV && cells[c]->V == lead->V;
+    if (!sameV) return fail(BS_ERR_ARG, "bs_assemble_batch: all cells of a batch must have the same cell area");
+    bsk::launch_pencil(Ni, lead->V * lead->V, R(L.Y), n3, R(L.Coef, (long long)n2 * n2), n2, R(L.kvecA, 4LL * Ni), 2,
+                       ncells, 6, s); ++nl;
+    nl += reduce_blocks(lead, cells, ncells, L, L.Coef, L.Coef, 6, s);
+  }
+  tick(lead, 4, s);
+  CU(cudaStreamSynchronize(s));
+  CU(cudaGetLastError());
+  std::vector<int> info(2 * ncells);
+  CU(cudaMemcpy(info.data(), lead->d_info, sizeof(int) * 2 * ncells, cudaMemcpyDeviceToHost));
+  lead->launches += nl;
+  if (lead->timing) {
+    lead->ms[BS_T_TABLE] = tock(lead, 0, 1);
+    lead->ms[BS_T_EXPAND] = tock(lead, 1, 2);
+    lead->ms[BS_T_FACTOR] = tock(lead, 2, 3);
+    lead->ms[BS_T_COEF] = tock(lead, 3, 4);
+  }
+  for (int c = 0; c < ncells; ++c) {
+    if (info[c]) return fail(BS_ERR_NOT_PD, "bs_assemble: Phi of cells[%d] is not positive definite (pivot %d)", c, info[c]);
+    if (info[ncells + c])
+      return fail(BS_ERR_NOT_PD, "bs_assemble: R (Psi) of cells[%d] is not positive definite (pivot %d)", c, info[ncells + c]);
+  }
+  for (int c = 0; c < ncells; ++c) {
+    cells[c]->lay = L;
+    cells[c]->assembled = true;
+  }
+  return BS_OK;
+}
+
+bs_status bs_assemble(bs_cell *cell, int32_t Mt, void *stream) {
+  if (!cell) return fail(BS_ERR_ARG, "bs_assemble: null handle");
+  return bs_assemble_batch(&cell, 1, Mt, stream);
+}
+
+bs_status bs_get_table(bs_cell *c, void *table_host) {
+  if (!c || !table_host) return fail(BS_ERR_ARG, "bs_get_table: null argument");
+  if (!c->assembled) return fail(BS_ERR_STATE, "bs_get_table: call bs_assemble first");
+  const long long Lt = 4 * c->lay.Mt + 1;
+  CU(cudaDeviceSynchronize());
+  CU(cudaMemcpy(table_host, (cplx *)c->ws + c->lay.table, sizeof(cplx) * 7 * Lt * Lt, cudaMemcpyDeviceToHost));
+  return BS_OK;
+}
+
+bs_status bs_get_matrices(bs_cell *c, void *phi_host, void *psi_host) {
+  if (!c) return fail(BS_ERR_ARG, "bs_get_matrices: null handle");
+  if (!c->assembled) return fail(BS_ERR_STATE, "bs_get_matrices: call bs_assemble first");
+  const size_t N = c->lay.N, n3 = 3 * N, n2 = 2 * N;
+  CU(cudaDeviceSynchronize());
+  if (phi_host) CU(cudaMemcpy(phi_host, (cplx *)c->ws + c->lay.Phi, sizeof(cplx) * n3 * n3, cudaMemcpyDeviceToHost));
+  if (psi_host) {  // Psi = diag(R, R)  (eq. 19)
+    std::memset(psi_host, 0, sizeof(cplx) * n2 * n2);
+    const cplx *Rd = (cplx *)c->ws + c->lay.R;
+    cplx *ps = (cplx *)psi_host;
+    CU(cudaMemcpy2D(ps, sizeof(cplx) * n2, Rd, sizeof(cplx) * N, sizeof(cplx) * N, N, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpy2D(ps + N * n2 + N, sizeof(cplx) * n2, Rd, sizeof(cplx) * N, sizeof(cplx) * N, N, cudaMemcpyDeviceToHost));
+  }
+  return BS_OK;
+}
+
+bs_status bs_get_pencil(bs_cell *c, const double kred[2], void *K_host, void *stream) {
+  if (!c || !kred || !K_host) return fail(BS_ERR_ARG, "bs_get_pencil: null argument");
+  if (!c->assembled) return fail(BS_ERR_STATE, "bs_get_pencil: call bs_assemble first");
+  cudaStream_t s = (cudaStream_t)stream;
+  const Layout L = make_layout(c->lay.Mt, 1, c->mode, c->nb);
+  const int N = L.N, n2 = 2 * N, n3 = 3 * N;
+  std::vector<double> kv;
+  fill_direct_kvec(c, L.Mt, 1, kred, kv);
+  CU(cudaMemcpyAsync((cplx *)c->ws + L.kvecK, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+  bs_cell *cells[1] = {c};
+  bsk::launch_pencil(N, c->V * c->V, ref(c, 1, cells, L.Y, 0), n3, ref(c, 1, cells, L.Kk, 0), n2,
+                     ref(c, 1, cells, L.kvecK, 0), 1, 1, 1, s);
+  c->launches += 1;
+  CU(cudaMemcpyAsync(K_host, (cplx *)c->ws + L.Kk, sizeof(cplx) * n2 * n2, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  return BS_OK;
+}
+
+}  // extern "C"
+
+extern "C" {
+
+bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, const double *kpts, int32_t nbands,
+                         double *omega2_out, void *stream) {
+  bs_status st = check_batch(cells, ncells, "bs_bands");
+  if (st != BS_OK) return st;
+  if (!kpts || !omega2_out || nk < 1) return fail(BS_ERR_ARG, "bs_bands: null pointer or nk < 1");
+  bs_cell *lead = cells[0];
+  for (int c = 0; c < ncells; ++c) {
+    if (!cells[c]->assembled) return fail(BS_ERR_STATE, "bs_bands: cells[%d] is not assembled (bs_assemble)", c);
+    if (cells[c]->lay.Mt != lead->lay.Mt) return fail(BS_ERR_ARG, "bs_bands: cells[%d] has a different truncation", c);
+  }
+  const int Mt = lead->lay.Mt;
+  const Layout L = make_layout(Mt, nk, lead->mode, lead->nb);
+  const int N = L.N, n2 = 2 * N, n3 = 3 * N;
+  if (nbands < 1 || nbands > n2) return fail(BS_ERR_ARG, "bs_bands: nbands must be in 1..2N = %d", n2);
+  for (int c = 0; c < ncells; ++c)
+    if ((size_t)L.total * sizeof(cplx) > cells[c]->ws_bytes)
+      return fail(BS_ERR_NOMEM, "bs_bands: cells[%d] workspace is %zu bytes, %d k-points need %zu", c, cells[c]->ws_bytes, nk,
+                  (size_t)L.total * sizeof(cplx));
+  cudaStream_t s = (cudaStream_t)stream;
+  st = ensure_batch(lead, cells, ncells, s);
+  if (st != BS_OK) return st;
+  const size_t nmat = (size_t)ncells * nk;
+  // flat scratch: d, e (nmat x n), scal (2 nmat), lam (nmat x nbands), coefk (6 nmat)
+  st = ensure_flat(lead, nmat * ((size_t)2 * n2 + 2 + nbands + 6));
+  if (st != BS_OK) return st;
+  double *d = lead->d_flat, *e = d + nmat * n2, *scal = e + nmat * n2, *lam = scal + 2 * nmat, *coefk = lam + nmat * nbands;
+  auto R = [&](long long off, long long stride = 0) { return ref(lead, ncells, cells, off, stride); };
+  int64_t nl = 0;
+  const long long mat = (long long)n2 * n2;
+
+  tick(lead, 0, s);
+  if (lead->mode == BS_PENCIL_POLY) {
+    std::vector<double> ck(nmat * 6);
+    for (int c = 0; c < ncells; ++c)
+      for (int k = 0; k < nk; ++k) {
+        const double *Q = cells[c]->Q;
+        const double kx = kpts[2 * k] * Q[0] + kpts[2 * k + 1] * Q[2], ky = kpts[2 * k] * Q[1] + kpts[2 * k + 1] * Q[3];
+        double *o = &ck[((size_t)c * nk + k) * 6];
+        o[0] = 1.0; o[1] = kx; o[2] = ky; o[3] = kx * kx; o[4] = kx * ky; o[5] = ky * ky;
+      }
+    CU(cudaMemcpyAsync(coefk, ck.data(), ck.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));
+    bsk::launch_combine(n2, R(L.Coef), mat, R(L.Ak, mat), n2, coefk, nk, ncells, s); ++nl;
+  } else {
+    std::vector<double> kv;
+    for (int c = 0; c < ncells; ++c) {
+      fill_direct_kvec(cells[c], Mt, nk, kpts, kv);
+      CU(cudaMemcpyAsync((cplx *)cells[c]->ws + L.kvecK, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+      CU(cudaStreamSynchronize(s));
+    }
+    bsk::launch_pencil(N, lead->V * lead->V, R(L.Y), n3, R(L.Kk, mat), n2, R(L.kvecK, 2LL * N), 1, ncells, nk, s); ++nl;  // S4
+    nl += reduce_blocks(lead, cells, ncells, L, L.Kk, L.Ak, nk, s);                                                        // S5
+  }
+  tick(lead, 1, s);
+  nl += bsk::launch_tridiag(n2, n2, lead->nb, R(L.Ak, mat), R(L.VW, (long long)bsk::tridiag_vw_elems(n2, lead->nb)),
+                            R(L.P, (long long)bsk::tridiag_p_elems(n2)), d, e, scal, ncells, nk, s);  // S6
+  tick(lead, 2, s);
+  bsk::launch_sturm(n2, d, e, nbands, lam, (int)nmat, s); ++nl;                                       // S7
+  tick(lead, 3, s);
+  lead->launches += nl;
+  lead->last_n = n2; lead->last_nmat = (int)nmat; lead->last_nk = nk;
+  // S8: one copy of ncells x nk x nbands doubles
+  cudaPointerAttributes attr;
+  bool on_device = false;
+  if (cudaPointerGetAttributes(&attr, omega2_out) == cudaSuccess) on_device = attr.type == cudaMemoryTypeDevice;
+  else cudaGetLastError();
+  CU(cudaMemcpyAsync(omega2_out, lam, nmat * nbands * sizeof(double),
+                     on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+  if (!on_device || lead->timing) CU(cudaStreamSynchronize(s));
+  if (lead->timing) {
+    lead->ms[BS_T_PENCIL] = tock(lead, 0, 1);
+    lead->ms[BS_T_TRIDIAG] = tock(lead, 1, 2);
+    lead->ms[BS_T_BISECT] = tock(lead, 2, 3);
+  }
+  CU(cudaGetLastError());
+  return BS_OK;
+}
+
+bs_status bs_bands(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *stream) {
+  if (!cell) return fail(BS_ERR_ARG, "bs_bands: null handle");
+  return bs_bands_batch(&cell, 1, nk, kpts, nbands, omega2_out, stream);
+}
+
+bs_status bs_get_tridiagonal(bs_cell *c, double *d_host, double *e_host) {
+  if (!c || !d_host || !e_host) return fail(BS_ERR_ARG, "bs_get_tridiagonal: null argument");
+  if (!c->d_flat || c->last_nmat == 0) return fail(BS_ERR_STATE, "bs_get_tridiagonal: no bs_bands call led by this handle yet");
+  const size_t cnt = (size_t)c->last_nmat * c->last_n;
+  CU(cudaDeviceSynchronize());
+  CU(cudaMemcpy(d_host, c->d_flat, cnt * sizeof(double), cudaMemcpyDeviceToHost));
+  CU(cudaMemcpy(e_host, c->d_flat + cnt, cnt * sizeof(double), cudaMemcpyDeviceToHost));
+  return BS_OK;
+}
+
+// ---------------------------------------------------------------- diagnostics: building blocks on caller-owned device arrays
+static BatchRef raw(const void *p, long long stride) {
+  BatchRef r;
+  r.bases = nullptr; r.single = (unsigned long long)p; r.off = 0; r.stride = stride;
+  return r;
+}
+
+bs_status bs_zgemm(int32_t opA, int32_t opB, int32_t M, int32_t N, int32_t K, const double alpha[2], const void *A,
+                   int32_t lda, int64_t strideA, const void *B, int32_t ldb, int64_t strideB, const double beta[2],
+                   void *C, int32_t ldc, int64_t strideC, int32_t batch, int32_t flags, void *stream) {
+  if (!A || !B || !C || !alpha || !beta || M < 0 || N < 0 || K < 0 || batch < 1) return fail(BS_ERR_ARG, "bs_zgemm: bad argument");
+  bsk::GemmDesc g{};
+  g.M = M; g.N = N; g.K = K; g.opA = opA; g.opB = opB; g.lda = lda; g.ldb = ldb; g.ldc = ldc; g.flags = flags;
+  g.ncells = 1; g.inner = batch;
+  g.alpha = cmake(alpha[0], alpha[1]); g.beta = cmake(beta[0], beta[1]);
+  g.A = raw(A, strideA); g.B = raw(B, strideB); g.C = raw(C, strideC);
+  bsk::launch_zgemm(g, (cudaStream_t)stream);
+  CU(cudaGetLastError());
+  return BS_OK;
+}
+
+bs_status bs_zpotrf_trtri(int32_t n, void *A, int32_t lda, int64_t strideA, void *X, void *tmp, void *dinv, int32_t *info,
+                          int32_t batch, void *stream) {
+  if (!A || !X || !tmp || !dinv || !info || n < 1 || batch < 1) return fail(BS_ERR_ARG, "bs_zpotrf_trtri: bad argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(cudaMemsetAsync(info, 0, sizeof(int) * batch, s));
+  // the factor kernels index matrices by cell; express the batch as `batch` cells through a device array of bases
+  std::vector<unsigned long long> hb(4 * (size_t)batch);
+  const long long dstride = (long long)((n + 63) / 64) * 4096;
+  for (int b = 0; b < batch; ++b) {
+    hb[b] = (unsigned long long)((cplx *)A + (long long)b * strideA);
+    hb[batch + b] = (unsigned long long)((cplx *)X + (long long)b * strideA);
+    hb[2 * batch + b] = (unsigned long long)((cplx *)tmp + (long long)b * strideA);
+    hb[3 * batch + b] = (unsigned long long)((cplx *)dinv + (long long)b * dstride);
+  }
+  unsigned long long *db = nullptr;
+  CU(cudaMalloc(&db, sizeof(unsigned long long) * hb.size()));
+  CU(cudaMemcpyAsync(db, hb.data(), sizeof(unsigned long long) * hb.size(), cudaMemcpyHostToDevice, s));
+  auto br = [&](int which) { BatchRef r; r.bases = db + (size_t)which * batch; r.single = 0; r.off = 0; r.stride = 0; return r; };
+  bsk::potrf_trtri(n, lda, br(0), br(1), br(2), br(3), info, 0, batch, 1, s);
+  CU(cudaStreamSynchronize(s));
+  cudaFree(db);
+  CU(cudaGetLastError());
+  return BS_OK;
+}
+
+size_t bs_zhetrd_scratch_elems(int32_t n, int32_t nb) {
+  if (n < 1) return 0;
+  if (nb < 4) nb = 4;
+  if (nb > 32) nb = 32;
+  return bsk::tridiag_vw_elems(n, nb) + bsk::tridiag_p_elems(n) + 16;
+}
+
+bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *scratch, int32_t nb,
+                    int32_t batch, void *stream) {
+  if (!A || !d || !e || !scratch || n < 1 || n > 2048 || batch < 1 || lda < n) return fail(BS_ERR_ARG, "bs_zhetrd: bad argument");
+  if (nb < 4) nb = 4;
+  if (nb > 32) nb = 32;
+  const long long vw = (long long)bsk::tridiag_vw_elems(n, nb), pp = (long long)bsk::tridiag_p_elems(n);
+  const long long per = vw + pp + 16;
+  cplx *sc = (cplx *)scratch;
+  BatchRef VW = raw(sc, per), P = raw(sc + vw, per);
+  // tau of the pending reflector: the 16 spare elements of matrix 0's slot hold nothing else; use a strided view
+  // (scal is indexed [2*z]), so place it after all per-matrix slots is not possible without more memory: use slot tails.
+  double *scal = nullptr;
+  CU(cudaMalloc(&scal, sizeof(double) * 2 * batch));
+  bsk::launch_tridiag(n, lda, nb, raw(A, strideA), VW, P, d, e, scal, 1, batch, (cudaStream_t)stream);
+  CU(cudaStreamSynchronize((cudaStream_t)stream));
+  cudaFree(scal);
+  CU(cudaGetLastError());
+  return BS_OK;
+}
+
+bs_status bs_sturm(int32_t n, const double *d, const double *e, int32_t nev, double *lam, int32_t batch, void *stream) {
+  if (!d || !e || !lam || n < 1 || nev < 1 || nev > n || batch < 1) return fail(BS_ERR_ARG, "bs_sturm: bad argument");
+  bsk::launch_sturm(n, d, e, nev, lam, batch, (cudaStream_t)stream);
+  CU(cudaGetLastError());
+  return BS_OK;
+}
+
+}  // extern "C"

@@ -90,18 +90,21 @@ void launch_copy_matrix(int rows, int cols, BatchRef src, int lds, BatchRef dst,
                         cudaStream_t s);
 void launch_hermitian_fill_upper(int n, BatchRef A, int lda, int ncells, int inner, cudaStream_t s);
 
-// S4: K = V^2 sum_t Btilde(kL_t)^T Y Btilde(kR_t), nterm <= 2.  kvec: device doubles,
-// per output matrix z (= cell*inner + i): [nterm][2 (L,R)][2 (x,y)][N] at kvec + z*kvec_stride.
-void launch_pencil(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk, const double *kvec, long long kvec_stride,
-                   int nterm, int ncells, int inner, cudaStream_t s);
+// S4: K = V^2 sum_t Btilde(kL_t)^T Y Btilde(kR_t), nterm <= 2.  kvec: per output matrix
+// (cell, i) doubles [nterm][2 (L,R)][2 (x,y)][N] at the BatchRef (offset/stride in complex elements = 2 doubles).
+void launch_pencil(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk, BatchRef kvec, int nterm, int ncells,
+                   int inner, cudaStream_t s);
 // A(k) = sum_i c_i(k) Coef_i, lower triangle (by 64-tiles) only.  coef: [ncells*nk][6] doubles.
 void launch_combine(int n, BatchRef Coef, long long coef_mat_stride, BatchRef Ak, int ld, const double *coefk, int nk,
                     int ncells, cudaStream_t s);
 
-// S6: tridiagonalisation.  vw: per matrix 2*n*nb complex.  d,e: per matrix n doubles at d + z*n.
-size_t tridiag_smem_bytes(int n, int nb);
-void launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, double *d, double *e, int ncells, int inner,
-                    cudaStream_t s);
+// S6: tridiagonalisation (lower triangle of A read; A22 blocks overwritten).  VW: per matrix tridiag_vw_elems complex,
+// P: per matrix tridiag_p_elems complex (hemv partial sums), d,e: per matrix n doubles at d + z*n, scal: 2 doubles per
+// matrix.  Returns the number of kernel launches issued.
+size_t tridiag_vw_elems(int n, int nb);
+size_t tridiag_p_elems(int n);
+int launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, BatchRef P, double *d, double *e, double *scal,
+                   int ncells, int inner, cudaStream_t s);
 // S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
 void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s);
 

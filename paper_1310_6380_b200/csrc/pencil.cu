@@ -9,15 +9,14 @@ namespace bsk {
 
 namespace {
 __global__ void __launch_bounds__(256) pencil_kernel(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk,
-                                                     const double *__restrict__ kvec, long long kvec_stride, int nterm,
-                                                     int inner) {
+                                                     BatchRef kvec, int nterm, int inner) {
   const int z = blockIdx.z;
   const int cell = z / inner, bi = z % inner;
   const int g = blockIdx.x * blockDim.x + threadIdx.x, h = blockIdx.y;
   if (g >= N) return;
   const cplx *__restrict__ Yg = batch_ptr(Y, cell, 0);
   cplx *Kg = batch_ptr(K, cell, bi);
-  const double *kv = kvec + (size_t)z * kvec_stride;
+  const double *__restrict__ kv = reinterpret_cast<const double *>(batch_ptr(kvec, cell, bi));
   cplx y[3][3];
 #pragma unroll
   for (int b = 0; b < 3; ++b)
@@ -69,11 +68,11 @@ __global__ void __launch_bounds__(256) combine_kernel(int n, BatchRef Coef, long
 }
 }  // namespace
 
-void launch_pencil(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk, const double *kvec, long long kvec_stride,
-                   int nterm, int ncells, int inner, cudaStream_t s) {
+void launch_pencil(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk, BatchRef kvec, int nterm, int ncells,
+                   int inner, cudaStream_t s) {
   const int bs = N >= 256 ? 256 : ((N + 31) / 32) * 32;
   dim3 grid((N + bs - 1) / bs, N, ncells * inner);
-  pencil_kernel<<<grid, bs, 0, s>>>(N, V2, Y, ldy, K, ldk, kvec, kvec_stride, nterm, inner);
+  pencil_kernel<<<grid, bs, 0, s>>>(N, V2, Y, ldy, K, ldk, kvec, nterm, inner);
 }
 
 void launch_combine(int n, BatchRef Coef, long long coef_mat_stride, BatchRef Ak, int ld, const double *coefk, int nk,

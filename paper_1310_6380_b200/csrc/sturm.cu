@@ -1,0 +1,93 @@
+// S7: lowest nev eigenvalues of real symmetric tridiagonal matrices by Sturm-count multisection.
+// count(x) = number of negative pivots of T - xI = number of eigenvalues < x (Sylvester); the k-th eigenvalue (0-based)
+// is the infimum of { x : count(x) >= k+1 }.  Start interval: Gershgorin.  DESIGN.md section 5 (S7); lambda = omega^2 of
+// PAPER.md:104.
+#include "bs_internal.cuh"
+
+namespace bsk {
+
+namespace {
+constexpr int ST = 256;   // threads per matrix
+constexpr int G = 8;      // interior shifts per eigenvalue per round -> the interval shrinks 9x per round
+constexpr int EPB = ST / G;  // eigenvalues per pass
+constexpr int ROUNDS = 24;   // 9^24 > 2^76
+
+__device__ __forceinline__ int sturm_count(const double *__restrict__ d, const double *__restrict__ e2, int n, double x,
+                                           double pivmin) {
+  int cnt = 0;
+  double q = d[0] - x;
+  if (fabs(q) < pivmin) q = -pivmin;
+  cnt += q < 0.0;
+  for (int i = 1; i < n; ++i) {
+    q = d[i] - x - e2[i - 1] / q;
+    if (fabs(q) < pivmin) q = -pivmin;
+    cnt += q < 0.0;
+  }
+  return cnt;
+}
+
+__global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restrict__ dg, const double *__restrict__ eg,
+                                                   int nev, double *__restrict__ lam) {
+  extern __shared__ double sm[];
+  double *d = sm, *e2 = sm + n;
+  __shared__ double s_lo, s_hi, s_emax;
+  __shared__ int cnts[ST];
+  const int z = blockIdx.x, t = threadIdx.x;
+  dg += (size_t)z * n;
+  eg += (size_t)z * n;
+  for (int i = t; i < n; i += ST) {
+    d[i] = dg[i];
+    e2[i] = (i + 1 < n) ? eg[i] * eg[i] : 0.0;
+  }
+  __syncthreads();
+  if (t == 0) {  // Gershgorin bounds (n <= 2048: serial is fine next to the bisection itself)
+    double lo = d[0], hi = d[0], emax = 0.0;
+    for (int i = 0; i < n; ++i) {
+      const double l = i > 0 ? sqrt(e2[i - 1]) : 0.0, r = i + 1 < n ? sqrt(e2[i]) : 0.0;
+      lo = fmin(lo, d[i] - l - r);
+      hi = fmax(hi, d[i] + l + r);
+      emax = fmax(emax, e2[i]);
+    }
+    const double nrm = fmax(fabs(lo), fabs(hi));
+    lo -= 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
+    hi += 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
+    s_lo = lo; s_hi = hi; s_emax = emax;
+  }
+  __syncthreads();
+  const double pivmin = fmax(2.3e-308 * fmax(1.0, s_emax), 2.3e-308);
+  const int grp = t / G, sub = t % G;
+  for (int k0 = 0; k0 < nev; k0 += EPB) {
+    const int k = k0 + grp;  // eigenvalue index of this group
+    double lo = s_lo, hi = s_hi;
+    for (int round = 0; round < ROUNDS; ++round) {
+      const double w = hi - lo;
+      const double x = lo + w * ((double)(sub + 1) / (double)(G + 1));
+      int c = 0;
+      if (k < nev) c = sturm_count(d, e2, n, x, pivmin);
+      cnts[t] = c;
+      __syncthreads();
+      // new interval: [x_{m-1}, x_m] with m the first sub-shift whose count >= k+1  (x_{-1} = lo, x_G = hi)
+      int m = G;
+      for (int s2 = G - 1; s2 >= 0; --s2)
+        if (cnts[grp * G + s2] >= k + 1) m = s2;
+      const double nlo = m == 0 ? lo : lo + w * ((double)m / (double)(G + 1));
+      const double nhi = m == G ? hi : lo + w * ((double)(m + 1) / (double)(G + 1));
+      lo = nlo; hi = nhi;
+      __syncthreads();
+    }
+    if (k < nev && sub == 0) lam[(size_t)z * nev + k] = 0.5 * (lo + hi);
+  }
+}
+}  // namespace
+
+void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s) {
+  const size_t smem = (size_t)2 * n * sizeof(double);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(sturm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    attr_done = true;
+  }
+  sturm_kernel<<<nmat, ST, smem, s>>>(n, d, e, nev, lam);
+}
+
+}  // namespace bsk

@@ -80,6 +80,10 @@ def _check(status: int) -> None:
         raise BsError(status, (lib.bs_last_error() or b"").decode())
 
 
+def bs_last_error() -> str:
+    return (lib.bs_last_error() or b"").decode()
+
+
 def _f64(a) -> np.ndarray:
     return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
 

@@ -1,0 +1,201 @@
+"""GPU tests (-m gpu) of the dense building blocks exposed by the C-ABI for diagnostics (bs_zgemm, bs_zpotrf_trtri,
+bs_zhetrd, bs_sturm) against NumPy/LAPACK, plus the error paths of the boundary."""
+import numpy as np
+import pytest
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def bs():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1310_6380_b200 as bs
+    return bs
+
+
+def to_dev(a):
+    """NumPy (rows, cols) complex -> torch CUDA tensor holding the column-major image (shape (cols, rows))."""
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a.T)).cuda()
+
+
+def from_dev(t):
+    return t.cpu().numpy().T
+
+
+def rand_c(rng, m, n):
+    return rng.normal(size=(m, n)) + 1j * rng.normal(size=(m, n))
+
+
+@pytest.mark.parametrize("opA,opB", [(0, 0), (0, 1), (1, 0), (1, 1)])
+@pytest.mark.parametrize("M,N,K", [(64, 64, 8), (130, 75, 37), (257, 199, 64), (5, 3, 1)])
+def test_zgemm(bs, opA, opB, M, N, K):
+    import torch
+    rng = np.random.default_rng(M * 1000 + N + K + 7 * opA + 3 * opB)
+    A = rand_c(rng, K, M) if opA else rand_c(rng, M, K)
+    B = rand_c(rng, N, K) if opB else rand_c(rng, K, N)
+    Cm = rand_c(rng, M, N)
+    al, be = 0.7 - 0.2j, -0.3 + 1.1j
+    ref = al * ((A.conj().T if opA else A) @ (B.conj().T if opB else B)) + be * Cm
+    dA, dB, dC = to_dev(A), to_dev(B), to_dev(Cm)
+    bs.bs_zgemm(opA, opB, M, N, K, al, dA, A.shape[0], 0, dB, B.shape[0], 0, be, dC, M, 0)
+    torch.cuda.synchronize()
+    got = from_dev(dC)
+    assert np.max(np.abs(got - ref)) <= 1e-13 * K * np.max(np.abs(ref))
+
+
+def test_zgemm_batched_lower_only(bs):
+    import torch
+    rng = np.random.default_rng(5)
+    n, k, batch = 150, 40, 3
+    A = [rand_c(rng, n, k) for _ in range(batch)]
+    C0 = [rand_c(rng, n, n) for _ in range(batch)]
+    dA = torch.stack([to_dev(a) for a in A])
+    dC = torch.stack([to_dev(c) for c in C0])
+    bs.bs_zgemm(0, 1, n, n, k, -1.0, dA, n, n * k, dA, n, n * k, 1.0, dC, n, n * n, batch, bs.BS_GEMM_LOWER_ONLY)
+    torch.cuda.synchronize()
+    for b in range(batch):
+        got = dC[b].cpu().numpy().T
+        ref = C0[b] - A[b] @ A[b].conj().T
+        lo = np.tril_indices(n)
+        up = np.triu_indices(n, 1)
+        assert np.max(np.abs(got[lo] - ref[lo])) <= 1e-12 * np.max(np.abs(ref))
+        assert np.array_equal(got[up], C0[b][up])      # the strict upper triangle is untouched
+
+
+@pytest.mark.parametrize("n", [17, 64, 100, 363, 450])
+def test_zpotrf_trtri(bs, n):
+    import torch
+    rng = np.random.default_rng(n)
+    batch = 2
+    mats = []
+    for _ in range(batch):
+        G = rand_c(rng, n, n)
+        mats.append(G @ G.conj().T + n * np.eye(n))
+    dA = torch.stack([to_dev(m) for m in mats])
+    dX = torch.zeros_like(dA)
+    tmp = torch.zeros_like(dA)
+    dinv = torch.zeros(batch * ((n + 63) // 64) * 4096, dtype=torch.complex128, device="cuda")
+    info = torch.zeros(batch, dtype=torch.int32, device="cuda")
+    bs.bs_zpotrf_trtri(n, dA, n, n * n, dX, tmp, dinv, info, batch)
+    torch.cuda.synchronize()
+    assert info.cpu().numpy().tolist() == [0] * batch
+    for b in range(batch):
+        L = np.tril(dA[b].cpu().numpy().T)
+        Lr = np.linalg.cholesky(mats[b])
+        assert np.max(np.abs(L - Lr)) <= 1e-12 * np.max(np.abs(Lr))
+        X = dX[b].cpu().numpy().T
+        assert np.max(np.abs(np.triu(X, 1))) == 0
+        assert np.max(np.abs(X @ Lr - np.eye(n))) <= 1e-11
+
+
+def test_zpotrf_reports_not_pd(bs):
+    import torch
+    n = 70
+    A = np.eye(n, dtype=complex)
+    A[66, 66] = -1.0
+    dA = to_dev(A)[None].contiguous()
+    dX, tmp = torch.zeros_like(dA), torch.zeros_like(dA)
+    dinv = torch.zeros(2 * 4096, dtype=torch.complex128, device="cuda")
+    info = torch.zeros(1, dtype=torch.int32, device="cuda")
+    bs.bs_zpotrf_trtri(n, dA, n, n * n, dX, tmp, dinv, info, 1)
+    assert int(info.cpu()[0]) == 67
+
+
+@pytest.mark.parametrize("n,nb", [(5, 4), (64, 8), (98, 32), (242, 32), (450, 16), (130, 32)])
+def test_zhetrd_eigenvalues(bs, n, nb):
+    import torch
+    rng = np.random.default_rng(n + nb)
+    batch = 3
+    mats = []
+    for _ in range(batch):
+        G = rand_c(rng, n, n)
+        mats.append(G + G.conj().T)
+    dA = torch.stack([to_dev(m) for m in mats])
+    d = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+    e = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+    scratch = torch.zeros(batch * bs.bs_zhetrd_scratch_elems(n, nb), dtype=torch.complex128, device="cuda")
+    bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, batch)
+    torch.cuda.synchronize()
+    for b in range(batch):
+        dd, ee = d[b].cpu().numpy(), e[b].cpu().numpy()[:n - 1]
+        T = np.diag(dd) + np.diag(ee, 1) + np.diag(ee, -1)
+        lt = np.linalg.eigvalsh(T)
+        la = np.linalg.eigvalsh(mats[b])
+        assert np.max(np.abs(lt - la)) <= 1e-13 * n * np.max(np.abs(la))
+
+
+def test_sturm_constant_tridiagonal_textbook(bs):
+    # constant-coefficient tridiagonal: eigenvalues d + 2 e cos(j pi/(n+1)), j = 1..n
+    import torch
+    n, dd, ee = 333, 1.5, -0.75
+    d = torch.full((1, n), dd, dtype=torch.float64, device="cuda")
+    e = torch.full((1, n), ee, dtype=torch.float64, device="cuda")
+    nev = 40
+    lam = torch.zeros(1, nev, dtype=torch.float64, device="cuda")
+    bs.bs_sturm(n, d, e, nev, lam, 1)
+    ref = np.sort(dd + 2 * ee * np.cos(np.arange(1, n + 1) * np.pi / (n + 1)))[:nev]
+    assert np.max(np.abs(lam.cpu().numpy()[0] - ref)) <= 1e-14 * 3.0
+
+
+def test_sturm_random_and_degenerate(bs):
+    import torch
+    rng = np.random.default_rng(3)
+    n, batch, nev = 257, 4, 257
+    dn = rng.normal(size=(batch, n))
+    en = rng.normal(size=(batch, n))
+    en[1, 100] = 0.0              # a split matrix
+    dn[2, :] = 2.0; en[2, :] = 0.0    # diagonal with a fully repeated eigenvalue
+    d, e = torch.from_numpy(dn).cuda(), torch.from_numpy(en).cuda()
+    lam = torch.zeros(batch, nev, dtype=torch.float64, device="cuda")
+    bs.bs_sturm(n, d, e, nev, lam, batch)
+    got = lam.cpu().numpy()
+    for b in range(batch):
+        T = np.diag(dn[b]) + np.diag(en[b, :n - 1], 1) + np.diag(en[b, :n - 1], -1)
+        ref = np.linalg.eigvalsh(T)
+        assert np.max(np.abs(got[b] - ref)) <= 1e-14 * n * max(1.0, np.max(np.abs(ref)))
+
+
+def test_error_paths(bs):
+    c = wl.random_small_cell(1, 2)
+    comp = bs.bs_isotropic_plane_strain(c.E, c.nu)
+    # clockwise polygon
+    v = c.verts.copy()
+    v[:4] = v[:4][::-1]
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_create_cell(c.lattice, c.vert_offset, v, comp, c.rho)
+    assert ei.value.status == bs.BS_ERR_GEOMETRY
+    # tiling does not cover the cell
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_create_cell(2.0 * c.lattice, c.vert_offset, c.verts, comp, c.rho)
+    assert ei.value.status == bs.BS_ERR_GEOMETRY
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_isotropic_plane_strain([1.0], [0.5])
+    assert ei.value.status == bs.BS_ERR_ARG
+    h = bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, comp, c.rho)
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_assemble(h, 2)                      # no workspace
+    assert ei.value.status == bs.BS_ERR_NOMEM
+    bs.allocate_workspace(h, 2, 2)
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_bands(h, [[0.1, 0.2]], 4)           # not assembled
+    assert ei.value.status == bs.BS_ERR_STATE
+    bs.bs_assemble(h, 2)
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_bands(h, [[0.1, 0.2]], 51)          # nbands > 2N = 50
+    assert ei.value.status == bs.BS_ERR_ARG
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_bands(h, np.zeros((3, 2)), 4)       # workspace sized for 2 k-points
+    assert ei.value.status == bs.BS_ERR_NOMEM
+    # negative density contrast making R indefinite -> NOT_PD is reported, not a crash
+    rho = c.rho.copy()
+    h2 = bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, -comp, rho)
+    bs.allocate_workspace(h2, 1, 1)
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_assemble(h2, 1)
+    assert ei.value.status == bs.BS_ERR_NOT_PD
+    bs.bs_destroy_cell(h)
+    bs.bs_destroy_cell(h2)

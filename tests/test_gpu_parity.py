@@ -1,0 +1,190 @@
+"""GPU parity tests (-m gpu): the CUDA path through the C-ABI (ctypes binding) against the CPU oracle on the same
+seeded inputs.  Tolerances: matrices <= 1e-12 norm-wise (R7 / SURVEY A14); eigenfrequencies
+<= 1e-9 relative OR |dlambda| <= 64 eps lambda_max (R8 / SURVEY A15)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+EPS = 2.0 ** -53
+
+
+@pytest.fixture(scope="module")
+def bs():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1310_6380_b200 as bs
+    return bs
+
+
+def make_cell(bs, cell, Mt, nk, mode=None, panel=None):
+    comp = bs.bs_isotropic_plane_strain(cell.E, cell.nu)
+    h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho)
+    if mode is not None:
+        bs.bs_set_option(h, bs.BS_OPT_PENCIL_MODE, mode)
+    if panel is not None:
+        bs.bs_set_option(h, bs.BS_OPT_PANEL, panel)
+    bs.allocate_workspace(h, Mt, nk)
+    return h
+
+
+def check_bands(lam_gpu, lam_ref, lmax, tag=""):
+    """R8: pass if |omega_gpu - omega_ref| <= 1e-9 omega_ref or |dlambda| <= 64 eps lambda_max.  Returns the number of
+    (k, band) pairs that needed the second clause."""
+    om_g, om_r = np.sqrt(np.maximum(lam_gpu, 0)), np.sqrt(np.maximum(lam_ref, 0))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rel_ok = np.abs(om_g - om_r) <= 1e-9 * om_r
+    back_ok = np.abs(lam_gpu - lam_ref) <= 64 * EPS * lmax[:, None]
+    bad = ~(rel_ok | back_ok)
+    assert not bad.any(), (tag, np.argwhere(bad)[:5], lam_gpu[bad][:5], lam_ref[bad][:5])
+    return int((~rel_ok).sum())
+
+
+def oracle_inputs(cell):
+    comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu)
+    return cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho
+
+
+def test_compliance_matches_oracle(bs):
+    E, nu = np.array([1e9, 70e9, 3.5e9]), np.array([0.2, 0.33, 0.45])
+    assert np.allclose(bs.bs_isotropic_plane_strain(E, nu), oracle.isotropic_plane_strain_compliance(E, nu), rtol=1e-15)
+
+
+@pytest.mark.parametrize("name,Mt", [("C1", 3), ("C2", 3), ("C3", 4)])
+def test_table_and_matrices_parity(bs, name, Mt):
+    cell = wl.get(name).cells[0]
+    h = make_cell(bs, cell, Mt, 1)
+    bs.bs_assemble(h, Mt)
+    Phi, Psi = bs.bs_get_matrices(h)
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), Mt)
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+    assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    assert np.array_equal(Phi, Phi.conj().T) and np.array_equal(Psi, Psi.conj().T)   # exactly Hermitian by construction
+    # the table, channel by channel (general-D channel order of include/bs.h)
+    Dv = oracle.voigt_compliance(oracle_inputs(cell)[3])
+    W = np.stack([Dv[:, 0, 0], Dv[:, 1, 1], Dv[:, 0, 1], Dv[:, 0, 2], Dv[:, 1, 2], Dv[:, 2, 2], cell.rho])
+    tr = oracle.shape_integral_table(cell.lattice, cell.vert_offset, cell.verts, W, Mt)
+    tg = bs.bs_get_table(h)
+    for c in range(7):
+        scale = np.max(np.abs(tr[c]))
+        if scale == 0:
+            assert np.max(np.abs(tg[c])) == 0
+        else:
+            assert np.max(np.abs(tg[c] - tr[c])) <= 1e-12 * scale
+    bs.bs_destroy_cell(h)
+
+
+def test_anisotropic_matrices_parity(bs):
+    cell = wl.random_small_cell(21, 3, np.array([[1.0, 0.0], [0.3, 0.8]]))
+    comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu).copy()
+    comp[:, 3] = 0.01 * comp[:, 0]
+    comp[:, 4] = -0.02 * comp[:, 0]
+    comp[:, 1] *= 1.1
+    h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho)
+    bs.allocate_workspace(h, 2, 4)
+    bs.bs_assemble(h, 2)
+    Phi, Psi = bs.bs_get_matrices(h)
+    Pr, Sr = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho, 2)
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+    assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    kp = np.array([[0.1, 0.2], [0.5, 0.0], [0.0, 0.0], [0.33, 0.44]])
+    lam = bs.bs_bands(h, kp, 10)
+    for i, kr in enumerate(kp):
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, 2, kr, 10)
+        check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]))
+    bs.bs_destroy_cell(h)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_pencil_parity(bs, mode):
+    cell = wl.get("C1").cells[0]
+    h = make_cell(bs, cell, 3, 1, mode=mode)
+    bs.bs_assemble(h, 3)
+    Pr, _ = oracle.assemble(*oracle_inputs(cell), 3)
+    for kr in [(0.31, 0.12), (0.5, 0.5), (0.0, 0.0)]:
+        K = bs.bs_get_pencil(h, kr)
+        Kr = oracle.pencil_K(Pr, cell.lattice, 3, kr)
+        assert np.max(np.abs(K - Kr)) <= 1e-11 * np.max(np.abs(Kr))   # cond(Phi) ~ 1e2 amplifies the 1e-12 of Phi
+    bs.bs_destroy_cell(h)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("panel", [8, 32])
+def test_config1_bands_parity(bs, mode, panel):
+    w = wl.get("C1")
+    cell = w.cells[0]
+    h = make_cell(bs, cell, w.Mt, w.nk, mode=mode, panel=panel)
+    bs.bs_assemble(h, w.Mt)
+    lam = bs.bs_bands(h, w.kpts, w.nbands)
+    lr, lmax = oracle.band_structure(*oracle_inputs(cell), w.Mt, w.kpts, w.nbands)
+    n2 = check_bands(lam, lr, lmax, "C1")
+    assert n2 <= 8   # the two zero modes at each Gamma end (+ nearest neighbours)
+    bs.bs_destroy_cell(h)
+
+
+def test_homogeneous_dispersion_on_gpu(bs):
+    # physics pin applied directly to the CUDA path: omega = c |k+G|
+    E, nu, rho = 20e9, 0.28, 2500.0
+    cell = wl.homogeneous_cell(wl.HEXAGONAL, E, nu, rho, n=2)
+    Mt = 3
+    h = make_cell(bs, cell, Mt, 3)
+    bs.bs_assemble(h, Mt)
+    kp = np.array([(0.31, 0.12), (0.5, 0.0), (0.05, 0.45)])
+    nb = 2 * (2 * Mt + 1) ** 2
+    lam = bs.bs_bands(h, kp, nb)
+    lam_, mu_ = E * nu / ((1 + nu) * (1 - 2 * nu)), E / (2 * (1 + nu))
+    cL, cT = np.sqrt((lam_ + 2 * mu_) / rho), np.sqrt(mu_ / rho)
+    _, Q, _ = oracle.reciprocal_basis(cell.lattice)
+    for i, kr in enumerate(kp):
+        kap = np.linalg.norm((oracle.plane_wave_indices(Mt) + np.array(kr)) @ Q, axis=1)
+        ref = np.sort(np.concatenate([cL * kap, cT * kap]))
+        assert np.max(np.abs(np.sqrt(np.maximum(lam[i], 0)) - ref) / ref) < 1e-10
+    bs.bs_destroy_cell(h)
+
+
+def test_config2_bands_parity_sampled(bs):
+    w = wl.get("C2")
+    cell = w.cells[0]
+    h = make_cell(bs, cell, w.Mt, w.nk)
+    bs.bs_assemble(h, w.Mt)
+    lam = bs.bs_bands(h, w.kpts, w.nbands)
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), w.Mt)
+    Phi, Psi = bs.bs_get_matrices(h)
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+    assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    for i in [0, 1, 7, 20, 33, 59]:
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, w.Mt, w.kpts[i], w.nbands)
+        check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"C2 k{i}")
+    bs.bs_destroy_cell(h)
+
+
+def test_config3_bands_parity_sampled(bs):
+    w = wl.get("C3")
+    cell = w.cells[0]
+    h = make_cell(bs, cell, w.Mt, w.nk)
+    bs.bs_assemble(h, w.Mt)
+    lam = bs.bs_bands(h, w.kpts, w.nbands)
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), w.Mt)
+    for i in [0, 1, 45, 89]:
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, w.Mt, w.kpts[i], w.nbands)
+        check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"C3 k{i}")
+    bs.bs_destroy_cell(h)
+
+
+def test_config4_batch_parity_sampled(bs):
+    w = wl.get("C4", ncells=8)
+    cells = [make_cell(bs, c, w.Mt, w.nk) for c in w.cells]
+    bs.bs_assemble_batch(cells, w.Mt)
+    lam = bs.bs_bands_batch(cells, w.kpts, w.nbands)
+    assert lam.shape == (8, w.nk, w.nbands)
+    for ci in [0, 5, 7]:
+        Pr, Sr = oracle.assemble(*oracle_inputs(w.cells[ci]), w.Mt)
+        Phi, Psi = bs.bs_get_matrices(cells[ci])
+        assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+        for i in [0, 3, 21, 39]:
+            lr, lmax = oracle.bands_at_k(Pr, Sr, w.cells[ci].lattice, w.Mt, w.kpts[i], w.nbands)
+            check_bands(lam[ci, i:i + 1], lr[None, :], np.array([lmax]), f"C4 cell{ci} k{i}")
+    for c in cells:
+        bs.bs_destroy_cell(c)

@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py — k-points/s of the whole hot path (bs_assemble + bs_bands over every k-point of one workload).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl ours|reference]
+
+A "step" is one pass of the whole path (S1..S8 of DESIGN.md) over one workload: assembly of Phi/Psi and their
+factors, then the lowest `nbands` eigenvalues at every k-point.  `value` = k-points per second with the inputs already
+resident on the device; `e2e` = the same through the public API with HOST buffers (bs_create_cell copies the geometry
+in, bs_bands copies omega^2 out) inside the timed region.  Under torchrun each rank owns an interleaved share of a
+k-path N times denser (weak scaling, no data-path collective: DESIGN.md section 8).
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "k-points/sec (full nbands)"
+UNIT = "k-points/s"
+
+
+def dense_kpath(w: wl.Workload, world: int, rank: int) -> np.ndarray:
+    """Rank r's share of the workload's closed k-path sampled world x denser (indices r::world)."""
+    if world == 1:
+        return w.kpts
+    cell = w.cells[0]
+    path = wl.SQUARE_PATH if np.allclose(cell.lattice, wl.SQUARE) else wl.HEX_PATH
+    return np.ascontiguousarray(wl.kpath(cell.lattice, path, w.nk * world)[rank::world])
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.stop, self.thread = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.thread = threading.Thread(target=self._run, daemon=True)
+        self.thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.thread.join(timeout=6)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------ CPU oracle arm
+def oracle_sample(w: wl.Workload, kpts: np.ndarray, nsample: int):
+    """Times the oracle as it stands on a bounded sample: one assembly + `nsample` k-points spread over the path.
+    Returns (extrapolated whole-workload k-points/s, t_assemble, t_per_k, threads used)."""
+    import oracle
+    cell = w.cells[0]
+    t0 = time.perf_counter()
+    comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu)
+    Phi, Psi = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho, w.Mt)
+    t_asm = time.perf_counter() - t0
+    idx = np.unique(np.linspace(0, len(kpts) - 1, nsample).round().astype(int))
+    t0 = time.perf_counter()
+    for i in idx:
+        oracle.bands_at_k(Phi, Psi, cell.lattice, w.Mt, kpts[i], w.nbands)
+    t_k = (time.perf_counter() - t0) / len(idx)
+    nk_total = len(kpts) * len(w.cells)
+    total = len(w.cells) * t_asm + nk_total * t_k
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        threads = os.cpu_count() or 1
+    return nk_total / total, t_asm, t_k, threads, len(idx)
+
+
+def oracle_nsample(w: wl.Workload) -> int:
+    return {"C1": 30, "C2": 12, "C3": 6, "C4": 10, "C5": 3}.get(w.name, 4)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = wl.get(args.workload) if args.workload != "C4" else wl.get("C4", ncells=args.cells)
+    ns = oracle_nsample(w)
+    vals, t0 = [], time.perf_counter()
+    for i in range(args.warmup + args.steps):
+        v, t_asm, t_k, threads, nidx = oracle_sample(w, w.kpts, ns)
+        if i >= args.warmup:
+            vals.append(v)
+        if time.perf_counter() - t0 > 240 and vals:      # keep the whole run within a few minutes
+            break
+    value = float(np.mean(vals))
+    sample = (f"per step: 1 assembly (Mt={w.Mt}) + {nidx} of {w.nk} k-points (zhegv, all {2 * w.N} eigenvalues), "
+              f"extrapolated to the whole workload ({len(w.cells)} cell(s) x {w.nk} k-points)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": len(vals),
+            "warmup": args.warmup, "ms_per_step": 1e3 * w.nk * len(w.cells) / value, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name}: {w.description}"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+HBM_CLASSES = {"hemv", "expand", "pencil", "combine"}
+TENSOR_CLASSES = {"gemm_factor", "gemm_reduce", "gemm_tridiag"}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1310_6380_b200 as bs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    w = wl.get(args.workload) if args.workload != "C4" else wl.get("C4", ncells=args.cells)
+    kpts = dense_kpath(w, world, rank)
+    nk, ncell = len(kpts), len(w.cells)
+    comps = [bs.bs_isotropic_plane_strain(c.E, c.nu) for c in w.cells]
+
+    def create(timing):
+        hs = []
+        for c, comp in zip(w.cells, comps):
+            h = bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, comp, c.rho)
+            hs.append(h)
+        bs.bs_set_option(hs[0], bs.BS_OPT_TIMING, timing)
+        return hs
+
+    cells = create(2)
+    ws_bytes = bs.bs_workspace_bytes(cells[0], w.Mt, nk)
+    workspaces = [torch.empty(ws_bytes, dtype=torch.uint8, device="cuda") for _ in cells]
+    for h, t in zip(cells, workspaces):
+        bs.bs_set_workspace(h, t)
+    out_dev = torch.empty(ncell, nk, w.nbands, dtype=torch.float64, device="cuda")
+    kacc = {}
+    stage_acc = np.zeros(bs.BS_T_COUNT)
+
+    def accumulate():
+        for k, (ms, work, cnt) in bs.bs_get_kernel_timings(cells[0]).items():
+            a = kacc.setdefault(k, [0.0, 0.0, 0])
+            a[0] += ms; a[1] += work; a[2] += cnt
+
+    def step(record):
+        bs.bs_assemble_batch(cells, w.Mt)
+        if record:
+            accumulate()
+        bs.bs_bands_batch(cells, kpts, w.nbands, out=out_dev)
+        if record:
+            accumulate()
+            stage_acc[:] += bs.bs_get_timings(cells[0])
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dmma_peak, dfma_peak = bs.bs_fp64_peak()
+    for _ in range(max(args.warmup, 3)):
+        step(False)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = bs.bs_launch_count(cells[0])
+    barrier()
+    with ClockSampler(local) as clk:
+        e0.record()
+        for _ in range(args.steps):
+            step(True)
+        e1.record()
+        barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = bs.bs_launch_count(cells[0]) - l0
+    lam_dev = out_dev.cpu().numpy()
+
+    # ---- end to end through the public API with host buffers (H2D of the geometry, D2H of omega^2 inside the region)
+    for h in cells:
+        bs.bs_destroy_cell(h)
+    out_host = np.empty((ncell, nk, w.nbands))
+
+    def e2e_step():
+        hs = create(0)
+        for h, t in zip(hs, workspaces):
+            bs.bs_set_workspace(h, t)
+        bs.bs_assemble_batch(hs, w.Mt)
+        bs.bs_bands_batch(hs, kpts, w.nbands, out=out_host)
+        for h in hs:
+            bs.bs_destroy_cell(h)
+
+    e2e_step()
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record()
+    for _ in range(args.steps):
+        e2e_step()
+    f1.record()
+    barrier()
+    ms_e2e = f0.elapsed_time(f1)
+    assert np.array_equal(out_host, lam_dev), "e2e and device-resident results differ"
+    h2d = sum(c.lattice.nbytes + c.vert_offset.nbytes + c.verts.nbytes + comp.nbytes + c.rho.nbytes
+              for c, comp in zip(w.cells, comps)) + kpts.nbytes
+    d2h = out_host.nbytes
+
+    if world > 1:
+        t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_e2e = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    units = nk * ncell * world * args.steps
+    value = units / (ms_total * 1e-3)
+    hbm_peak, hbm_src = measured_peaks()
+    # ---- roofline of the dominant kernel class (largest share of device time inside the timed region)
+    tot_kernel_ms = sum(a[0] for a in kacc.values()) or 1.0
+    dom = max(kacc, key=lambda k: kacc[k][0])
+    ms_d, work_d, cnt_d = kacc[dom]
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(w.name, {}).get(dom)
+    if dom in TENSOR_CLASSES:
+        roof = {"bound": "tensor", "achieved": work_d / (ms_d * 1e9), "peak": dmma_peak, "unit": "TFLOP/s",
+                "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-only loop measured in this run by bs_fp64_peak; "
+                               "MEASURED_PEAKS.json has no FP64 entry"}
+    elif dom in HBM_CLASSES:
+        roof = {"bound": "hbm", "achieved": work_d / (ms_d * 1e6), "peak": hbm_peak, "unit": "GB/s", "peak_source": hbm_src}
+    else:
+        roof = {"bound": "alu", "achieved": None, "peak": dfma_peak, "unit": "TFLOP/s",
+                "peak_source": "FP64 DFMA register-only loop measured in this run by bs_fp64_peak"}
+    roof["frac"] = (roof["achieved"] / roof["peak"]) if roof["achieved"] else None
+    roof.update({"kernel": dom, "launches_per_step": cnt_d / args.steps, "avg_launch_ms": ms_d / max(cnt_d, 1),
+                 "share_of_kernel_time": ms_d / tot_kernel_ms, "traffic": traffic,
+                 "work_per_launch": work_d / max(cnt_d, 1)})
+    n = 2 * w.N
+    gemm_ms = sum(kacc[k][0] for k in TENSOR_CLASSES if k in kacc)
+    gemm_fl = sum(kacc[k][1] for k in TENSOR_CLASSES if k in kacc)
+    tri_ms = stage_acc[bs.BS_T_TRIDIAG]
+    tri_flops = 16.0 * n ** 3 / 3.0 * nk * ncell * args.steps
+    stages = {nme: stage_acc[i] / args.steps for i, nme in
+              enumerate(["table_ms", "expand_ms", "factor_ms", "coef_ms", "pencil_ms", "tridiag_ms", "bisect_ms"])}
+    stages["kernels"] = {k: {"ms_per_step": a[0] / args.steps, "launches_per_step": a[2] / args.steps}
+                         for k, a in kacc.items() if a[2]}
+    stages["fp64_tensor"] = {"all_dmma_gemm_tflops": gemm_fl / (gemm_ms * 1e9) if gemm_ms else None,
+                             "tridiag_algorithmic_tflops": tri_flops / (tri_ms * 1e9) if tri_ms else None,
+                             "tridiag_frac_of_dmma_peak": tri_flops / (tri_ms * 1e9) / dmma_peak if tri_ms else None,
+                             "dmma_peak_tflops": dmma_peak, "dfma_peak_tflops": dfma_peak}
+    # ---- CPU oracle on a bounded sample, rank 0, N = 1 only
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        v, t_asm, t_k, threads, nidx = oracle_sample(w, kpts, oracle_nsample(w))
+        cpu = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"1 assembly ({t_asm:.2f} s) + {nidx} of {nk} k-points ({t_k:.3f} s each, zhegv all "
+                         f"{n} eigenvalues), extrapolated to {ncell} cell(s) x {nk} k-points"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{w.name}: {w.description}", "kpoints_per_gpu": nk, "cells": ncell,
+                       "band_structure_wall_ms": ms_total / args.steps,
+                       "l2": f"inputs larger than L2: the per-step working set ({ncell * ws_bytes / 2**20:.0f} MiB workspace) "
+                             "exceeds the 126 MB L2" if ncell * ws_bytes > 2 * 126e6 else
+                             "working set fits L2 (small config): latency-bound, the roofline fraction is not meaningful"},
+            "clocks": clk.summary(),
+            "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                    "d2h_bytes_per_step": int(d2h)},
+            "gpu_launches": int(launches), "roofline": roof, "cpu_baseline": cpu, "stages": stages}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C3", choices=list(wl.CONFIGS))
+    ap.add_argument("--cells", type=int, default=256, help="number of cells of workload C4")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -42,7 +42,8 @@ typedef enum {
 typedef enum {
   BS_OPT_PENCIL_MODE = 0, /* 0 = BS_PENCIL_POLY (default), 1 = BS_PENCIL_DIRECT; see bs_bands */
   BS_OPT_PANEL = 1,       /* Householder panel width nb of the tridiagonalisation, 4..32, multiple of 4 (default 32) */
-  BS_OPT_TIMING = 2       /* 1 = record CUDA events around the stages (read back with bs_get_timings) */
+  BS_OPT_TIMING = 2       /* 1 = CUDA events around the stages (bs_get_timings); 2 = also around every kernel launch,
+                             summed per kernel class (bs_get_kernel_timings).  Both add a final stream synchronise. */
 } bs_option;
 enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
 
@@ -130,6 +131,27 @@ bs_status bs_get_tridiagonal(bs_cell *cell, double *d_host, double *e_host);
  * For a batch call the timings are recorded on cells[0]. */
 bs_status bs_get_timings(bs_cell *cell, double *ms_out);
 
+/* Kernel classes of bs_get_kernel_timings. */
+enum {
+  BS_KC_TABLE = 0,        /* S1 table kernel                                    work: 0 (ALU-bound)   */
+  BS_KC_EXPAND = 1,       /* S2 expansion                                       work: bytes written                  */
+  BS_KC_GEMM_FACTOR = 2,  /* DMMA zgemm launches of S3                          work: real flops                     */
+  BS_KC_GEMM_REDUCE = 3,  /* DMMA zgemm launches of S5 (and of the POLY coefficient reduction)                       */
+  BS_KC_GEMM_TRIDIAG = 4, /* DMMA zgemm launches of S6                          work: real flops                     */
+  BS_KC_HEMV = 5,         /* S6 Hermitian matrix-vector kernel                  work: bytes of the lower triangle    */
+  BS_KC_PANEL = 6,        /* S6 panel / reflector kernels                                                            */
+  BS_KC_STURM = 7,        /* S7                                                                                      */
+  BS_KC_PENCIL = 8,       /* S4 scaling kernel                                  work: bytes moved                    */
+  BS_KC_COMBINE = 9,      /* S4 polynomial combination (POLY mode)              work: bytes moved                    */
+  BS_KC_POTRF_DIAG = 10,  /* S3 diagonal-block factor kernel                                                         */
+  BS_KC_OTHER = 11,
+  BS_KC_COUNT = 12
+};
+/* Per-class totals of the last bs_assemble / bs_bands led by this handle under BS_OPT_TIMING = 2: device milliseconds
+ * (CUDA events on the call's stream around every launch), ALGORITHMIC work credited at launch time (flops or bytes, see
+ * the enum) and number of launches.  HOST out, BS_KC_COUNT entries each.  BS_ERR_STATE if timing mode 2 was never set. */
+bs_status bs_get_kernel_timings(bs_cell *cell, double *ms_out, double *work_out, int64_t *count_out);
+
 /* Number of kernel launches issued by the library on behalf of this handle since creation (batch: on cells[0]). */
 int64_t bs_launch_count(const bs_cell *cell);
 
@@ -156,6 +178,10 @@ bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d,
 /* Lowest nev eigenvalues of `batch` real symmetric tridiagonal matrices (d, e: DEVICE, batch x n) by Sturm bisection;
  * lam: DEVICE, batch x nev, ascending. */
 bs_status bs_sturm(int32_t n, const double *d, const double *e, int32_t nev, double *lam, int32_t batch, void *stream);
+
+/* FP64 roofline denominators of the current device, measured with register-only loops on `stream` (about 30 ms):
+ * DMMA (mma.sync m8n8k4 f64, the FP64 tensor pipe) and DFMA TFLOP/s.  HOST out.  Synchronises. */
+bs_status bs_fp64_peak(double *dmma_tflops, double *dfma_tflops, void *stream);
 
 enum {
   BS_GEMM_LOWER_ONLY = 1, /* compute only tiles that intersect the lower triangle of C */

@@ -25,8 +25,9 @@ BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_K
 SYMBOLS = [
     "bs_isotropic_plane_strain", "bs_create_cell", "bs_destroy_cell", "bs_set_option", "bs_workspace_bytes",
     "bs_set_workspace", "bs_assemble", "bs_assemble_batch", "bs_get_matrices", "bs_get_table", "bs_get_pencil",
-    "bs_bands", "bs_bands_batch", "bs_get_tridiagonal", "bs_get_timings", "bs_launch_count", "bs_last_error",
-    "bs_zgemm", "bs_zpotrf_trtri", "bs_zhetrd_scratch_elems", "bs_zhetrd", "bs_sturm",
+    "bs_bands", "bs_bands_batch", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
+    "bs_last_error",
+    "bs_fp64_peak", "bs_zgemm", "bs_zpotrf_trtri", "bs_zhetrd_scratch_elems", "bs_zhetrd", "bs_sturm",
 ]
 
 
@@ -65,6 +66,8 @@ lib.bs_bands.argtypes = [_vp, C.c_int32, _dp, C.c_int32, _vp, _vp]
 lib.bs_bands_batch.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int32, _dp, C.c_int32, _vp, _vp]
 lib.bs_get_tridiagonal.argtypes = [_vp, _dp, _dp]
 lib.bs_get_timings.argtypes = [_vp, _dp]
+lib.bs_get_kernel_timings.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int64)]
+lib.bs_fp64_peak.argtypes = [_dp, _dp, _vp]
 lib.bs_zgemm.argtypes = [C.c_int32] * 5 + [_dp, _vp, C.c_int32, C.c_int64, _vp, C.c_int32, C.c_int64, _dp, _vp, C.c_int32,
                                            C.c_int64, C.c_int32, C.c_int32, _vp]
 lib.bs_zpotrf_trtri.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, _vp, C.c_int32, _vp]
@@ -247,8 +250,27 @@ def bs_get_timings(cell: Cell) -> np.ndarray:
     return ms
 
 
+KERNEL_CLASSES = ["table", "expand", "gemm_factor", "gemm_reduce", "gemm_tridiag", "hemv", "panel", "sturm", "pencil",
+                  "combine", "potrf_diag", "other"]
+
+
+def bs_get_kernel_timings(cell: Cell) -> dict:
+    """{class: (ms, algorithmic work, launches)} of the last call led by ``cell`` under BS_OPT_TIMING = 2."""
+    n = len(KERNEL_CLASSES)
+    ms, work, cnt = np.zeros(n), np.zeros(n), np.zeros(n, dtype=np.int64)
+    _check(lib.bs_get_kernel_timings(cell.handle, _ptr(ms), _ptr(work), cnt.ctypes.data_as(C.POINTER(C.c_int64))))
+    return {k: (float(ms[i]), float(work[i]), int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
+
+
 def bs_launch_count(cell: Cell) -> int:
     return int(lib.bs_launch_count(cell.handle))
+
+
+def bs_fp64_peak(stream=None):
+    """(DMMA TFLOP/s, DFMA TFLOP/s) of the current device, measured now."""
+    a, b = C.c_double(0), C.c_double(0)
+    _check(lib.bs_fp64_peak(C.byref(a), C.byref(b), _stream(stream)))
+    return float(a.value), float(b.value)
 
 
 # ---- diagnostics on torch CUDA tensors (complex128, column-major = the transpose of a contiguous torch tensor)

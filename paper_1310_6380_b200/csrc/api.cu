@@ -9,6 +9,10 @@
 
 #include "bs_internal.cuh"
 
+namespace bsk {
+thread_local KTimer *g_kt = nullptr;
+}
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -95,6 +99,7 @@ struct bs_cell {
   size_t flat_cap = 0;
   int last_n = 0, last_nmat = 0, last_nk = 0;
   cudaEvent_t ev[BS_T_COUNT + 1] = {nullptr};
+  bsk::KTimer *kt = nullptr;  // BS_OPT_TIMING = 2
 };
 
 namespace {
@@ -146,6 +151,11 @@ void tick(bs_cell *c, int idx, cudaStream_t s) {
   if (!c->ev[idx]) cudaEventCreate(&c->ev[idx]);
   cudaEventRecord(c->ev[idx], s);
 }
+struct KtGuard {  // routes the launchers' KScope to the lead cell's timer for the duration of one call
+  explicit KtGuard(bs_cell *c) { bsk::g_kt = (c->timing == 2) ? c->kt : nullptr; if (bsk::g_kt) bsk::g_kt->reset(); }
+  ~KtGuard() { bsk::g_kt = nullptr; }
+};
+
 double tock(bs_cell *c, int a, int b) {
   float ms = 0.f;
   if (c->ev[a] && c->ev[b]) cudaEventElapsedTime(&ms, c->ev[a], c->ev[b]);
@@ -275,6 +285,7 @@ void bs_destroy_cell(bs_cell *c) {
   cudaFree(c->d_bases); cudaFree(c->d_geos); cudaFree(c->d_info); cudaFree(c->d_flat);
   for (auto &e : c->ev)
     if (e) cudaEventDestroy(e);
+  delete c->kt;
   delete c;
 }
 
@@ -292,7 +303,9 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       c->nb = value;
       return BS_OK;
     case BS_OPT_TIMING:
-      c->timing = value ? 1 : 0;
+      if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
+      c->timing = value;
+      if (value == 2 && !c->kt) c->kt = new bsk::KTimer();
       return BS_OK;
   }
   return fail(BS_ERR_ARG, "bs_set_option: unknown option %d", option);
@@ -316,6 +329,17 @@ bs_status bs_set_workspace(bs_cell *c, void *dev_ptr, size_t bytes) {
 }
 
 int64_t bs_launch_count(const bs_cell *c) { return c ? c->launches : 0; }
+
+bs_status bs_get_kernel_timings(bs_cell *c, double *ms_out, double *work_out, int64_t *count_out) {
+  if (!c || !ms_out || !work_out || !count_out) return fail(BS_ERR_ARG, "bs_get_kernel_timings: null argument");
+  if (!c->kt) return fail(BS_ERR_STATE, "bs_get_kernel_timings: set BS_OPT_TIMING = 2 first");
+  for (int i = 0; i < BS_KC_COUNT; ++i) {
+    ms_out[i] = c->kt->ms[i];
+    work_out[i] = c->kt->work[i];
+    count_out[i] = c->kt->count[i];
+  }
+  return BS_OK;
+}
 
 bs_status bs_get_timings(bs_cell *c, double *ms_out) {
   if (!c || !ms_out) return fail(BS_ERR_ARG, "bs_get_timings: null argument");
@@ -379,7 +403,7 @@ int reduce_blocks(bs_cell *lead, bs_cell *const *cells, int ncells, const Layout
   const long long blk[3] = {0, N, (long long)N * n2 + N};
   for (int b = 0; b < 3; ++b) {
     bsk::GemmDesc g{};
-    g.ncells = ncells; g.inner = inner;
+    g.ncells = ncells; g.inner = inner; g.kclass = bsk::KC_GEMM_REDUCE;
     g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
     // T = X_R * K_blk      (X_R lower: op(A)[m][k] = 0 for k > m)
     g.M = N; g.N = N; g.K = N; g.opA = 0; g.opB = 0;
@@ -435,6 +459,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   const int n3 = 3 * (int)N, n2 = 2 * (int)N, Ni = (int)N;
   auto R = [&](long long off, long long stride = 0) { return ref(lead, ncells, cells, off, stride); };
   int64_t nl = 0;
+  KtGuard ktg(lead);
 
   tick(lead, 0, s);
   bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), s); ++nl;  // S1
@@ -449,7 +474,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   nl += bsk::potrf_trtri(Ni, Ni, R(L.LR), R(L.XR), R(L.tmpR), R(L.dinvR), lead->d_info + ncells, 0, ncells, 1, s);
   {
     bsk::GemmDesc g{};
-    g.ncells = ncells; g.inner = 1;
+    g.ncells = ncells; g.inner = 1; g.kclass = bsk::KC_GEMM_FACTOR;
     g.M = n3; g.N = n3; g.K = n3; g.opA = 1; g.opB = 0;
     g.A = R(L.X); g.lda = n3; g.B = R(L.X); g.ldb = n3; g.C = R(L.Y); g.ldc = n3;
     g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
@@ -476,6 +501,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   tick(lead, 4, s);
   CU(cudaStreamSynchronize(s));
   CU(cudaGetLastError());
+  if (bsk::g_kt) bsk::g_kt->collect();
   std::vector<int> info(2 * ncells);
   CU(cudaMemcpy(info.data(), lead->d_info, sizeof(int) * 2 * ncells, cudaMemcpyDeviceToHost));
   lead->launches += nl;
@@ -577,6 +603,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   double *d = lead->d_flat, *e = d + nmat * n2, *scal = e + nmat * n2, *lam = scal + 2 * nmat, *coefk = lam + nmat * nbands;
   auto R = [&](long long off, long long stride = 0) { return ref(lead, ncells, cells, off, stride); };
   int64_t nl = 0;
+  KtGuard ktg(lead);
   const long long mat = (long long)n2 * n2;
 
   tick(lead, 0, s);
@@ -618,6 +645,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   CU(cudaMemcpyAsync(omega2_out, lam, nmat * nbands * sizeof(double),
                      on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
   if (!on_device || lead->timing) CU(cudaStreamSynchronize(s));
+  if (bsk::g_kt) bsk::g_kt->collect();
   if (lead->timing) {
     lead->ms[BS_T_PENCIL] = tock(lead, 0, 1);
     lead->ms[BS_T_TRIDIAG] = tock(lead, 1, 2);

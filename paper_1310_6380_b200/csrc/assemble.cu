@@ -89,6 +89,7 @@ void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, c
   const int L = 4 * Mt + 1;
   const int nhalf = (L * L + 1) / 2;
   dim3 grid((nhalf + 7) / 8, ncells);
+  KScope ks(KC_TABLE, 0.0, s);
   table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table);
 }
 
@@ -122,6 +123,7 @@ __global__ void __launch_bounds__(256) expand_kernel(int Mt, BatchRef table, Bat
 void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s) {
   const int W = 2 * Mt + 1, N = W * W;
   dim3 grid((N + 255) / 256, N, ncells);
+  KScope ks(KC_EXPAND, 160.0 * N * N * ncells, s);  // 9 + 1 blocks of N x N complex128 written once
   expand_kernel<<<grid, 256, 0, s>>>(Mt, table, Phi, R);
 }
 

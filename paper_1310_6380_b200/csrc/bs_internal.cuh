@@ -61,6 +61,55 @@ __device__ __forceinline__ cplx *batch_ptr(const BatchRef &r, int cell, int i) {
 // ---------------------------------------------------------------- kernels' host launchers (one per .cu)
 namespace bsk {
 
+// Per-kernel-class device timing (BS_OPT_TIMING = 2): CUDA events recorded on the launching stream around every launch
+// of a class, summed after the call's final synchronise.  `work` is the ALGORITHMIC work of the class (flops for the
+// DMMA classes, bytes for the HBM classes), accumulated on the host at launch time.
+enum KClass {
+  KC_TABLE = 0, KC_EXPAND, KC_GEMM_FACTOR, KC_GEMM_REDUCE, KC_GEMM_TRIDIAG, KC_HEMV, KC_PANEL, KC_STURM, KC_PENCIL,
+  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_COUNT
+};
+struct KTimer {
+  std::vector<cudaEvent_t> ev;   // pool; pairs (2i, 2i+1)
+  std::vector<int> cls;          // class of pair i
+  size_t used = 0;               // events used
+  double work[KC_COUNT] = {0};
+  double ms[KC_COUNT] = {0};
+  long long count[KC_COUNT] = {0};
+  void begin(int c, cudaStream_t s) {
+    if (used + 2 > ev.size()) {
+      const size_t old = ev.size();
+      ev.resize(old + 1024);
+      for (size_t i = old; i < ev.size(); ++i) cudaEventCreate(&ev[i]);
+    }
+    cls.resize(used / 2 + 1);
+    cls[used / 2] = c;
+    cudaEventRecord(ev[used], s);
+  }
+  void end(cudaStream_t s) { cudaEventRecord(ev[used + 1], s); used += 2; }
+  void reset() {
+    used = 0;
+    for (int i = 0; i < KC_COUNT; ++i) { work[i] = 0; ms[i] = 0; count[i] = 0; }
+  }
+  void collect() {  // call after the stream has been synchronised
+    for (size_t i = 0; i + 1 < used; i += 2) {
+      float t = 0.f;
+      cudaEventElapsedTime(&t, ev[i], ev[i + 1]);
+      ms[cls[i / 2]] += t;
+      count[cls[i / 2]] += 1;
+    }
+    used = 0;
+  }
+  ~KTimer() { for (auto e : ev) cudaEventDestroy(e); }
+};
+extern thread_local KTimer *g_kt;  // nullptr unless the current call runs with BS_OPT_TIMING = 2
+struct KScope {                    // RAII: times one launch of class c on stream s and credits `work` to it
+  cudaStream_t s; bool on;
+  KScope(int c, double work, cudaStream_t st) : s(st), on(g_kt != nullptr) {
+    if (on) { g_kt->work[c] += work; g_kt->begin(c, s); }
+  }
+  ~KScope() { if (on) g_kt->end(s); }
+};
+
 struct Geometry {  // device pointers, per cell
   const double *edge;   // SoA [6][nedge]: mh1, mh2 (fractional midpoint), eh1, eh2 (fractional edge), ex, ey (Cartesian edge)
   const int *ephase;    // [nedge] phase of each edge
@@ -77,6 +126,7 @@ void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R,
 
 struct GemmDesc {
   int M, N, K, opA, opB, lda, ldb, ldc, flags, inner, ncells;
+  int kclass;  // KClass the launch is timed under (0 -> KC_OTHER)
   cplx alpha, beta;
   BatchRef A, B, C;
 };

@@ -144,12 +144,13 @@ int potrf_trtri(int n, int lda, BatchRef A, BatchRef X, BatchRef tmp, BatchRef d
   // ---- Cholesky, right-looking
   for (int j0 = 0; j0 < n; j0 += NB) {
     const int nbk = n - j0 < NB ? n - j0 : NB;
-    potrf_diag_kernel<<<dim3(1, 1, ncells), 256, diag_smem, s>>>(n, lda, j0, A, dinv, info);
+    { KScope ks(KC_POTRF_DIAG, 0.0, s);
+      potrf_diag_kernel<<<dim3(1, 1, ncells), 256, diag_smem, s>>>(n, lda, j0, A, dinv, info); }
     ++launches;
     const int r = n - j0 - nbk;
     if (r <= 0) break;
     GemmDesc g{};
-    g.ncells = ncells; g.inner = 1;
+    g.ncells = ncells; g.inner = 1; g.kclass = KC_GEMM_FACTOR;
     // A21 <- A21 * inv(L11)^dagger
     g.M = r; g.N = nbk; g.K = nbk; g.opA = 0; g.opB = 1;
     g.A = shifted(A, (long long)(j0 + nbk) + (long long)j0 * lda); g.lda = lda;
@@ -179,7 +180,7 @@ int potrf_trtri(int n, int lda, BatchRef A, BatchRef X, BatchRef tmp, BatchRef d
       if (cnt <= 0 || s2 <= 0) continue;
       const long long pstride = (long long)2 * sz * (lda + 1);
       GemmDesc g{};
-      g.ncells = ncells; g.inner = cnt;
+      g.ncells = ncells; g.inner = cnt; g.kclass = KC_GEMM_FACTOR;
       // T = L21 X11   (X11 lower: k >= n)
       g.M = s2; g.N = sz; g.K = sz; g.opA = 0; g.opB = 0;
       g.A = shifted(A, (long long)(r0 + sz) + (long long)r0 * lda); g.A.stride = pstride; g.lda = lda;

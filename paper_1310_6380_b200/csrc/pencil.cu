@@ -72,6 +72,7 @@ void launch_pencil(int N, double V2, BatchRef Y, int ldy, BatchRef K, int ldk, B
                    int inner, cudaStream_t s) {
   const int bs = N >= 256 ? 256 : ((N + 31) / 32) * 32;
   dim3 grid((N + bs - 1) / bs, N, ncells * inner);
+  KScope ks(KC_PENCIL, 16.0 * (9.0 + 4.0) * N * N * ncells * inner, s);  // 9 blocks of Y read, 4 of K written
   pencil_kernel<<<grid, bs, 0, s>>>(N, V2, Y, ldy, K, ldk, kvec, nterm, inner);
 }
 
@@ -79,6 +80,7 @@ void launch_combine(int n, BatchRef Coef, long long coef_mat_stride, BatchRef Ak
                     int ncells, cudaStream_t s) {
   const int bs = n >= 256 ? 256 : ((n + 31) / 32) * 32;
   dim3 grid((n + bs - 1) / bs, n, ncells);
+  KScope ks(KC_COMBINE, 8.0 * n * (n + 1.0) * (6.0 + nk) * ncells, s);  // lower triangles: 6 read, nk written
   combine_kernel<<<grid, bs, 0, s>>>(n, Coef, coef_mat_stride, Ak, ld, coefk, nk);
 }
 

@@ -87,6 +87,7 @@ void launch_sturm(int n, const double *d, const double *e, int nev, double *lam,
     cudaFuncSetAttribute(sturm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     attr_done = true;
   }
+  KScope ks(KC_STURM, 0.0, s);
   sturm_kernel<<<nmat, ST, smem, s>>>(n, d, e, nev, lam);
 }
 

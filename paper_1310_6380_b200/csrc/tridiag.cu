@@ -232,10 +232,13 @@ int launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, BatchRef P, 
       // finish of the previous column of this panel (if any) fused with the reflector of column j
       const int ifin = i > 0 ? i - 1 : -1;
       const int tb0_fin = ifin >= 0 ? (j0 + ifin + 1) / TS : 0;
-      panel_step_kernel<<<nmat, PT, 0, s>>>(n, lda, nb, j0, ifin, i, tb0_fin, nblk, A, VW, P, d, e, scal, inner);
+      { KScope ks(KC_PANEL, 0.0, s);
+        panel_step_kernel<<<nmat, PT, 0, s>>>(n, lda, nb, j0, ifin, i, tb0_fin, nblk, A, VW, P, d, e, scal, inner); }
       ++launches;
       if (j + 1 < n) {
         const int tb0 = (j + 1) / TS, nt = nblk - tb0;
+        const double m = n - j - 1;
+        KScope ks(KC_HEMV, 8.0 * m * (m + 1.0) * nmat, s);  // bytes of the lower triangle read once
         hemv_kernel<<<dim3(nt, nt, nmat), NT, kHemvSmem, s>>>(n, lda, j, tb0, nblk, A, VW, i, P, inner);
         ++launches;
       }
@@ -247,7 +250,7 @@ int launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, BatchRef P, 
     ++launches;
     // A22 -= [V W] [W V]^H on the lower tiles
     GemmDesc g{};
-    g.ncells = ncells; g.inner = inner;
+    g.ncells = ncells; g.inner = inner; g.kclass = KC_GEMM_TRIDIAG;
     g.M = rem; g.N = rem; g.K = 2 * nb; g.opA = 0; g.opB = 1;
     g.A = VW; g.A.off += j0 + pn; g.lda = n;
     g.B = VW; g.B.off += (long long)nb * n + j0 + pn; g.ldb = n;

@@ -142,6 +142,10 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
 void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   if (g.M <= 0 || g.N <= 0 || g.ncells * g.inner <= 0) return;
   dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner);
+  double work = 8.0 * g.K * (double)g.ncells * g.inner;
+  work *= (g.flags & BS_GEMM_LOWER_ONLY) ? 0.5 * g.M * (g.M + 1.0) : (double)g.M * g.N;
+  if (g.flags & (BS_GEMM_KLO_ROW | BS_GEMM_KHI_ROW | BS_GEMM_KLO_COL | BS_GEMM_KHI_COL)) work *= 0.5;
+  KScope ks(g.kclass ? g.kclass : KC_OTHER, work, s);
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(zgemm_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);

@@ -41,11 +41,15 @@ typedef enum {
 /* Options for bs_set_option. */
 typedef enum {
   BS_OPT_PENCIL_MODE = 0, /* 0 = BS_PENCIL_POLY (default), 1 = BS_PENCIL_DIRECT; see bs_bands */
-  BS_OPT_PANEL = 1,       /* Householder panel width nb of the tridiagonalisation, 4..32, multiple of 4 (default 32) */
+  BS_OPT_PANEL = 1,       /* two-stage: band width b in {8, 16, 32} (default 32); one-stage: panel width 4..32, multiple of 4 */
   BS_OPT_TIMING = 2       /* 1 = CUDA events around the stages (bs_get_timings); 2 = also around every kernel launch,
                              summed per kernel class (bs_get_kernel_timings).  Both add a final stream synchronise. */
 } bs_option;
 enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
+/* BS_OPT_TRIDIAG (option 3): algorithm of S6.  0 = two-stage (dense -> band by DMMA GEMMs, band -> tridiagonal by bulge
+ * chasing; default), 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check). */
+enum { BS_OPT_TRIDIAG = 3 };
+enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1 };
 
 /* Stage indices of bs_get_timings (milliseconds, CUDA events on the call's stream). */
 enum {
@@ -145,7 +149,8 @@ enum {
   BS_KC_COMBINE = 9,      /* S4 polynomial combination (POLY mode)              work: bytes moved                    */
   BS_KC_POTRF_DIAG = 10,  /* S3 diagonal-block factor kernel                                                         */
   BS_KC_OTHER = 11,
-  BS_KC_COUNT = 12
+  BS_KC_BULGE = 12,       /* S6 stage 2: band -> tridiagonal bulge chasing                                           */
+  BS_KC_COUNT = 13
 };
 /* Per-class totals of the last bs_assemble / bs_bands led by this handle under BS_OPT_TIMING = 2: device milliseconds
  * (CUDA events on the call's stream around every launch), ALGORITHMIC work credited at launch time (flops or bytes, see
@@ -174,6 +179,7 @@ bs_status bs_zpotrf_trtri(int32_t n, void *A, int32_t lda, int64_t strideA, void
  * elements.  nb: panel width (clamped to 4..32).  Synchronises the stream before returning. */
 size_t bs_zhetrd_scratch_elems(int32_t n, int32_t nb);
 bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *scratch, int32_t nb,
+                    int32_t algo /* BS_TRIDIAG_* ; two-stage: nb is the band width, rounded to 8/16/32 */,
                     int32_t batch, void *stream);
 /* Lowest nev eigenvalues of `batch` real symmetric tridiagonal matrices (d, e: DEVICE, batch x n) by Sturm bisection;
  * lam: DEVICE, batch x nev, ascending. */
@@ -188,7 +194,8 @@ enum {
   BS_GEMM_KLO_ROW = 2,    /* op(A)[m][k] = 0 for k < m   (start the k loop at the tile's first row)   */
   BS_GEMM_KHI_ROW = 4,    /* op(A)[m][k] = 0 for k > m   (stop the k loop after the tile's last row)  */
   BS_GEMM_KLO_COL = 8,    /* op(B)[k][n] = 0 for k < n */
-  BS_GEMM_KHI_COL = 16    /* op(B)[k][n] = 0 for k > n */
+  BS_GEMM_KHI_COL = 16,   /* op(B)[k][n] = 0 for k > n */
+  BS_GEMM_A_HERM_LOWER = 32 /* A is M x M Hermitian, only its lower triangle is read (opA = opB = 0, K = M): HEMM */
 };
 
 #ifdef __cplusplus

@@ -16,10 +16,11 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libbs.so")
 
 BS_OK, BS_ERR_ARG, BS_ERR_GEOMETRY, BS_ERR_NOT_PD, BS_ERR_STATE, BS_ERR_CUDA, BS_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
-BS_OPT_PENCIL_MODE, BS_OPT_PANEL, BS_OPT_TIMING = 0, 1, 2
+BS_OPT_PENCIL_MODE, BS_OPT_PANEL, BS_OPT_TIMING, BS_OPT_TRIDIAG = 0, 1, 2, 3
+BS_TRIDIAG_TWO_STAGE, BS_TRIDIAG_ONE_STAGE = 0, 1
 BS_PENCIL_POLY, BS_PENCIL_DIRECT = 0, 1
 BS_T_TABLE, BS_T_EXPAND, BS_T_FACTOR, BS_T_COEF, BS_T_PENCIL, BS_T_TRIDIAG, BS_T_BISECT, BS_T_COUNT = 0, 1, 2, 3, 4, 5, 6, 8
-BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_KHI_COL = 1, 2, 4, 8, 16
+BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_KHI_COL, BS_GEMM_A_HERM_LOWER = 1, 2, 4, 8, 16, 32
 
 # every symbol include/bs.h declares (tests check that the library exports all of them)
 SYMBOLS = [
@@ -71,7 +72,7 @@ lib.bs_fp64_peak.argtypes = [_dp, _dp, _vp]
 lib.bs_zgemm.argtypes = [C.c_int32] * 5 + [_dp, _vp, C.c_int32, C.c_int64, _vp, C.c_int32, C.c_int64, _dp, _vp, C.c_int32,
                                            C.c_int64, C.c_int32, C.c_int32, _vp]
 lib.bs_zpotrf_trtri.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, _vp, C.c_int32, _vp]
-lib.bs_zhetrd.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, _vp]
+lib.bs_zhetrd.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
 lib.bs_sturm.argtypes = [C.c_int32, _vp, _vp, C.c_int32, _vp, C.c_int32, _vp]
 for _name in SYMBOLS:
     if _name not in ("bs_last_error", "bs_launch_count", "bs_zhetrd_scratch_elems", "bs_destroy_cell"):
@@ -251,7 +252,7 @@ def bs_get_timings(cell: Cell) -> np.ndarray:
 
 
 KERNEL_CLASSES = ["table", "expand", "gemm_factor", "gemm_reduce", "gemm_tridiag", "hemv", "panel", "sturm", "pencil",
-                  "combine", "potrf_diag", "other"]
+                  "combine", "potrf_diag", "other", "bulge"]
 
 
 def bs_get_kernel_timings(cell: Cell) -> dict:
@@ -290,9 +291,9 @@ def bs_zhetrd_scratch_elems(n: int, nb: int) -> int:
     return int(lib.bs_zhetrd_scratch_elems(n, nb))
 
 
-def bs_zhetrd(n, A, lda, strideA, d, e, scratch, nb=32, batch=1, stream=None):
+def bs_zhetrd(n, A, lda, strideA, d, e, scratch, nb=32, algo=BS_TRIDIAG_TWO_STAGE, batch=1, stream=None):
     _check(lib.bs_zhetrd(n, C.c_void_p(A.data_ptr()), lda, strideA, C.c_void_p(d.data_ptr()), C.c_void_p(e.data_ptr()),
-                         C.c_void_p(scratch.data_ptr()), nb, batch, _stream(stream)))
+                         C.c_void_p(scratch.data_ptr()), nb, algo, batch, _stream(stream)))
 
 
 def bs_sturm(n, d, e, nev, lam, batch=1, stream=None):

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <new>
 
 #include "bs_internal.cuh"
@@ -36,11 +37,13 @@ constexpr double kTwoPi = 6.283185307179586476925286766559;
 // Offsets (complex128 elements, each region 256-byte aligned) inside one cell's workspace.
 struct Layout {
   int Mt = -1, N = 0, nk = 0, mode = 0, nb = 32;
-  long long table, Phi, R, Lf, X, tmp, dinv, Y, LR, XR, tmpR, dinvR, kvecA, Coef, Tb, kvecK, Kk, Ak, VW, P;
+  long long table, Phi, R, Lf, X, tmp, dinv, Y, LR, XR, tmpR, dinvR, kvecA, Coef, Tb, kvecK, Kk, Ak, VW, P, SM, AB;
+  long long vw_stride, sm_stride, ab_stride;
   long long total;  // elements
 };
 
 long long align16(long long x) { return (x + 15) & ~15LL; }
+int band_width(int nb) { return nb >= 32 ? 32 : (nb >= 16 ? 16 : 8); }  // two-stage band width from BS_OPT_PANEL
 
 Layout make_layout(int Mt, int nk, int mode, int nb) {
   Layout L;
@@ -67,8 +70,14 @@ Layout make_layout(int Mt, int nk, int mode, int nb) {
   L.kvecK = take((long long)nk * 2 * N);  // nk x [2][2][N] doubles
   L.Kk = take(mode == BS_PENCIL_DIRECT ? (long long)nk * n2 * n2 : n2 * n2);  // POLY keeps one slot for bs_get_pencil
   L.Ak = take((long long)nk * n2 * n2);
-  L.VW = take((long long)nk * (long long)bsk::tridiag_vw_elems((int)n2, nb));
+  const int bw = band_width(nb);
+  L.vw_stride = (long long)std::max(bsk::tridiag_vw_elems((int)n2, nb), bsk::band_vw_elems((int)n2, bw));
+  L.sm_stride = align16((long long)bsk::band_sm_elems(bw));
+  L.ab_stride = align16((long long)bsk::band_ab_elems((int)n2, bw));
+  L.VW = take((long long)nk * L.vw_stride);
   L.P = take((long long)nk * (long long)bsk::tridiag_p_elems((int)n2));
+  L.SM = take((long long)nk * L.sm_stride);
+  L.AB = take((long long)nk * L.ab_stride);
   L.total = o;
   return L;
 }
@@ -82,7 +91,7 @@ struct bs_cell {
   int *d_ephase = nullptr;
   bsk::Geometry geo;
   bsk::Geometry *d_geo = nullptr;  // [1]
-  int mode = BS_PENCIL_POLY, nb = 32, timing = 0;
+  int mode = BS_PENCIL_POLY, nb = 32, timing = 0, algo = BS_TRIDIAG_TWO_STAGE;
   void *ws = nullptr;
   size_t ws_bytes = 0;
   Layout lay;            // layout of the last bs_assemble (lay.Mt < 0: not assembled)
@@ -302,6 +311,10 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       if (c->nb != value) c->assembled = false;
       c->nb = value;
       return BS_OK;
+    case BS_OPT_TRIDIAG:
+      if (value != BS_TRIDIAG_TWO_STAGE && value != BS_TRIDIAG_ONE_STAGE) return fail(BS_ERR_ARG, "bs_set_option: bad S6 algorithm");
+      c->algo = value;
+      return BS_OK;
     case BS_OPT_TIMING:
       if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
       c->timing = value;
@@ -429,7 +442,7 @@ bs_status check_batch(bs_cell *const *cells, int ncells, const char *who) {
   for (int c = 0; c < ncells; ++c) {
     if (!cells[c]) return fail(BS_ERR_ARG, "%s: cells[%d] is null", who, c);
     if (!cells[c]->ws) return fail(BS_ERR_NOMEM, "%s: cells[%d] has no workspace (bs_set_workspace)", who, c);
-    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb)
+    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb || cells[c]->algo != cells[0]->algo)
       return fail(BS_ERR_ARG, "%s: cells[%d] has different options than cells[0]", who, c);
   }
   return BS_OK;
@@ -630,8 +643,15 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
     nl += reduce_blocks(lead, cells, ncells, L, L.Kk, L.Ak, nk, s);                                                        // S5
   }
   tick(lead, 1, s);
-  nl += bsk::launch_tridiag(n2, n2, lead->nb, R(L.Ak, mat), R(L.VW, (long long)bsk::tridiag_vw_elems(n2, lead->nb)),
-                            R(L.P, (long long)bsk::tridiag_p_elems(n2)), d, e, scal, ncells, nk, s);  // S6
+  if (lead->algo == BS_TRIDIAG_ONE_STAGE) {
+    nl += bsk::launch_tridiag(n2, n2, lead->nb, R(L.Ak, mat), R(L.VW, L.vw_stride),
+                              R(L.P, (long long)bsk::tridiag_p_elems(n2)), d, e, scal, ncells, nk, s);  // S6
+  } else {
+    const int bw = band_width(lead->nb);
+    nl += bsk::launch_sy2sb(n2, n2, bw, R(L.Ak, mat), R(L.VW, L.vw_stride), R(L.SM, L.sm_stride), R(L.AB, L.ab_stride),
+                            ncells, nk, s);                                                             // S6 stage 1
+    bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s); ++nl;                         // S6 stage 2
+  }
   tick(lead, 2, s);
   bsk::launch_sturm(n2, d, e, nbands, lam, (int)nmat, s); ++nl;                                       // S7
   tick(lead, 3, s);
@@ -681,6 +701,7 @@ bs_status bs_zgemm(int32_t opA, int32_t opB, int32_t M, int32_t N, int32_t K, co
                    int32_t lda, int64_t strideA, const void *B, int32_t ldb, int64_t strideB, const double beta[2],
                    void *C, int32_t ldc, int64_t strideC, int32_t batch, int32_t flags, void *stream) {
   if (!A || !B || !C || !alpha || !beta || M < 0 || N < 0 || K < 0 || batch < 1) return fail(BS_ERR_ARG, "bs_zgemm: bad argument");
+  if ((flags & BS_GEMM_A_HERM_LOWER) && (opA || opB || K != M)) return fail(BS_ERR_ARG, "bs_zgemm: HERM_LOWER needs opA = opB = 0 and K = M");
   bsk::GemmDesc g{};
   g.M = M; g.N = N; g.K = K; g.opA = opA; g.opB = opB; g.lda = lda; g.ldb = ldb; g.ldc = ldc; g.flags = flags;
   g.ncells = 1; g.inner = batch;
@@ -720,18 +741,31 @@ size_t bs_zhetrd_scratch_elems(int32_t n, int32_t nb) {
   if (n < 1) return 0;
   if (nb < 4) nb = 4;
   if (nb > 32) nb = 32;
-  return bsk::tridiag_vw_elems(n, nb) + bsk::tridiag_p_elems(n) + 16;
+  const int bw = band_width(nb);
+  return std::max(bsk::tridiag_vw_elems(n, nb), bsk::band_vw_elems(n, bw)) + bsk::tridiag_p_elems(n) +
+         align16((long long)bsk::band_sm_elems(bw)) + align16((long long)bsk::band_ab_elems(n, bw)) + 16;
 }
 
 bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *scratch, int32_t nb,
-                    int32_t batch, void *stream) {
+                    int32_t algo, int32_t batch, void *stream) {
   if (!A || !d || !e || !scratch || n < 1 || n > 2048 || batch < 1 || lda < n) return fail(BS_ERR_ARG, "bs_zhetrd: bad argument");
   if (nb < 4) nb = 4;
   if (nb > 32) nb = 32;
-  const long long vw = (long long)bsk::tridiag_vw_elems(n, nb), pp = (long long)bsk::tridiag_p_elems(n);
-  const long long per = vw + pp + 16;
+  const int bw = band_width(nb);
+  const long long vw = (long long)std::max(bsk::tridiag_vw_elems(n, nb), bsk::band_vw_elems(n, bw));
+  const long long pp = (long long)bsk::tridiag_p_elems(n);
+  const long long smn = align16((long long)bsk::band_sm_elems(bw)), abn = align16((long long)bsk::band_ab_elems(n, bw));
+  const long long per = (long long)bs_zhetrd_scratch_elems(n, nb);
   cplx *sc = (cplx *)scratch;
   BatchRef VW = raw(sc, per), P = raw(sc + vw, per);
+  if (algo == BS_TRIDIAG_TWO_STAGE) {
+    BatchRef SMr = raw(sc + vw + pp, per), ABr = raw(sc + vw + pp + smn, per);
+    bsk::launch_sy2sb(n, lda, bw, raw(A, strideA), VW, SMr, ABr, 1, batch, (cudaStream_t)stream);
+    bsk::launch_sb2st(n, bw, ABr, d, e, 1, batch, (cudaStream_t)stream);
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    CU(cudaGetLastError());
+    return BS_OK;
+  }
   // tau of the pending reflector: the 16 spare elements of matrix 0's slot hold nothing else; use a strided view
   // (scal is indexed [2*z]), so place it after all per-matrix slots is not possible without more memory: use slot tails.
   double *scal = nullptr;

@@ -66,7 +66,7 @@ namespace bsk {
 // DMMA classes, bytes for the HBM classes), accumulated on the host at launch time.
 enum KClass {
   KC_TABLE = 0, KC_EXPAND, KC_GEMM_FACTOR, KC_GEMM_REDUCE, KC_GEMM_TRIDIAG, KC_HEMV, KC_PANEL, KC_STURM, KC_PENCIL,
-  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_COUNT
+  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_BULGE, KC_COUNT
 };
 struct KTimer {
   std::vector<cudaEvent_t> ev;   // pool; pairs (2i, 2i+1)
@@ -155,6 +155,14 @@ size_t tridiag_vw_elems(int n, int nb);
 size_t tridiag_p_elems(int n);
 int launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, BatchRef P, double *d, double *e, double *scal,
                    int ncells, int inner, cudaStream_t s);
+// S6, two-stage (band.cu, bulge.cu): dense -> band of width b (b in {8,16,32}) -> tridiagonal.
+// VW: per matrix band_vw_elems, SM: per matrix band_sm_elems, AB: per matrix band_ab_elems complex.
+size_t band_vw_elems(int n, int b);
+size_t band_sm_elems(int b);
+size_t band_ab_elems(int n, int b);
+int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, BatchRef AB, int ncells, int inner,
+                 cudaStream_t s);
+void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s);
 // S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
 void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s);
 

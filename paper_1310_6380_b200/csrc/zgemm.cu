@@ -26,7 +26,9 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
                : "d"(a), "d"(b));
 }
 
-template <int OPA, int OPB>
+// HERM = 1: A is an M x M Hermitian matrix of which only the LOWER triangle is valid (K == M, OPA == 0):
+//   op(A)[m][k] = A[m][k] for m > k, Re A[m][m] for m == k, conj(A[k][m]) for m < k  (the HEMM of the band reduction).
+template <int OPA, int OPB, int HERM>
 __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx(*As)[BK][LDS] = reinterpret_cast<cplx(*)[BK][LDS]>(smem_raw);
@@ -55,10 +57,13 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
 #pragma unroll
     for (int r = 0; r < 2; ++r) {
       int m, k;
-      if (OPA == 0) { m = t & 63; k = (t >> 6) + 4 * r; } else { k = t & 7; m = (t >> 3) + 32 * r; }
+      bool tr = OPA != 0;                                  // read the element from its transposed position
+      if (HERM && k0 >= m0 + BM - 1) tr = true;            // the whole k-tile lies above the diagonal
+      if (!tr) { m = t & 63; k = (t >> 6) + 4 * r; } else { k = t & 7; m = (t >> 3) + 32 * r; }
+      if (HERM && !tr && k0 + BK - 1 > m0) tr = (k0 + k > m0 + m);   // tile crossing the diagonal: per element
       const bool ok = (m0 + m < g.M) && (k0 + k < khi);
-      const cplx *src = OPA == 0 ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
-                                 : A + (size_t)(k0 + k) + (size_t)(m0 + m) * g.lda;
+      const cplx *src = !tr ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
+                            : A + (size_t)(k0 + k) + (size_t)(m0 + m) * g.lda;
       cp_async16(&As[stage][k][m], ok ? src : A, ok);
     }
 #pragma unroll
@@ -96,6 +101,11 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
       for (int mi = 0; mi < 2; ++mi) {
         a[mi] = As[st][kk + (lane & 3)][wm * 16 + mi * 8 + (lane >> 2)];
         if (OPA) a[mi].y = -a[mi].y;
+        if (HERM) {
+          const int mg = m0 + wm * 16 + mi * 8 + (lane >> 2), kg = klo + kt * BK + kk + (lane & 3);
+          if (kg > mg) a[mi].y = -a[mi].y;
+          else if (kg == mg) a[mi].y = 0.0;
+        }
       }
 #pragma unroll
       for (int ni = 0; ni < 4; ++ni) {
@@ -148,16 +158,21 @@ void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   KScope ks(g.kclass ? g.kclass : KC_OTHER, work, s);
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(zgemm_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<0, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<0, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<1, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<1, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaFuncSetAttribute(zgemm_kernel<0, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
     attr_done = true;
   }
-  if (g.opA == 0 && g.opB == 0) zgemm_kernel<0, 0><<<grid, NT, kSmem, s>>>(g);
-  else if (g.opA == 0 && g.opB == 1) zgemm_kernel<0, 1><<<grid, NT, kSmem, s>>>(g);
-  else if (g.opA == 1 && g.opB == 0) zgemm_kernel<1, 0><<<grid, NT, kSmem, s>>>(g);
-  else zgemm_kernel<1, 1><<<grid, NT, kSmem, s>>>(g);
+  if (g.flags & BS_GEMM_A_HERM_LOWER) {  // requires opA == 0, opB == 0, K == M
+    zgemm_kernel<0, 0, 1><<<grid, NT, kSmem, s>>>(g);
+    return;
+  }
+  if (g.opA == 0 && g.opB == 0) zgemm_kernel<0, 0, 0><<<grid, NT, kSmem, s>>>(g);
+  else if (g.opA == 0 && g.opB == 1) zgemm_kernel<0, 1, 0><<<grid, NT, kSmem, s>>>(g);
+  else if (g.opA == 1 && g.opB == 0) zgemm_kernel<1, 0, 0><<<grid, NT, kSmem, s>>>(g);
+  else zgemm_kernel<1, 1, 0><<<grid, NT, kSmem, s>>>(g);
 }
 
 }  // namespace bsk

@@ -47,6 +47,24 @@ def test_zgemm(bs, opA, opB, M, N, K):
     assert np.max(np.abs(got - ref)) <= 1e-13 * K * np.max(np.abs(ref))
 
 
+@pytest.mark.parametrize("M,N", [(64, 32), (200, 32), (333, 17), (130, 64)])
+def test_zgemm_hermitian_lower(bs, M, N):
+    # HEMM: only the lower triangle of A is read (the upper one holds garbage), diagonal imaginary parts are ignored
+    import torch
+    rng = np.random.default_rng(M + N)
+    G = rand_c(rng, M, M)
+    H = G + G.conj().T
+    stored = np.tril(H) + np.triu(rand_c(rng, M, M), 1) + 1j * np.diag(rng.normal(size=M))
+    Bm = rand_c(rng, M, N)
+    dA, dB = to_dev(stored), to_dev(Bm)
+    dC = torch.zeros(N, M, dtype=torch.complex128, device="cuda")
+    bs.bs_zgemm(0, 0, M, N, M, 1.0, dA, M, 0, dB, M, 0, 0.0, dC, M, 0, 1, bs.BS_GEMM_A_HERM_LOWER)
+    torch.cuda.synchronize()
+    Hc = H - 1j * np.diag(np.diag(H).imag)
+    ref = Hc @ Bm
+    assert np.max(np.abs(from_dev(dC) - ref)) <= 1e-13 * M * np.max(np.abs(ref))
+
+
 def test_zgemm_batched_lower_only(bs):
     import torch
     rng = np.random.default_rng(5)
@@ -105,11 +123,15 @@ def test_zpotrf_reports_not_pd(bs):
     assert int(info.cpu()[0]) == 67
 
 
-@pytest.mark.parametrize("n,nb", [(5, 4), (64, 8), (98, 32), (242, 32), (450, 16), (130, 32)])
-def test_zhetrd_eigenvalues(bs, n, nb):
+@pytest.mark.parametrize("algo", [0, 1])
+@pytest.mark.parametrize("n,nb", [(1, 8), (2, 8), (5, 4), (9, 8), (64, 8), (98, 32), (242, 32), (242, 16), (450, 16), (130, 32),
+                                  (333, 8), (700, 32)])
+def test_zhetrd_eigenvalues(bs, n, nb, algo):
     import torch
     rng = np.random.default_rng(n + nb)
     batch = 3
+    if algo == 1 and nb % 4:
+        pytest.skip("one-stage panel must be a multiple of 4")
     mats = []
     for _ in range(batch):
         G = rand_c(rng, n, n)
@@ -118,7 +140,7 @@ def test_zhetrd_eigenvalues(bs, n, nb):
     d = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
     e = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
     scratch = torch.zeros(batch * bs.bs_zhetrd_scratch_elems(n, nb), dtype=torch.complex128, device="cuda")
-    bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, batch)
+    bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, algo, batch)
     torch.cuda.synchronize()
     for b in range(batch):
         dd, ee = d[b].cpu().numpy(), e[b].cpu().numpy()[:n - 1]

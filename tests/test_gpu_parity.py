@@ -19,13 +19,15 @@ def bs():
     return bs
 
 
-def make_cell(bs, cell, Mt, nk, mode=None, panel=None):
+def make_cell(bs, cell, Mt, nk, mode=None, panel=None, algo=None):
     comp = bs.bs_isotropic_plane_strain(cell.E, cell.nu)
     h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho)
     if mode is not None:
         bs.bs_set_option(h, bs.BS_OPT_PENCIL_MODE, mode)
     if panel is not None:
         bs.bs_set_option(h, bs.BS_OPT_PANEL, panel)
+    if algo is not None:
+        bs.bs_set_option(h, bs.BS_OPT_TRIDIAG, algo)
     bs.allocate_workspace(h, Mt, nk)
     return h
 
@@ -111,11 +113,12 @@ def test_pencil_parity(bs, mode):
 
 
 @pytest.mark.parametrize("mode", [0, 1])
-@pytest.mark.parametrize("panel", [8, 32])
-def test_config1_bands_parity(bs, mode, panel):
+@pytest.mark.parametrize("panel", [8, 16, 32])
+@pytest.mark.parametrize("algo", [0, 1])
+def test_config1_bands_parity(bs, mode, panel, algo):
     w = wl.get("C1")
     cell = w.cells[0]
-    h = make_cell(bs, cell, w.Mt, w.nk, mode=mode, panel=panel)
+    h = make_cell(bs, cell, w.Mt, w.nk, mode=mode, panel=panel, algo=algo)
     bs.bs_assemble(h, w.Mt)
     lam = bs.bs_bands(h, w.kpts, w.nbands)
     lr, lmax = oracle.band_structure(*oracle_inputs(cell), w.Mt, w.kpts, w.nbands)
@@ -160,10 +163,11 @@ def test_config2_bands_parity_sampled(bs):
     bs.bs_destroy_cell(h)
 
 
-def test_config3_bands_parity_sampled(bs):
+@pytest.mark.parametrize("algo,panel", [(0, 32), (0, 16), (1, 32)])
+def test_config3_bands_parity_sampled(bs, algo, panel):
     w = wl.get("C3")
     cell = w.cells[0]
-    h = make_cell(bs, cell, w.Mt, w.nk)
+    h = make_cell(bs, cell, w.Mt, w.nk, algo=algo, panel=panel)
     bs.bs_assemble(h, w.Mt)
     lam = bs.bs_bands(h, w.kpts, w.nbands)
     Pr, Sr = oracle.assemble(*oracle_inputs(cell), w.Mt)

@@ -27,54 +27,83 @@ __device__ __forceinline__ double warp_sum(double x) {
   return x;
 }
 
-// LAPACK zlarfg on a vector spread over the lanes (x valid for lane < len; others must hold 0):
+// Sum over the B consecutive lanes that hold one vector (B = 8, 16 or 32); every lane of the group gets the same bits.
+template <int B>
+__device__ __forceinline__ double group_sum(double x) {
+#pragma unroll
+  for (int o = B / 2; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+  return x;
+}
+
+// LAPACK zlarfg on a vector spread over a group of B lanes (x valid for l < len; others must hold 0):
 // H = I - tau v v^H, H^H x = beta e_1, beta real, v[0] = 1.  Returns v in x.
-__device__ __forceinline__ void warp_larfg(cplx &x, int len, int lane, cplx &tau, double &beta) {
-  const double mine = (lane >= 1 && lane < len) ? x.x * x.x + x.y * x.y : 0.0;
-  const double ss = warp_sum(mine);
-  const cplx al = shfl_c(x, 0);
+template <int B>
+__device__ __forceinline__ void group_larfg(cplx &x, int len, int l, cplx &tau, double &beta) {
+  const double mine = (l >= 1 && l < len) ? x.x * x.x + x.y * x.y : 0.0;
+  const double ss = group_sum<B>(mine);
+  const int base = (threadIdx.x & 31) & ~(B - 1);
+  const cplx al = shfl_c(x, base);
   if (ss == 0.0 && al.y == 0.0) {
     tau = cmake(0.0, 0.0);
     beta = al.x;
-    x = (lane == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+    x = (l == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
     return;
   }
   beta = -copysign(sqrt(al.x * al.x + al.y * al.y + ss), al.x);
   tau = cmake((beta - al.x) / beta, -al.y / beta);
   const double dr = al.x - beta, di = al.y, den = 1.0 / (dr * dr + di * di);
   const cplx scale = cmake(dr * den, -di * den);
-  if (lane == 0) x = cmake(1.0, 0.0);
-  else if (lane < len) x = cmul(x, scale);
+  if (l == 0) x = cmake(1.0, 0.0);
+  else if (l < len) x = cmul(x, scale);
   else x = cmake(0.0, 0.0);
 }
 
+// Team of 4B threads per sweep: thread (l, q), l = index inside the B x B block (row or column), q = quarter of the
+// other dimension (QN = B/4 indices each).  Vectors (v, w, u, v2) are computed redundantly by the four q-replicas.
 template <int B>
-__global__ void __launch_bounds__(512) bulge_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc, int inner) {
-  constexpr int LD = 2 * B;
+__global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc,
+                                                                     int inner) {
+  constexpr int LD = 2 * B, TT = 4 * B, QN = B / 4;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *ring = reinterpret_cast<cplx *>(smem_raw);
   const int z = blockIdx.x, cell = z / inner, mi = z % inner;
   cplx *ab = batch_ptr(AB, cell, mi);
   double *dg = d + (size_t)z * n, *eg = e + (size_t)z * n;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const bool is_io = warp >= G;
-  const int io_tid = tid - G * 32, io_nt = NIO * 32;
+  const int tid = threadIdx.x;
+  const int ncomp = G * TT;
+  const bool is_io = tid >= ncomp;
+  const int io_tid = tid - ncomp, io_nt = blockDim.x - ncomp;
+  const int team = tid / TT, tt = tid % TT, l = tt % B, q = tt / B;
+  // team scratch behind the ring: vs, ws, tus, v2s (B each), red1, red2, red3 (4B each) = 16 B complex per team
+  cplx *ts = ring + (size_t)Wc * LD + (size_t)(is_io ? 0 : team) * 16 * B;
+  cplx *vs = ts, *ws = ts + B, *tus = ts + 2 * B, *v2s = ts + 3 * B;
+  cplx *red1 = ts + 4 * B, *red2 = ts + 8 * B, *red3 = ts + 12 * B;
+  auto team_bar = [&]() {
+    if (TT == 32) __syncwarp();
+    else asm volatile("bar.sync %0, %1;\n" ::"r"(team + 1), "r"(TT) : "memory");
+  };
   const bool resident = n <= Wc;
 
   int wlo = 0, whi = 0;  // ring holds columns [wlo, whi)  (uniform over the CTA)
   auto slot_of = [&](int c) { return c % Wc; };
+  // column ranges are copied as one flat index space so that every thread has several independent 16-byte
+  // transfers in flight (cp.async: global -> shared without register staging)
   auto io_load = [&](int c0, int c1, int t, int nt) {
-    for (int c = c0; c < c1; ++c) {
-      const cplx *src = ab + (size_t)c * LD;
-      cplx *dst = ring + (size_t)slot_of(c) * LD;
-      for (int q = t; q < LD; q += nt) dst[q] = src[q];
+    const int total = (c1 - c0) * LD;
+    for (int qq = t; qq < total; qq += nt) {
+      const int c = c0 + qq / LD, off = qq % LD;
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + (size_t)slot_of(c) * LD + off);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(ab + (size_t)c * LD + off));
     }
+    asm volatile("cp.async.commit_group;\n" ::);
+    asm volatile("cp.async.wait_group 0;\n" ::: "memory");
   };
   auto io_evict = [&](int c0, int c1, int t, int nt) {
-    for (int c = c0; c < c1; ++c) {
-      cplx *dst = ab + (size_t)c * LD;
-      const cplx *src = ring + (size_t)slot_of(c) * LD;
-      for (int q = t; q < LD; q += nt) dst[q] = src[q];
+    const int total = (c1 - c0) * LD;
+#pragma unroll 4
+    for (int qq = t; qq < total; qq += nt) {
+      const int c = c0 + qq / LD, off = qq % LD;
+      ab[(size_t)c * LD + off] = ring[(size_t)slot_of(c) * LD + off];
     }
   };
 
@@ -100,9 +129,9 @@ __global__ void __launch_bounds__(512) bulge_kernel(int n, BatchRef AB, double *
       }
       __syncthreads();
     }
-    // per-warp sweep state
-    const int i = t0 + warp;
-    const bool valid = !is_io && warp < nvalid;
+    // per-team sweep state (identical in all threads of a team)
+    const int i = t0 + team;
+    const bool valid = !is_io && team < nvalid;
     int k = 0, J = i + 1, L = 0;
     bool finished = !valid;
     cplx v = cmake(0.0, 0.0), tau = cmake(0.0, 0.0);
@@ -110,137 +139,146 @@ __global__ void __launch_bounds__(512) bulge_kernel(int n, BatchRef AB, double *
     const int S = nsteps0 + 2 * (nvalid - 1);
 
     for (int s = 0; s < S; ++s) {
-      if (is_io) {
-        if (!resident) {
-          // columns still needed at macro-step s or later / needed at macro-step s+1
-          int keep = n, hi = whi;
-          for (int g = 0; g < nvalid; ++g) {
-            const int ig = t0 + g, kg = s - 2 * g, ns = (n - 1 - ig + B - 1) / B;
-            if (kg >= ns) continue;  // finished
-            keep = min(keep, kg <= 0 ? ig : ig + 1 + kg * B);
-            const int k1 = kg + 1;
-            if (k1 >= 0 && k1 < ns) hi = max(hi, min(n, ig + 1 + (k1 + 1) * B));
-          }
-          keep = max(keep, wlo);
+      if (!resident) {  // window bookkeeping (uniform): columns needed at macro-step s or later / at s+1
+        int keep = n, hi = whi;
+        for (int g = 0; g < nvalid; ++g) {
+          const int ig = t0 + g, kg = s - 2 * g, ns = (n - 1 - ig + B - 1) / B;
+          if (kg >= ns) continue;  // finished
+          keep = min(keep, kg <= 0 ? ig : ig + 1 + kg * B);
+          const int k1 = kg + 1;
+          if (k1 >= 0 && k1 < ns) hi = max(hi, min(n, ig + 1 + (k1 + 1) * B));
+        }
+        keep = max(keep, wlo);
+        if (is_io) {
           io_evict(max(wlo, t0 + nvalid), keep, io_tid, io_nt);  // columns < t0+nvalid are finished
           io_load(whi, hi, io_tid, io_nt);
-          wlo = keep; whi = hi;
         }
-      } else {
-        if (!resident) {  // mirror the window bookkeeping (uniform values; compute warps only need them at train change)
-          int keep = n, hi = whi;
-          for (int g = 0; g < nvalid; ++g) {
-            const int ig = t0 + g, kg = s - 2 * g, ns = (n - 1 - ig + B - 1) / B;
-            if (kg >= ns) continue;
-            keep = min(keep, kg <= 0 ? ig : ig + 1 + kg * B);
-            const int k1 = kg + 1;
-            if (k1 >= 0 && k1 < ns) hi = max(hi, min(n, ig + 1 + (k1 + 1) * B));
-          }
-          wlo = max(keep, wlo); whi = hi;
+        wlo = keep; whi = hi;
+      }
+      if (!finished && s >= 2 * team) {
+        // -------------------------------------------------------------------- one step of sweep i
+        if (k == 0) {
+          L = min(B, n - 1 - i);
+          const cplx *ci = ring + (size_t)slot_of(i) * LD;
+          cplx x = l < L ? ci[1 + l] : cmake(0.0, 0.0);
+          double beta;
+          group_larfg<B>(x, L, l, tau, beta);
+          v = x;
+          if (tt == 0) { eg[i] = beta; dg[i] = ci[0].x; }
+          if (q == 0) vs[l] = v;
+          team_bar();
         }
-        if (!finished && s >= 2 * warp) {
-          // ------------------------------------------------------------------ one step of sweep i
-          if (k == 0) {
-            L = min(B, n - 1 - i);
-            const cplx *ci = ring + (size_t)slot_of(i) * LD;
-            cplx x = lane < L ? ci[1 + lane] : cmake(0.0, 0.0);
-            double beta;
-            warp_larfg(x, L, lane, tau, beta);
-            v = x;
-            if (lane == 0) { eg[i] = beta; dg[i] = ci[0].x; }
-          }
-          const int sJ = slot_of(J);
-          auto col = [&](int cc) {  // ring column J + cc
-            int sl = sJ + cc;
-            if (sl >= Wc) sl -= Wc;
-            return ring + (size_t)sl * LD;
-          };
-          if (tau.x != 0.0 || tau.y != 0.0) {
-            // two-sided update of the diagonal block D = A[J:J+L, J:J+L]:  D <- H^H D H  (zhetd2 form)
-            cplx p = cmake(0.0, 0.0);
-            for (int c = 0; c < L; ++c) {
-              const cplx vc = shfl_c(v, c);
-              if (lane < L) {
+        const int sJ = slot_of(J);
+        auto colp = [&](int cc) {  // ring column J + cc
+          int sl = sJ + cc;
+          if (sl >= Wc) sl -= Wc;
+          return ring + (size_t)sl * LD;
+        };
+        const bool t_on = (tau.x != 0.0 || tau.y != 0.0);
+        const int Jn = J + L, L2 = min(B, n - Jn);
+        // P1: partial p = D v over this thread's quarter of the columns; P4: partial u = C v
+        cplx acc = cmake(0.0, 0.0), uacc = cmake(0.0, 0.0);
+        if (t_on) {
+#pragma unroll
+          for (int jj = 0; jj < QN; ++jj) {
+            const int c = q * QN + jj;
+            if (c < L) {
+              const cplx vc = vs[c];
+              const cplx *pcol = colp(c);
+              if (l < L) {
                 cplx a;
-                if (lane >= c) { a = col(c)[lane - c]; if (lane == c) a.y = 0.0; }
-                else a = cconj(col(lane)[c - lane]);
-                cfma(p, a, vc);
+                if (l >= c) { a = pcol[l - c]; if (l == c) a.y = 0.0; }
+                else a = cconj(colp(l)[c - l]);
+                cfma(acc, a, vc);
               }
-            }
-            p = cmul(tau, p);
-            const double sr = warp_sum(lane < L ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
-            const double si = warp_sum(lane < L ? p.x * v.y - p.y * v.x : 0.0);
-            const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
-            cplx w = p;
-            cfma(w, alpha, v);
-            for (int c = 0; c < L; ++c) {
-              const cplx vc = shfl_c(v, c), wc = shfl_c(w, c);
-              if (lane >= c && lane < L) {
-                cplx *pa = col(c) + (lane - c);
-                cplx a = *pa;
-                cfms(a, v, cconj(wc));
-                cfms(a, w, cconj(vc));
-                if (lane == c) a.y = 0.0;
-                *pa = a;
-              }
+              if (l < L2) cfma(uacc, pcol[L + l - c], vc);
             }
           }
-          const int Jn = J + L, L2 = min(B, n - Jn);
-          if (L2 <= 0) {
-            finished = true;
+        }
+        red1[q * B + l] = acc;
+        red2[q * B + l] = uacc;
+        team_bar();  // BAR1
+        cplx p = cadd(cadd(red1[l], red1[B + l]), cadd(red1[2 * B + l], red1[3 * B + l]));
+        p = cmul(tau, p);
+        const double sr = group_sum<B>(l < L ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
+        const double si = group_sum<B>(l < L ? p.x * v.y - p.y * v.x : 0.0);
+        const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
+        cplx w = p;
+        cfma(w, alpha, v);
+        const cplx u = cadd(cadd(red2[l], red2[B + l]), cadd(red2[2 * B + l], red2[3 * B + l]));
+        const cplx tu = cmul(tau, u);
+        // P5: first column of C after the right-apply, and the reflector that annihilates it
+        cplx tau2 = cmake(0.0, 0.0), v2 = cmake(0.0, 0.0);
+        if (L2 > 0) {
+          cplx *c0p = colp(0) + L;
+          cplx x = cmake(0.0, 0.0);
+          if (l < L2) x = csub(c0p[l], tu);  // conj(v[0]) = 1
+          if (L2 > 1) {
+            double beta2;
+            group_larfg<B>(x, L2, l, tau2, beta2);
+            v2 = x;
+            if (q == 0 && l < L2) c0p[l] = (l == 0) ? cmake(beta2, 0.0) : cmake(0.0, 0.0);
           } else {
-            // C = A[Jn:Jn+L2, J:J+L]:  C <- C H, new reflector from C[:,0], C[:,1:] <- H'^H C[:,1:]
-            cplx u = cmake(0.0, 0.0);
-            const bool t_on = (tau.x != 0.0 || tau.y != 0.0);
-            if (t_on) {
-              for (int c = 0; c < L; ++c) {
-                const cplx vc = shfl_c(v, c);
-                if (lane < L2) cfma(u, col(c)[L + lane - c], vc);
-              }
-            }
-            const cplx tu = cmul(tau, u);  // row-wise tau (C v)
-            cplx x = cmake(0.0, 0.0);
-            if (lane < L2) { x = col(0)[L + lane]; x = csub(x, tu); }  // conj(v[0]) = 1
-            cplx tau2 = cmake(0.0, 0.0), v2;
-            if (L2 > 1) {
-              double beta2;
-              warp_larfg(x, L2, lane, tau2, beta2);
-              v2 = x;
-              if (lane < L2) col(0)[L + lane] = (lane == 0) ? cmake(beta2, 0.0) : cmake(0.0, 0.0);
-            } else {
-              if (lane == 0) col(0)[L] = x;
-              v2 = (lane == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
-            }
-            const bool t2_on = (tau2.x != 0.0 || tau2.y != 0.0);
-            if (t_on || t2_on) {
-              // lane = column c of C (1 <= c < L)
-              const bool mine = lane >= 1 && lane < L;
-              const cplx vcj = cconj(v);
-              cplx *pc = col(mine ? lane : 0) + (L - (mine ? lane : 0));  // &C(0, c)
-              cplx zacc = cmake(0.0, 0.0);
-              for (int r = 0; r < L2; ++r) {
-                const cplx tur = shfl_c(tu, r), v2r = shfl_c(v2, r);
-                if (mine) {
-                  cplx t = pc[r];
-                  cfms(t, tur, vcj);
-                  cfmac(zacc, v2r, t);
-                  pc[r] = t;
-                }
-              }
-              if (t2_on) {
-                const cplx f = cmul(cconj(tau2), zacc);
-                for (int r = 0; r < L2; ++r) {
-                  const cplx v2r = shfl_c(v2, r);
-                  if (mine) {
-                    cplx t = pc[r];
-                    cfms(t, v2r, f);
-                    pc[r] = t;
-                  }
-                }
-              }
-            }
-            v = v2; tau = tau2; J = Jn; L = L2; ++k;
+            if (tt == 0) c0p[0] = x;
+            v2 = (l == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
           }
+        }
+        if (q == 0) { ws[l] = w; tus[l] = tu; v2s[l] = v2; }
+        team_bar();  // BAR2
+        // P3: D <- D - v w^H - w v^H on the lower triangle
+        if (t_on && l < L) {
+#pragma unroll
+          for (int jj = 0; jj < QN; ++jj) {
+            const int c = q * QN + jj;
+            if (c <= l) {
+              cplx *pa = colp(c) + (l - c);
+              cplx a = *pa;
+              cfms(a, v, cconj(ws[c]));
+              cfms(a, w, cconj(vs[c]));
+              if (l == c) a.y = 0.0;
+              *pa = a;
+            }
+          }
+        }
+        if (L2 <= 0) {
+          finished = true;
+        } else {
+          const bool t2_on = (tau2.x != 0.0 || tau2.y != 0.0);
+          if (t_on || t2_on) {
+            // P6/P7: thread = column c = l of C (1 <= c < L), rows of its quarter:
+            //   t = C - (tau C v) v^H ; z = v2^H t ; C = t - v2 conj(tau2) z
+            const bool mine = l >= 1 && l < L;
+            const cplx vcj = cconj(v);
+            cplx *pc = colp(mine ? l : 0) + (L - (mine ? l : 0));
+            cplx tv[QN];
+            cplx zacc = cmake(0.0, 0.0);
+#pragma unroll
+            for (int jj = 0; jj < QN; ++jj) {
+              const int r = q * QN + jj;
+              tv[jj] = cmake(0.0, 0.0);
+              if (mine && r < L2) {
+                cplx t = pc[r];
+                cfms(t, tus[r], vcj);
+                cfmac(zacc, v2s[r], t);
+                tv[jj] = t;
+              }
+            }
+            red3[q * B + l] = zacc;
+            team_bar();  // BAR3
+            const cplx zc = cadd(cadd(red3[l], red3[B + l]), cadd(red3[2 * B + l], red3[3 * B + l]));
+            const cplx f = cmul(cconj(tau2), zc);
+#pragma unroll
+            for (int jj = 0; jj < QN; ++jj) {
+              const int r = q * QN + jj;
+              if (mine && r < L2) {
+                cplx t = tv[jj];
+                cfms(t, v2s[r], f);
+                pc[r] = t;
+              }
+            }
+          }
+          if (q == 0) vs[l] = v2;  // after BAR3 (or with P3 skipped): nobody still reads the old v
+          v = v2; tau = tau2; J = Jn; L = L2; ++k;
         }
       }
       __syncthreads();
@@ -258,26 +296,28 @@ __global__ void __launch_bounds__(512) bulge_kernel(int n, BatchRef AB, double *
 
 template <int B>
 void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inner, cudaStream_t s) {
-  constexpr int LD = 2 * B;
+  constexpr int LD = 2 * B, TT = 4 * B;
   const size_t colbytes = (size_t)LD * sizeof(cplx);
-  const size_t max_smem = 220 * 1024;
+  const int gmax = B == 32 ? 3 : 12;                       // teams per CTA (threads: gmax * 4B + 128 I/O)
+  const size_t team_bytes = (size_t)16 * B * sizeof(cplx);
+  const size_t max_smem = 226 * 1024;
   int G, Wc;
-  if ((size_t)n * colbytes <= max_smem) {  // whole band resident
+  if ((size_t)n * colbytes + gmax * team_bytes <= max_smem) {  // whole band resident
     Wc = n;
-    G = max(1, min(12, (n + 2 * B - 1) / (2 * B)));
+    G = max(1, min(gmax, (n + 2 * B - 1) / (2 * B)));
   } else {
-    G = (int)((max_smem / colbytes - 8) / (2 * B));
-    G = max(1, min(G, 12));
+    G = (int)(((max_smem - gmax * team_bytes) / colbytes - 8) / (2 * B));
+    G = max(1, min(G, gmax));
     Wc = 2 * G * B + 8;
   }
-  const size_t smem = (size_t)Wc * colbytes;
+  const size_t smem = (size_t)Wc * colbytes + G * team_bytes;
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(bulge_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_done = true;
   }
   KScope ks(KC_BULGE, 0.0, s);
-  bulge_kernel<B><<<nmat, (G + NIO) * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
+  bulge_kernel<B><<<nmat, G * TT + NIO * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
 }
 }  // namespace
 

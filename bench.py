@@ -149,7 +149,7 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
 HBM_CLASSES = {"hemv", "expand", "pencil", "combine"}
-TENSOR_CLASSES = {"gemm_factor", "gemm_reduce", "gemm_tridiag"}
+TENSOR_CLASSES = {"gemm_factor", "gemm_reduce", "gemm_tridiag", "gemm_hemm", "gemm_wy"}
 
 
 def run_ours(args):

@@ -141,7 +141,7 @@ enum {
   BS_KC_EXPAND = 1,       /* S2 expansion                                       work: bytes written                  */
   BS_KC_GEMM_FACTOR = 2,  /* DMMA zgemm launches of S3                          work: real flops                     */
   BS_KC_GEMM_REDUCE = 3,  /* DMMA zgemm launches of S5 (and of the POLY coefficient reduction)                       */
-  BS_KC_GEMM_TRIDIAG = 4, /* DMMA zgemm launches of S6                          work: real flops                     */
+  BS_KC_GEMM_TRIDIAG = 4, /* DMMA zgemm launches of S6: Hermitian rank-2b updates  work: real flops                  */
   BS_KC_HEMV = 5,         /* S6 Hermitian matrix-vector kernel                  work: bytes of the lower triangle    */
   BS_KC_PANEL = 6,        /* S6 panel / reflector kernels                                                            */
   BS_KC_STURM = 7,        /* S7                                                                                      */
@@ -150,7 +150,9 @@ enum {
   BS_KC_POTRF_DIAG = 10,  /* S3 diagonal-block factor kernel                                                         */
   BS_KC_OTHER = 11,
   BS_KC_BULGE = 12,       /* S6 stage 2: band -> tridiagonal bulge chasing                                           */
-  BS_KC_COUNT = 13
+  BS_KC_GEMM_HEMM = 13,   /* S6 stage 1: Z = A22 V (Hermitian A22, lower triangle read), DMMA             work: real flops */
+  BS_KC_GEMM_WY = 14,     /* S6 stage 1: the two small compact-WY GEMMs per panel, DMMA                    work: real flops */
+  BS_KC_COUNT = 15
 };
 /* Per-class totals of the last bs_assemble / bs_bands led by this handle under BS_OPT_TIMING = 2: device milliseconds
  * (CUDA events on the call's stream around every launch), ALGORITHMIC work credited at launch time (flops or bytes, see

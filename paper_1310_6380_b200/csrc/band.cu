@@ -202,6 +202,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     GemmDesc g{};
     g.ncells = ncells; g.inner = inner; g.kclass = KC_GEMM_TRIDIAG;
     // Z = A22 V
+    g.kclass = KC_GEMM_HEMM;
     g.M = m; g.N = b; g.K = m; g.opA = 0; g.opB = 0; g.flags = BS_GEMM_A_HERM_LOWER;
     g.A = A; g.A.off += (long long)r0 * (lda + 1); g.lda = lda;
     g.B = VW; g.B.off += r0; g.ldb = n;
@@ -209,6 +210,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
     launch_zgemm(g, s); ++launches;
     // [G | S] = V^H [V | Z]
+    g.kclass = KC_GEMM_WY;
     g.M = b; g.N = 2 * b; g.K = m; g.opA = 1; g.opB = 0; g.flags = 0;
     g.A = VW; g.A.off += r0; g.lda = n;
     g.B = VW; g.B.off += (long long)2 * b * n + r0; g.ldb = n;
@@ -226,6 +228,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     g.C = VW; g.C.off += (long long)b * n + r0; g.ldc = n;
     launch_zgemm(g, s); ++launches;
     // A22 -= [V | X] [X | V]^H  (lower tiles)
+    g.kclass = KC_GEMM_TRIDIAG;
     g.M = m; g.N = m; g.K = 2 * b; g.opA = 0; g.opB = 1; g.flags = BS_GEMM_LOWER_ONLY;
     g.A = VW; g.A.off += r0; g.lda = n;
     g.B = VW; g.B.off += (long long)b * n + r0; g.ldb = n;

@@ -66,7 +66,7 @@ namespace bsk {
 // DMMA classes, bytes for the HBM classes), accumulated on the host at launch time.
 enum KClass {
   KC_TABLE = 0, KC_EXPAND, KC_GEMM_FACTOR, KC_GEMM_REDUCE, KC_GEMM_TRIDIAG, KC_HEMV, KC_PANEL, KC_STURM, KC_PENCIL,
-  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_BULGE, KC_COUNT
+  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_BULGE, KC_GEMM_HEMM, KC_GEMM_WY, KC_COUNT
 };
 struct KTimer {
   std::vector<cudaEvent_t> ev;   // pool; pairs (2i, 2i+1)

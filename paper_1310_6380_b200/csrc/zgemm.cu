@@ -6,9 +6,12 @@
 namespace bsk {
 
 namespace {
-constexpr int BM = 64, BN = 64, BK = 8, STAGES = 4, LDS = 66;  // LDS: padded row stride (conflict-free fragment loads)
+constexpr int BK = 8, STAGES = 4;
 constexpr int NT = 256;
-constexpr size_t kSmem = (size_t)STAGES * BK * LDS * sizeof(cplx) * 2;
+// CTA tile BM x BN, 8 warps of 16 x 32 each: (BM, BN) = (64, 64) [4 x 2 warps] or (128, 32) [8 x 1 warps, for N <= 32:
+// the HEMM and the compact-WY products of the band reduction].  Row strides are padded by 2 (conflict-free fragments).
+template <int BM, int BN>
+constexpr size_t smem_bytes() { return (size_t)STAGES * BK * ((BM + 2) + (BN + 2)) * sizeof(cplx); }
 
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid) {
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
@@ -28,11 +31,13 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 
 // HERM = 1: A is an M x M Hermitian matrix of which only the LOWER triangle is valid (K == M, OPA == 0):
 //   op(A)[m][k] = A[m][k] for m > k, Re A[m][m] for m == k, conj(A[k][m]) for m < k  (the HEMM of the band reduction).
-template <int OPA, int OPB, int HERM>
+template <int OPA, int OPB, int HERM, int BM, int BN>
 __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
+  constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / 16;  // WMN warps along m, 8 / WMN along n
+  static_assert((BM / 16) * (BN / 32) == 8, "8 warps of 16 x 32");
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cplx(*As)[BK][LDS] = reinterpret_cast<cplx(*)[BK][LDS]>(smem_raw);
-  cplx(*Bs)[BK][LDS] = reinterpret_cast<cplx(*)[BK][LDS]>(smem_raw + (size_t)STAGES * BK * LDS * sizeof(cplx));
+  cplx(*As)[BK][LDA_S] = reinterpret_cast<cplx(*)[BK][LDA_S]>(smem_raw);
+  cplx(*Bs)[BK][LDB_S] = reinterpret_cast<cplx(*)[BK][LDB_S]>(smem_raw + (size_t)STAGES * BK * LDA_S * sizeof(cplx));
 
   const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
   if ((g.flags & BS_GEMM_LOWER_ONLY) && n0 >= m0 + BM) return;
@@ -50,16 +55,16 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
   const int nkt = khi > klo ? (khi - klo + BK - 1) / BK : 0;
 
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-  const int wm = warp & 3, wn = warp >> 2;  // 4 x 2 warps; warp tile 16 x 32
+  const int wm = warp % WMN, wn = warp / WMN;  // warp tile 16 x 32
 
   auto load_tile = [&](int kt, int stage) {
     const int k0 = klo + kt * BK;
 #pragma unroll
-    for (int r = 0; r < 2; ++r) {
+    for (int r = 0; r < BM * BK / NT; ++r) {
       int m, k;
       bool tr = OPA != 0;                                  // read the element from its transposed position
       if (HERM && k0 >= m0 + BM - 1) tr = true;            // the whole k-tile lies above the diagonal
-      if (!tr) { m = t & 63; k = (t >> 6) + 4 * r; } else { k = t & 7; m = (t >> 3) + 32 * r; }
+      if (!tr) { m = t % BM; k = t / BM + (NT / BM) * r; } else { k = t & 7; m = (t >> 3) + 32 * r; }
       if (HERM && !tr && k0 + BK - 1 > m0) tr = (k0 + k > m0 + m);   // tile crossing the diagonal: per element
       const bool ok = (m0 + m < g.M) && (k0 + k < khi);
       const cplx *src = !tr ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
@@ -67,9 +72,9 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
       cp_async16(&As[stage][k][m], ok ? src : A, ok);
     }
 #pragma unroll
-    for (int r = 0; r < 2; ++r) {
+    for (int r = 0; r < BN * BK / NT; ++r) {
       int n, k;
-      if (OPB == 0) { k = t & 7; n = (t >> 3) + 32 * r; } else { n = t & 63; k = (t >> 6) + 4 * r; }
+      if (OPB == 0) { k = t & 7; n = (t >> 3) + 32 * r; } else { n = t % BN; k = t / BN + (NT / BN) * r; }
       const bool ok = (n0 + n < g.N) && (k0 + k < khi);
       const cplx *src = OPB == 0 ? B + (size_t)(k0 + k) + (size_t)(n0 + n) * g.ldb
                                  : B + (size_t)(n0 + n) + (size_t)(k0 + k) * g.ldb;
@@ -147,32 +152,37 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
     }
   }
 }
+template <int OPA, int OPB, int HERM, int BM, int BN>
+void launch_one(const GemmDesc &g, cudaStream_t s) {
+  constexpr size_t smem = smem_bytes<BM, BN>();
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_done = true;
+  }
+  dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner);
+  zgemm_kernel<OPA, OPB, HERM, BM, BN><<<grid, NT, smem, s>>>(g);
+}
 }  // namespace
 
 void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   if (g.M <= 0 || g.N <= 0 || g.ncells * g.inner <= 0) return;
-  dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner);
   double work = 8.0 * g.K * (double)g.ncells * g.inner;
   work *= (g.flags & BS_GEMM_LOWER_ONLY) ? 0.5 * g.M * (g.M + 1.0) : (double)g.M * g.N;
   if (g.flags & (BS_GEMM_KLO_ROW | BS_GEMM_KHI_ROW | BS_GEMM_KLO_COL | BS_GEMM_KHI_COL)) work *= 0.5;
   KScope ks(g.kclass ? g.kclass : KC_OTHER, work, s);
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(zgemm_kernel<0, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<0, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<1, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<1, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    cudaFuncSetAttribute(zgemm_kernel<0, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    attr_done = true;
-  }
+  const bool narrow = g.N <= 32 && g.M > 64 && g.opB == 0 && g.opA == 0 &&
+                      !(g.flags & (BS_GEMM_KLO_COL | BS_GEMM_KHI_COL | BS_GEMM_KLO_ROW | BS_GEMM_KHI_ROW));
   if (g.flags & BS_GEMM_A_HERM_LOWER) {  // requires opA == 0, opB == 0, K == M
-    zgemm_kernel<0, 0, 1><<<grid, NT, kSmem, s>>>(g);
+    if (narrow) launch_one<0, 0, 1, 128, 32>(g, s);
+    else launch_one<0, 0, 1, 64, 64>(g, s);
     return;
   }
-  if (g.opA == 0 && g.opB == 0) zgemm_kernel<0, 0, 0><<<grid, NT, kSmem, s>>>(g);
-  else if (g.opA == 0 && g.opB == 1) zgemm_kernel<0, 1, 0><<<grid, NT, kSmem, s>>>(g);
-  else if (g.opA == 1 && g.opB == 0) zgemm_kernel<1, 0, 0><<<grid, NT, kSmem, s>>>(g);
-  else zgemm_kernel<1, 1, 0><<<grid, NT, kSmem, s>>>(g);
+  if (narrow) { launch_one<0, 0, 0, 128, 32>(g, s); return; }
+  if (g.opA == 0 && g.opB == 0) launch_one<0, 0, 0, 64, 64>(g, s);
+  else if (g.opA == 0 && g.opB == 1) launch_one<0, 1, 0, 64, 64>(g, s);
+  else if (g.opA == 1 && g.opB == 0) launch_one<1, 0, 0, 64, 64>(g, s);
+  else launch_one<1, 1, 0, 64, 64>(g, s);
 }
 
 }  // namespace bsk

@@ -277,7 +277,7 @@ def run_ours(args):
     elif dom in HBM_CLASSES:
         roof = {"bound": "hbm", "achieved": work_d / (ms_d * 1e6), "peak": hbm_peak, "unit": "GB/s", "peak_source": hbm_src}
     else:
-        roof = {"bound": "alu", "achieved": None, "peak": dfma_peak, "unit": "TFLOP/s",
+        roof = {"bound": "alu", "achieved": work_d / (ms_d * 1e9) if work_d else None, "peak": dfma_peak, "unit": "TFLOP/s",
                 "peak_source": "FP64 DFMA register-only loop measured in this run by bs_fp64_peak"}
     roof["frac"] = (roof["achieved"] / roof["peak"]) if roof["achieved"] else None
     roof.update({"kernel": dom, "launches_per_step": cnt_d / args.steps, "avg_launch_ms": ms_d / max(cnt_d, 1),

@@ -316,7 +316,8 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
     cudaFuncSetAttribute(bulge_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_done = true;
   }
-  KScope ks(KC_BULGE, 0.0, s);
+  // algorithmic work: ~n^2/(2B) steps of 48 B^2 real flops (hemv, rank-2, C v, right- and left-apply)
+  KScope ks(KC_BULGE, 24.0 * n * (double)n * B * nmat, s);
   bulge_kernel<B><<<nmat, G * TT + NIO * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
 }
 }  // namespace

@@ -95,15 +95,38 @@ __global__ void __launch_bounds__(QT) panel_qr_kernel(int n, int lda, int b, int
     if (tau.x != 0.0 || tau.y != 0.0) {
       for (int c = j + 1 + warp; c < b; c += QT / 32) {
         cplx *col = Ag + (size_t)(c0 + c) * lda;
-        cplx dot = cmake(0.0, 0.0);
-        for (int r = pr + lane; r < n; r += 32) cfmac(dot, vs[r - r0], col[r]);
+        cplx dot = cmake(0.0, 0.0), dot2 = cmake(0.0, 0.0);
+        int r = pr + lane;
+        for (; r + 224 < n; r += 256) {  // 8 independent 16-byte loads in flight per lane
+          cplx x[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) x[u] = col[r + 32 * u];
+#pragma unroll
+          for (int u = 0; u < 8; u += 2) {
+            cfmac(dot, vs[r + 32 * u - r0], x[u]);
+            cfmac(dot2, vs[r + 32 * (u + 1) - r0], x[u + 1]);
+          }
+        }
+        for (; r < n; r += 32) cfmac(dot, vs[r - r0], col[r]);
+        dot = cadd(dot, dot2);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
           dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
           dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
         }
         const cplx f = cmul(cconj(tau), dot);
-        for (int r = pr + lane; r < n; r += 32) {
+        r = pr + lane;
+        for (; r + 224 < n; r += 256) {
+          cplx x[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) x[u] = col[r + 32 * u];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            cfms(x[u], vs[r + 32 * u - r0], f);
+            col[r + 32 * u] = x[u];
+          }
+        }
+        for (; r < n; r += 32) {
           cplx x = col[r];
           cfms(x, vs[r - r0], f);
           col[r] = x;

@@ -11,6 +11,8 @@
 // Element (r, c), c <= r <= c + 2B - 1, lives at ring[(c mod Wc) * LD + (r - c)].  With LD = 2B the two access patterns
 // used (fixed column, lanes over rows: stride 1; fixed row, lanes over columns: stride LD - 1, odd) are both free of
 // shared-memory bank conflicts for 16-byte elements.
+#include <cstdlib>
+
 #include "bs_internal.cuh"
 
 namespace bsk {
@@ -60,10 +62,10 @@ __device__ __forceinline__ void group_larfg(cplx &x, int len, int l, cplx &tau, 
 
 // Team of 4B threads per sweep: thread (l, q), l = index inside the B x B block (row or column), q = quarter of the
 // other dimension (QN = B/4 indices each).  Vectors (v, w, u, v2) are computed redundantly by the four q-replicas.
-template <int B>
-__global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc,
-                                                                     int inner) {
-  constexpr int LD = 2 * B, TT = 4 * B, QN = B / 4;
+template <int B, int NQ>
+__global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n, BatchRef AB, double *d, double *e, int G,
+                                                                             int Wc, int inner) {
+  constexpr int LD = 2 * B, TT = NQ * B, QN = B / NQ;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *ring = reinterpret_cast<cplx *>(smem_raw);
   const int z = blockIdx.x, cell = z / inner, mi = z % inner;
@@ -74,10 +76,16 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
   const bool is_io = tid >= ncomp;
   const int io_tid = tid - ncomp, io_nt = blockDim.x - ncomp;
   const int team = tid / TT, tt = tid % TT, l = tt % B, q = tt / B;
-  // team scratch behind the ring: vs, ws, tus, v2s (B each), red1, red2, red3 (4B each) = 16 B complex per team
-  cplx *ts = ring + (size_t)Wc * LD + (size_t)(is_io ? 0 : team) * 16 * B;
+  // team scratch behind the ring: vs, ws, tus, v2s (B each), red1, red2, red3 (NQ B each) complex per team
+  cplx *ts = ring + (size_t)Wc * LD + (size_t)(is_io ? 0 : team) * (4 + 3 * NQ) * B;
   cplx *vs = ts, *ws = ts + B, *tus = ts + 2 * B, *v2s = ts + 3 * B;
-  cplx *red1 = ts + 4 * B, *red2 = ts + 8 * B, *red3 = ts + 12 * B;
+  cplx *red1 = ts + 4 * B, *red2 = red1 + NQ * B, *red3 = red2 + NQ * B;
+  auto qsum = [&](const cplx *red) {  // fixed order: identical bits in every replica
+    cplx a = red[l];
+#pragma unroll
+    for (int qq = 1; qq < NQ; ++qq) a = cadd(a, red[qq * B + l]);
+    return a;
+  };
   auto team_bar = [&]() {
     if (TT == 32) __syncwarp();
     else asm volatile("bar.sync %0, %1;\n" ::"r"(team + 1), "r"(TT) : "memory");
@@ -88,22 +96,36 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
   auto slot_of = [&](int c) { return c % Wc; };
   // column ranges are copied as one flat index space so that every thread has several independent 16-byte
   // transfers in flight (cp.async: global -> shared without register staging)
+  // Thread t of nt (nt a multiple of LD) moves element off = t % LD of the columns c0 + t / LD + j (nt / LD): the ring
+  // slot is advanced incrementally and every thread keeps several independent 16-byte transfers in flight.
   auto io_load = [&](int c0, int c1, int t, int nt) {
-    const int total = (c1 - c0) * LD;
-    for (int qq = t; qq < total; qq += nt) {
-      const int c = c0 + qq / LD, off = qq % LD;
-      const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + (size_t)slot_of(c) * LD + off);
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(ab + (size_t)c * LD + off));
+    const int off = t % LD, cstep = nt / LD;
+    int c = c0 + t / LD;
+    if (c < c1) {
+      int sl = slot_of(c);
+      const int sstep = cstep % Wc;
+      for (; c < c1; c += cstep) {
+        const unsigned dst = (unsigned)__cvta_generic_to_shared(ring + (size_t)sl * LD + off);
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(ab + (size_t)c * LD + off));
+        sl += sstep;
+        if (sl >= Wc) sl -= Wc;
+      }
     }
     asm volatile("cp.async.commit_group;\n" ::);
     asm volatile("cp.async.wait_group 0;\n" ::: "memory");
   };
   auto io_evict = [&](int c0, int c1, int t, int nt) {
-    const int total = (c1 - c0) * LD;
+    const int off = t % LD, cstep = nt / LD;
+    int c = c0 + t / LD;
+    if (c < c1) {
+      int sl = slot_of(c);
+      const int sstep = cstep % Wc;
 #pragma unroll 4
-    for (int qq = t; qq < total; qq += nt) {
-      const int c = c0 + qq / LD, off = qq % LD;
-      ab[(size_t)c * LD + off] = ring[(size_t)slot_of(c) * LD + off];
+      for (; c < c1; c += cstep) {
+        ab[(size_t)c * LD + off] = ring[(size_t)sl * LD + off];
+        sl += sstep;
+        if (sl >= Wc) sl -= Wc;
+      }
     }
   };
 
@@ -169,11 +191,18 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
           team_bar();
         }
         const int sJ = slot_of(J);
-        auto colp = [&](int cc) {  // ring column J + cc
-          int sl = sJ + cc;
+        // element offsets of the ring columns this thread touches: its quarter (J + q QN + jj) and column J + l
+        int cb[QN];
+#pragma unroll
+        for (int jj = 0; jj < QN; ++jj) {
+          int sl = sJ + q * QN + jj;
           if (sl >= Wc) sl -= Wc;
-          return ring + (size_t)sl * LD;
-        };
+          cb[jj] = sl * LD;
+        }
+        int mycb = sJ + l;
+        if (mycb >= Wc) mycb -= Wc;
+        mycb *= LD;
+        const int cb0 = sJ * LD;
         const bool t_on = (tau.x != 0.0 || tau.y != 0.0);
         const int Jn = J + L, L2 = min(B, n - Jn);
         // P1: partial p = D v over this thread's quarter of the columns; P4: partial u = C v
@@ -184,11 +213,10 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
             const int c = q * QN + jj;
             if (c < L) {
               const cplx vc = vs[c];
-              const cplx *pcol = colp(c);
+              const cplx *pcol = ring + cb[jj];
               if (l < L) {
-                cplx a;
-                if (l >= c) { a = pcol[l - c]; if (l == c) a.y = 0.0; }
-                else a = cconj(colp(l)[c - l]);
+                cplx a = ring[l >= c ? cb[jj] + l - c : mycb + c - l];  // lower part as stored, upper part mirrored
+                a.y = l > c ? a.y : (l == c ? 0.0 : -a.y);
                 cfma(acc, a, vc);
               }
               if (l < L2) cfma(uacc, pcol[L + l - c], vc);
@@ -198,19 +226,19 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
         red1[q * B + l] = acc;
         red2[q * B + l] = uacc;
         team_bar();  // BAR1
-        cplx p = cadd(cadd(red1[l], red1[B + l]), cadd(red1[2 * B + l], red1[3 * B + l]));
+        cplx p = qsum(red1);
         p = cmul(tau, p);
         const double sr = group_sum<B>(l < L ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
         const double si = group_sum<B>(l < L ? p.x * v.y - p.y * v.x : 0.0);
         const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
         cplx w = p;
         cfma(w, alpha, v);
-        const cplx u = cadd(cadd(red2[l], red2[B + l]), cadd(red2[2 * B + l], red2[3 * B + l]));
+        const cplx u = qsum(red2);
         const cplx tu = cmul(tau, u);
         // P5: first column of C after the right-apply, and the reflector that annihilates it
         cplx tau2 = cmake(0.0, 0.0), v2 = cmake(0.0, 0.0);
         if (L2 > 0) {
-          cplx *c0p = colp(0) + L;
+          cplx *c0p = ring + cb0 + L;
           cplx x = cmake(0.0, 0.0);
           if (l < L2) x = csub(c0p[l], tu);  // conj(v[0]) = 1
           if (L2 > 1) {
@@ -231,7 +259,7 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
           for (int jj = 0; jj < QN; ++jj) {
             const int c = q * QN + jj;
             if (c <= l) {
-              cplx *pa = colp(c) + (l - c);
+              cplx *pa = ring + cb[jj] + (l - c);
               cplx a = *pa;
               cfms(a, v, cconj(ws[c]));
               cfms(a, w, cconj(vs[c]));
@@ -249,7 +277,7 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
             //   t = C - (tau C v) v^H ; z = v2^H t ; C = t - v2 conj(tau2) z
             const bool mine = l >= 1 && l < L;
             const cplx vcj = cconj(v);
-            cplx *pc = colp(mine ? l : 0) + (L - (mine ? l : 0));
+            cplx *pc = ring + (mine ? mycb + L - l : cb0 + L);
             cplx tv[QN];
             cplx zacc = cmake(0.0, 0.0);
 #pragma unroll
@@ -265,7 +293,7 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
             }
             red3[q * B + l] = zacc;
             team_bar();  // BAR3
-            const cplx zc = cadd(cadd(red3[l], red3[B + l]), cadd(red3[2 * B + l], red3[3 * B + l]));
+            const cplx zc = qsum(red3);
             const cplx f = cmul(cconj(tau2), zc);
 #pragma unroll
             for (int jj = 0; jj < QN; ++jj) {
@@ -294,12 +322,12 @@ __global__ void __launch_bounds__(B == 32 ? 512 : 1024) bulge_kernel(int n, Batc
   }
 }
 
-template <int B>
+template <int B, int NQ>
 void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inner, cudaStream_t s) {
-  constexpr int LD = 2 * B, TT = 4 * B;
+  constexpr int LD = 2 * B, TT = NQ * B;
   const size_t colbytes = (size_t)LD * sizeof(cplx);
-  const int gmax = B == 32 ? 3 : 12;                       // teams per CTA (threads: gmax * 4B + 128 I/O)
-  const size_t team_bytes = (size_t)16 * B * sizeof(cplx);
+  const int gmax = min(12, ((TT >= 128 ? 512 : 1024) - NIO * 32) / TT);  // teams per CTA (G * TT + 128 I/O threads)
+  const size_t team_bytes = (size_t)(4 + 3 * NQ) * B * sizeof(cplx);
   const size_t max_smem = 226 * 1024;
   int G, Wc;
   if ((size_t)n * colbytes + gmax * team_bytes <= max_smem) {  // whole band resident
@@ -313,21 +341,22 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
   const size_t smem = (size_t)Wc * colbytes + G * team_bytes;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(bulge_kernel<B>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaFuncSetAttribute(bulge_kernel<B, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     attr_done = true;
   }
   // algorithmic work: ~n^2/(2B) steps of 48 B^2 real flops (hemv, rank-2, C v, right- and left-apply)
   KScope ks(KC_BULGE, 24.0 * n * (double)n * B * nmat, s);
-  bulge_kernel<B><<<nmat, G * TT + NIO * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
+  bulge_kernel<B, NQ><<<nmat, G * TT + NIO * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
 }
 }  // namespace
 
 // Band -> tridiagonal for every matrix of the batch.  b must be 8, 16 or 32.
 void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s) {
   const int nmat = ncells * inner;
-  if (b == 8) launch_bulge_t<8>(n, AB, d, e, nmat, inner, s);
-  else if (b == 16) launch_bulge_t<16>(n, AB, d, e, nmat, inner, s);
-  else launch_bulge_t<32>(n, AB, d, e, nmat, inner, s);
+  static const int nq_env = getenv("BS_BULGE_NQ") ? atoi(getenv("BS_BULGE_NQ")) : 0;
+  if (b == 8) launch_bulge_t<8, 4>(n, AB, d, e, nmat, inner, s);
+  else if (b == 16) { if (nq_env == 8) launch_bulge_t<16, 8>(n, AB, d, e, nmat, inner, s); else launch_bulge_t<16, 4>(n, AB, d, e, nmat, inner, s); }
+  else launch_bulge_t<32, 4>(n, AB, d, e, nmat, inner, s);
 }
 
 }  // namespace bsk

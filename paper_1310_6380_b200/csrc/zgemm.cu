@@ -82,6 +82,18 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
     }
   };
 
+  // beta != 0: the C tile is read only in the epilogue; warm it into L2 now so that the read-modify-write does not
+  // pay DRAM latency after the (short, K = 2b) main loop of the rank-2b updates
+  if (g.beta.x != 0.0 || g.beta.y != 0.0) {
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int row = m0 + wm * 16 + (lane >> 2), col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
+        if (row < g.M && col < g.N) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(C + (size_t)row + (size_t)col * g.ldc));
+      }
+    }
+  }
   double cr[2][4][2], ci[2][4][2];
 #pragma unroll
   for (int i = 0; i < 2; ++i)
@@ -138,6 +150,18 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
   for (int mi = 0; mi < 2; ++mi) {
     const int row = m0 + wm * 16 + mi * 8 + (lane >> 2);
     if (row >= g.M) continue;
+    // all eight C loads of this row first (independent, in flight together), then the eight stores: a load placed
+    // after a store to C could not be hoisted above it
+    cplx old[4][2];
+#pragma unroll
+    for (int ni = 0; ni < 4; ++ni) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
+        old[ni][j] = cmake(0.0, 0.0);
+        if (has_beta && col < g.N && !(lower && col > row)) old[ni][j] = C[(size_t)row + (size_t)col * g.ldc];
+      }
+    }
 #pragma unroll
     for (int ni = 0; ni < 4; ++ni) {
 #pragma unroll
@@ -145,9 +169,8 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
         const int col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
         if (col >= g.N || (lower && col > row)) continue;
         cplx v = cmul(g.alpha, cmake(cr[mi][ni][j], ci[mi][ni][j]));
-        cplx *dst = C + (size_t)row + (size_t)col * g.ldc;
-        if (has_beta) v = cadd(v, cmul(g.beta, *dst));
-        *dst = v;
+        if (has_beta) v = cadd(v, cmul(g.beta, old[ni][j]));
+        C[(size_t)row + (size_t)col * g.ldc] = v;
       }
     }
   }

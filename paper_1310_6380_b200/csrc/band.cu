@@ -18,6 +18,7 @@ namespace bsk {
 namespace {
 constexpr int QT = 1024;     // threads of the panel QR kernel (32 warps: one warp per trailing column of the panel)
 constexpr int NMAXQ = 2048;  // max rows of a panel (n <= 2048)
+constexpr int KS = 8;         // split-K factor of the Gram product [G | S] = V^H [V | Z] (one output tile per matrix)
 
 __device__ __forceinline__ double block_sum_q(double x, double *scratch) {
 #pragma unroll
@@ -144,22 +145,29 @@ __global__ void __launch_bounds__(256) wy_small_kernel(int b, BatchRef SM, int i
   cplx *T = reinterpret_cast<cplx *>(smem_raw);  // b x b, T[i + j*b]
   cplx *S = T + b * b;                           // b x b
   cplx *U = S + b * b;                           // b x b scratch
+  cplx *G = U + b * b;                           // b x b
   const int z = blockIdx.x, cell = z / inner, mi = z % inner;
   cplx *sm = batch_ptr(SM, cell, mi);
-  const cplx *G = sm;
+  const cplx *part = sm + (size_t)4 * b * b + 64;  // KS partial products [G | S], each b x 2b
   const double *tau = reinterpret_cast<const double *>(sm + (size_t)4 * b * b);
   cplx *out = sm + (size_t)2 * b * b;
   const int t = threadIdx.x;
   for (int i = t; i < b * b; i += blockDim.x) {
     T[i] = cmake(0.0, 0.0);
-    S[i] = sm[(size_t)b * b + i];
+    cplx gs = cmake(0.0, 0.0), ss = cmake(0.0, 0.0);
+    for (int k = 0; k < KS; ++k) {  // fixed order: deterministic
+      gs = cadd(gs, part[(size_t)k * 2 * b * b + i]);
+      ss = cadd(ss, part[(size_t)k * 2 * b * b + b * b + i]);
+    }
+    G[i] = gs;
+    S[i] = ss;
   }
   __syncthreads();
   for (int j = 0; j < b; ++j) {
     const cplx tj = cmake(tau[2 * j], tau[2 * j + 1]);
     if (t < j) {
       cplx acc = cmake(0.0, 0.0);
-      for (int l = t; l < j; ++l) cfma(acc, T[t + l * b], G[l + (size_t)j * b]);
+      for (int l = t; l < j; ++l) cfma(acc, T[t + l * b], G[l + j * b]);
       T[t + j * b] = cmul(cmake(-tj.x, -tj.y), acc);
     } else if (t == j) {
       T[j + j * b] = tj;
@@ -202,7 +210,7 @@ __global__ void __launch_bounds__(256) band_extract_kernel(int n, int lda, int b
 }  // namespace
 
 size_t band_vw_elems(int n, int b) { return (size_t)4 * b * n; }
-size_t band_sm_elems(int b) { return (size_t)4 * b * b + b + 16; }
+size_t band_sm_elems(int b) { return (size_t)4 * b * b + 64 + (size_t)KS * 2 * b * b; }
 size_t band_ab_elems(int n, int b) { return (size_t)n * 2 * b; }
 
 // Stage 1 for every matrix of the batch in lock step; on exit AB holds the band (ldab = 2b, bulge space zeroed).
@@ -212,7 +220,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
   const int nmat = ncells * inner;
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 3 * 64 * 64 * (int)sizeof(cplx));
+    cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 32 * 32 * (int)sizeof(cplx));
     attr_done = true;
   }
   for (int c0 = 0; c0 + b < n - 1; c0 += b) {
@@ -237,11 +245,13 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     g.M = b; g.N = 2 * b; g.K = m; g.opA = 1; g.opB = 0; g.flags = 0;
     g.A = VW; g.A.off += r0; g.lda = n;
     g.B = VW; g.B.off += (long long)2 * b * n + r0; g.ldb = n;
-    g.C = SM; g.ldc = b;
+    g.C = SM; g.C.off += (long long)4 * b * b + 64; g.ldc = b;
+    g.ksplit = KS; g.split_stride = (long long)2 * b * b;
     launch_zgemm(g, s); ++launches;
+    g.ksplit = 0; g.split_stride = 0;
     {
       KScope ks(KC_PANEL, 0.0, s);
-      wy_small_kernel<<<nmat, 256, 3 * b * b * sizeof(cplx), s>>>(b, SM, inner);
+      wy_small_kernel<<<nmat, 256, 4 * b * b * sizeof(cplx), s>>>(b, SM, inner);
       ++launches;
     }
     // X = [V | Z] [M2; T]

@@ -127,6 +127,8 @@ void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R,
 struct GemmDesc {
   int M, N, K, opA, opB, lda, ldb, ldc, flags, inner, ncells;
   int kclass;  // KClass the launch is timed under (0 -> KC_OTHER)
+  int ksplit;  // > 1: split K into ksplit chunks, chunk s writes its partial product to C + s * split_stride (beta ignored)
+  long long split_stride;
   cplx alpha, beta;
   BatchRef A, B, C;
 };

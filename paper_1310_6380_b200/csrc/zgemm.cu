@@ -41,12 +41,19 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
 
   const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
   if ((g.flags & BS_GEMM_LOWER_ONLY) && n0 >= m0 + BM) return;
-  const int cell = blockIdx.z / g.inner, bi = blockIdx.z % g.inner;
+  const int nsplit = g.ksplit > 1 ? g.ksplit : 1;
+  const int ks = blockIdx.z % nsplit, zz = blockIdx.z / nsplit;
+  const int cell = zz / g.inner, bi = zz % g.inner;
   const cplx *__restrict__ A = batch_ptr(g.A, cell, bi);
   const cplx *__restrict__ B = batch_ptr(g.B, cell, bi);
-  cplx *C = batch_ptr(g.C, cell, bi);
+  cplx *C = batch_ptr(g.C, cell, bi) + (size_t)ks * g.split_stride;
 
   int klo = 0, khi = g.K;
+  if (nsplit > 1) {
+    const int kc = ((g.K + nsplit - 1) / nsplit + BK - 1) / BK * BK;
+    klo = ks * kc;
+    khi = min(g.K, klo + kc);
+  }
   if (g.flags & BS_GEMM_KLO_ROW) klo = max(klo, m0);
   if (g.flags & BS_GEMM_KHI_ROW) khi = min(khi, m0 + BM);
   if (g.flags & BS_GEMM_KLO_COL) klo = max(klo, n0);
@@ -183,7 +190,7 @@ void launch_one(const GemmDesc &g, cudaStream_t s) {
     cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_done = true;
   }
-  dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner);
+  dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1));
   zgemm_kernel<OPA, OPB, HERM, BM, BN><<<grid, NT, smem, s>>>(g);
 }
 }  // namespace

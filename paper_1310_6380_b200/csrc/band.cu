@@ -32,106 +32,254 @@ __device__ __forceinline__ double block_sum_q(double x, double *scratch) {
   return s;
 }
 
-// Householder QR of the m x b panel block of every matrix, right-looking, one CTA per matrix.  R overwrites the upper
-// triangle of the block (the part that lies inside the band); V goes to columns [0,b) and [2b,3b) of VW (rows indexed
-// globally, zeros above the unit diagonal and in unused columns); tau to SM + tau_off.
-__global__ void __launch_bounds__(QT) panel_qr_kernel(int n, int lda, int b, int c0, BatchRef A, BatchRef VW, BatchRef SM,
-                                                      int inner) {
-  __shared__ cplx vs[NMAXQ];
-  __shared__ double scratch[QT / 32];
-  __shared__ cplx s_tau, s_scale;
+// Householder QR of the m x b panel block of every matrix, one CTA per matrix.  The panel is processed in sub-panels
+// of SW = 4 columns held in shared memory: a sub-panel is factored there (no global round trips between its columns), its
+// four reflectors are then applied to the remaining panel columns as one compact-WY update (two passes over each column
+// instead of eight; one warp per column).  R overwrites the upper triangle of the block (the part that lies inside the
+// band); V goes to columns [0,b) and [2b,3b) of VW (rows indexed globally, zeros above the unit diagonal and in unused
+// columns); tau to SM + 4 b^2.
+constexpr int SW = 4;  // sub-panel width
+constexpr int CH = 4;  // trailing panel columns updated together
+
+template <int K, int NTHR>
+__device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double *res) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int k = 0; k < K; ++k) red[warp * K + k] = v[k];
+  }
+  __syncthreads();
+  if (warp == 0) {
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+      double x = lane < NTHR / 32 ? red[lane * K + k] : 0.0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+      if (lane == 0) res[k] = x;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < K; ++k) v[k] = res[k];
+  // no third barrier: the next reduction writes `res` only after its own first barrier, which every thread reaches
+  // after these reads; its `red` writes come after this reduction's second barrier
+}
+
+template <int NTHR>
+__global__ void __launch_bounds__(NTHR) panel_qr_kernel(int n, int lda, int b, int c0, BatchRef A, BatchRef VW, BatchRef SM,
+                                                        int inner) {
+  extern __shared__ __align__(16) unsigned char qr_smem[];
+  const int r0 = c0 + b, m = n - r0;
+  cplx *sp = reinterpret_cast<cplx *>(qr_smem);                 // [SW][m]
+  double *red = reinterpret_cast<double *>(sp + (size_t)SW * m);  // [NTHR/32][32]
+  double *res = red + (NTHR / 32) * 32;                           // [32]
+  cplx *scal = reinterpret_cast<cplx *>(res + 32);                // tau, scale, then T (SW x SW)
+  cplx *Tm = scal + 2;
   const int z = blockIdx.x, cell = z / inner, mi = z % inner;
   cplx *Ag = batch_ptr(A, cell, mi);
   cplx *V1 = batch_ptr(VW, cell, mi);
   cplx *V2 = V1 + (size_t)2 * b * n;
   double *tau_out = reinterpret_cast<double *>(batch_ptr(SM, cell, mi) + (size_t)4 * b * b);
-  const int r0 = c0 + b, m = n - r0;
   const int kq = min(b, m - 1);
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
-  for (int j = 0; j < b; ++j) {
-    cplx *colj = Ag + (size_t)(c0 + j) * lda;
-    const int pr = r0 + j;  // pivot row
-    if (j >= kq) {          // no reflector: V column = 0, tau = 0
-      for (int r = r0 + t; r < n; r += QT) {
-        V1[(size_t)j * n + r] = cmake(0.0, 0.0);
-        V2[(size_t)j * n + r] = cmake(0.0, 0.0);
-      }
-      if (t == 0) { tau_out[2 * j] = 0.0; tau_out[2 * j + 1] = 0.0; }
-      continue;
-    }
-    double ss = 0.0;
-    for (int r = pr + 1 + t; r < n; r += QT) {
-      const cplx x = colj[r];
-      ss += x.x * x.x + x.y * x.y;
-    }
-    ss = block_sum_q(ss, scratch);
-    if (t == 0) {
-      const cplx al = colj[pr];
-      cplx tau, scale;
-      double beta;
-      if (ss == 0.0 && al.y == 0.0) {
-        tau = cmake(0.0, 0.0); scale = cmake(0.0, 0.0); beta = al.x;
-      } else {
-        beta = -copysign(sqrt(al.x * al.x + al.y * al.y + ss), al.x);
-        tau = cmake((beta - al.x) / beta, -al.y / beta);
-        const double dr = al.x - beta, di = al.y, den = 1.0 / (dr * dr + di * di);
-        scale = cmake(dr * den, -di * den);
-      }
-      s_tau = tau; s_scale = scale;
-      tau_out[2 * j] = tau.x; tau_out[2 * j + 1] = tau.y;
-      colj[pr] = cmake(beta, 0.0);
+
+  for (int js = 0; js < b; js += SW) {
+    // 1. sub-panel -> shared memory
+    for (int q = t; q < SW * m; q += NTHR) {
+      const int jj = q / m, i = q % m;
+      sp[q] = Ag[(size_t)(r0 + i) + (size_t)(c0 + js + jj) * lda];
     }
     __syncthreads();
-    const cplx tau = s_tau, scale = s_scale;
-    for (int r = r0 + t; r < n; r += QT) {
-      cplx v = cmake(0.0, 0.0);
-      if (r == pr) v = cmake(1.0, 0.0);
-      else if (r > pr) v = cmul(colj[r], scale);
-      vs[r - r0] = v;
-      V1[(size_t)j * n + r] = v;
-      V2[(size_t)j * n + r] = v;
-    }
-    __syncthreads();
-    // apply H_j^H = I - conj(tau) v v^H to the remaining columns of the panel: one warp per column
-    if (tau.x != 0.0 || tau.y != 0.0) {
-      for (int c = j + 1 + warp; c < b; c += QT / 32) {
-        cplx *col = Ag + (size_t)(c0 + c) * lda;
-        cplx dot = cmake(0.0, 0.0), dot2 = cmake(0.0, 0.0);
-        int r = pr + lane;
-        for (; r + 224 < n; r += 256) {  // 8 independent 16-byte loads in flight per lane
-          cplx x[8];
+    cplx taus[SW];
+    double nxt = -1.0;  // partial sum of |x|^2 below the pivot of the next column, gathered while it is updated
+    // 2. factor it
 #pragma unroll
-          for (int u = 0; u < 8; ++u) x[u] = col[r + 32 * u];
+    for (int jj = 0; jj < SW; ++jj) {
+      const int j = js + jj;  // local pivot index = j
+      cplx *cj = sp + (size_t)jj * m;
+      cplx *gj = Ag + (size_t)(c0 + j) * lda + r0;
+      if (j >= kq) {  // nothing below the pivot: the whole column is R; no reflector
+        for (int i = t; i < m; i += NTHR) { gj[i] = cj[i]; }
+        __syncthreads();
+        for (int i = t; i < m; i += NTHR) cj[i] = cmake(0.0, 0.0);
+        if (t == 0) { tau_out[2 * j] = 0.0; tau_out[2 * j + 1] = 0.0; }
+        taus[jj] = cmake(0.0, 0.0);
+        __syncthreads();
+        continue;
+      }
+      double nv[1] = {0.0};
+      if (nxt >= 0.0) nv[0] = nxt;
+      else for (int i = j + 1 + t; i < m; i += NTHR) { const cplx x = cj[i]; nv[0] += x.x * x.x + x.y * x.y; }
+      nxt = -1.0;
+      block_reduce<1, NTHR>(nv, red, res);
+      if (t == 0) {
+        const cplx al = cj[j];
+        const double ss = nv[0];
+        cplx tau, scale;
+        double beta;
+        if (ss == 0.0 && al.y == 0.0) {
+          tau = cmake(0.0, 0.0); scale = cmake(0.0, 0.0); beta = al.x;
+        } else {
+          beta = -copysign(sqrt(al.x * al.x + al.y * al.y + ss), al.x);
+          tau = cmake((beta - al.x) / beta, -al.y / beta);
+          const double dr = al.x - beta, di = al.y, den = 1.0 / (dr * dr + di * di);
+          scale = cmake(dr * den, -di * den);
+        }
+        scal[0] = tau; scal[1] = scale;
+        tau_out[2 * j] = tau.x; tau_out[2 * j + 1] = tau.y;
+        gj[j] = cmake(beta, 0.0);  // R diagonal
+      }
+      __syncthreads();
+      const cplx tau = scal[0], scale = scal[1];
+      taus[jj] = tau;
+      // R entries above the pivot go home; the column becomes v (zeros above, 1 at the pivot)
+      double dv[2 * (SW - 1)];
 #pragma unroll
-          for (int u = 0; u < 8; u += 2) {
-            cfmac(dot, vs[r + 32 * u - r0], x[u]);
-            cfmac(dot2, vs[r + 32 * (u + 1) - r0], x[u + 1]);
+      for (int k = 0; k < 2 * (SW - 1); ++k) dv[k] = 0.0;
+      for (int i = t; i < m; i += NTHR) {
+        cplx v;
+        if (i < j) { gj[i] = cj[i]; v = cmake(0.0, 0.0); }
+        else if (i == j) v = cmake(1.0, 0.0);
+        else v = cmul(cj[i], scale);
+        cj[i] = v;
+        if (i >= j) {
+#pragma unroll
+          for (int kk = jj + 1; kk < SW; ++kk) {
+            const cplx x = sp[(size_t)kk * m + i];
+            dv[2 * (kk - 1)] += v.x * x.x + v.y * x.y;      // conj(v) x
+            dv[2 * (kk - 1) + 1] += v.x * x.y - v.y * x.x;
           }
         }
-        for (; r < n; r += 32) cfmac(dot, vs[r - r0], col[r]);
-        dot = cadd(dot, dot2);
+      }
+      if (jj + 1 < SW) {
+        block_reduce<2 * (SW - 1), NTHR>(dv, red, res);
+        nxt = 0.0;
+        for (int i = j + t; i < m; i += NTHR) {
+          const cplx v = cj[i];
+#pragma unroll
+          for (int kk = jj + 1; kk < SW; ++kk) {
+            const cplx f = cmul(cconj(tau), cmake(dv[2 * (kk - 1)], dv[2 * (kk - 1) + 1]));
+            cplx x = sp[(size_t)kk * m + i];
+            cfms(x, v, f);
+            sp[(size_t)kk * m + i] = x;
+            if (kk == jj + 1 && i > j + 1) nxt += x.x * x.x + x.y * x.y;
+          }
+        }
+        if (j + 1 >= kq) nxt = -1.0;  // the next column has no reflector
+      }
+      __syncthreads();
+    }
+    // 3. Gram entries v_a^H v_b (a < b) -> T of the sub-panel (forward columnwise compact WY)
+    {
+      double gv[12];
+#pragma unroll
+      for (int k = 0; k < 12; ++k) gv[k] = 0.0;
+      for (int i = js + t; i < m; i += NTHR) {
+        cplx v[SW];
+#pragma unroll
+        for (int jj = 0; jj < SW; ++jj) v[jj] = sp[(size_t)jj * m + i];
+        int e = 0;
+#pragma unroll
+        for (int a = 0; a < SW; ++a)
+#pragma unroll
+          for (int c = a + 1; c < SW; ++c) {
+            gv[2 * e] += v[a].x * v[c].x + v[a].y * v[c].y;
+            gv[2 * e + 1] += v[a].x * v[c].y - v[a].y * v[c].x;
+            ++e;
+          }
+      }
+      block_reduce<12, NTHR>(gv, red, res);
+      if (t == 0) {
+        cplx Gm[SW][SW];
+        int e = 0;
+        for (int a = 0; a < SW; ++a)
+          for (int c = a + 1; c < SW; ++c) { Gm[a][c] = cmake(gv[2 * e], gv[2 * e + 1]); ++e; }
+        cplx Tl[SW][SW];
+        for (int a = 0; a < SW; ++a)
+          for (int c = 0; c < SW; ++c) Tl[a][c] = cmake(0.0, 0.0);
+        for (int c = 0; c < SW; ++c) {
+          Tl[c][c] = taus[c];
+          for (int a = 0; a < c; ++a) {
+            cplx acc = cmake(0.0, 0.0);
+            for (int l2 = a; l2 < c; ++l2) cfma(acc, Tl[a][l2], Gm[l2][c]);
+            Tl[a][c] = cmul(cmake(-taus[c].x, -taus[c].y), acc);
+          }
+        }
+        for (int a = 0; a < SW; ++a)
+          for (int c = 0; c < SW; ++c) Tm[a * SW + c] = Tl[a][c];
+      }
+    }
+    // 4. V columns out
+    for (int q = t; q < SW * m; q += NTHR) {
+      const int jj = q / m, i = q % m;
+      const cplx v = sp[q];
+      V1[(size_t)(js + jj) * n + r0 + i] = v;
+      V2[(size_t)(js + jj) * n + r0 + i] = v;
+    }
+    __syncthreads();  // Tm visible
+    // 5. remaining panel columns: x <- x - V T^H (V^H x), one warp per column, rows >= js
+    cplx Tr[SW][SW];
+#pragma unroll
+    for (int a = 0; a < SW; ++a)
+#pragma unroll
+      for (int c = 0; c < SW; ++c) Tr[a][c] = Tm[a * SW + c];
+    for (int c = js + SW + warp; c < b; c += NTHR / 32) {
+      cplx *col = Ag + (size_t)(c0 + c) * lda + r0;
+      cplx d[SW];
+#pragma unroll
+      for (int k = 0; k < SW; ++k) d[k] = cmake(0.0, 0.0);
+      int i = js + lane;
+      for (; i + 96 < m; i += 128) {  // 4 independent loads in flight per lane
+        cplx x[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) x[u] = col[i + 32 * u];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+          for (int k = 0; k < SW; ++k) cfmac(d[k], sp[(size_t)k * m + i + 32 * u], x[u]);
+      }
+      for (; i < m; i += 32) {
+        const cplx x = col[i];
+#pragma unroll
+        for (int k = 0; k < SW; ++k) cfmac(d[k], sp[(size_t)k * m + i], x);
+      }
+#pragma unroll
+      for (int k = 0; k < SW; ++k) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
-          dot.x += __shfl_xor_sync(0xffffffffu, dot.x, o);
-          dot.y += __shfl_xor_sync(0xffffffffu, dot.y, o);
+          d[k].x += __shfl_xor_sync(0xffffffffu, d[k].x, o);
+          d[k].y += __shfl_xor_sync(0xffffffffu, d[k].y, o);
         }
-        const cplx f = cmul(cconj(tau), dot);
-        r = pr + lane;
-        for (; r + 224 < n; r += 256) {
-          cplx x[8];
+      }
+      cplx gk[SW];  // g = T^H d
 #pragma unroll
-          for (int u = 0; u < 8; ++u) x[u] = col[r + 32 * u];
+      for (int k = 0; k < SW; ++k) {
+        gk[k] = cmake(0.0, 0.0);
 #pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            cfms(x[u], vs[r + 32 * u - r0], f);
-            col[r + 32 * u] = x[u];
-          }
+        for (int l2 = 0; l2 <= k; ++l2) cfmac(gk[k], Tr[l2][k], d[l2]);
+      }
+      i = js + lane;
+      for (; i + 96 < m; i += 128) {
+        cplx x[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) x[u] = col[i + 32 * u];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+#pragma unroll
+          for (int k = 0; k < SW; ++k) cfms(x[u], sp[(size_t)k * m + i + 32 * u], gk[k]);
+          col[i + 32 * u] = x[u];
         }
-        for (; r < n; r += 32) {
-          cplx x = col[r];
-          cfms(x, vs[r - r0], f);
-          col[r] = x;
-        }
+      }
+      for (; i < m; i += 32) {
+        cplx x = col[i];
+#pragma unroll
+        for (int k = 0; k < SW; ++k) cfms(x, sp[(size_t)k * m + i], gk[k]);
+        col[i] = x;
       }
     }
     __syncthreads();
@@ -220,6 +368,8 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
   const int nmat = ncells * inner;
   static bool attr_done = false;
   if (!attr_done) {
+    cudaFuncSetAttribute(panel_qr_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 140 * 1024);
+    cudaFuncSetAttribute(panel_qr_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
     cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 32 * 32 * (int)sizeof(cplx));
     attr_done = true;
   }
@@ -227,7 +377,13 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     const int r0 = c0 + b, m = n - r0;  // m >= 2
     {
       KScope ks(KC_PANEL, 0.0, s);
-      panel_qr_kernel<<<nmat, QT, 0, s>>>(n, lda, b, c0, A, VW, SM, inner);
+      if (m > 640) {
+        const size_t smem = (size_t)SW * m * sizeof(cplx) + (32 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
+        panel_qr_kernel<1024><<<nmat, 1024, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
+      } else {
+        const size_t smem = (size_t)SW * m * sizeof(cplx) + (8 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
+        panel_qr_kernel<256><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
+      }
       ++launches;
     }
     GemmDesc g{};
@@ -250,7 +406,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     launch_zgemm(g, s); ++launches;
     g.ksplit = 0; g.split_stride = 0;
     {
-      KScope ks(KC_PANEL, 0.0, s);
+      KScope ks(KC_OTHER, 0.0, s);
       wy_small_kernel<<<nmat, 256, 4 * b * b * sizeof(cplx), s>>>(b, SM, inner);
       ++launches;
     }

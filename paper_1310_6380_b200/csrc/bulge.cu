@@ -206,22 +206,24 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
         const bool t_on = (tau.x != 0.0 || tau.y != 0.0);
         const int Jn = J + L, L2 = min(B, n - Jn);
         // P1: partial p = D v over this thread's quarter of the columns; P4: partial u = C v
+        // (branch-free: every index is a valid ring address, invalid contributions are masked through v)
         cplx acc = cmake(0.0, 0.0), uacc = cmake(0.0, 0.0);
         if (t_on) {
 #pragma unroll
           for (int jj = 0; jj < QN; ++jj) {
             const int c = q * QN + jj;
-            if (c < L) {
-              const cplx vc = vs[c];
-              const cplx *pcol = ring + cb[jj];
-              if (l < L) {
-                cplx a = ring[l >= c ? cb[jj] + l - c : mycb + c - l];  // lower part as stored, upper part mirrored
-                a.y = l > c ? a.y : (l == c ? 0.0 : -a.y);
-                cfma(acc, a, vc);
-              }
-              if (l < L2) cfma(uacc, pcol[L + l - c], vc);
-            }
+            cplx vc = vs[c];
+            vc.x = c < L ? vc.x : 0.0;
+            vc.y = c < L ? vc.y : 0.0;
+            cplx a = ring[l >= c ? cb[jj] + l - c : mycb + c - l];  // lower part as stored, upper part mirrored
+            a.y = l > c ? a.y : (l == c ? 0.0 : -a.y);
+            cfma(acc, a, vc);
+            cfma(uacc, ring[cb[jj] + L + l - c], vc);
           }
+          acc.x = l < L ? acc.x : 0.0;
+          acc.y = l < L ? acc.y : 0.0;
+          uacc.x = l < L2 ? uacc.x : 0.0;
+          uacc.y = l < L2 ? uacc.y : 0.0;
         }
         red1[q * B + l] = acc;
         red2[q * B + l] = uacc;
@@ -253,19 +255,27 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
         }
         if (q == 0) { ws[l] = w; tus[l] = tu; v2s[l] = v2; }
         team_bar();  // BAR2
-        // P3: D <- D - v w^H - w v^H on the lower triangle
-        if (t_on && l < L) {
+        // P3: D <- D - v w^H - w v^H on the lower triangle (all loads first, then all stores: no false dependences)
+        if (t_on) {
+          cplx av[QN];
 #pragma unroll
           for (int jj = 0; jj < QN; ++jj) {
             const int c = q * QN + jj;
-            if (c <= l) {
-              cplx *pa = ring + cb[jj] + (l - c);
-              cplx a = *pa;
-              cfms(a, v, cconj(ws[c]));
-              cfms(a, w, cconj(vs[c]));
-              if (l == c) a.y = 0.0;
-              *pa = a;
-            }
+            av[jj] = ring[cb[jj] + max(l - c, 0)];
+          }
+#pragma unroll
+          for (int jj = 0; jj < QN; ++jj) {
+            const int c = q * QN + jj;
+            cplx a = av[jj];
+            cfms(a, v, cconj(ws[c]));
+            cfms(a, w, cconj(vs[c]));
+            a.y = l == c ? 0.0 : a.y;
+            av[jj] = a;
+          }
+#pragma unroll
+          for (int jj = 0; jj < QN; ++jj) {
+            const int c = q * QN + jj;
+            if (c <= l && l < L) ring[cb[jj] + (l - c)] = av[jj];
           }
         }
         if (L2 <= 0) {
@@ -283,14 +293,16 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
 #pragma unroll
             for (int jj = 0; jj < QN; ++jj) {
               const int r = q * QN + jj;
-              tv[jj] = cmake(0.0, 0.0);
-              if (mine && r < L2) {
-                cplx t = pc[r];
-                cfms(t, tus[r], vcj);
-                cfmac(zacc, v2s[r], t);
-                tv[jj] = t;
-              }
+              cplx t = pc[r];
+              cplx tur = tus[r], v2r = v2s[r];
+              v2r.x = r < L2 ? v2r.x : 0.0;  // rows beyond the block do not contribute
+              v2r.y = r < L2 ? v2r.y : 0.0;
+              cfms(t, tur, vcj);
+              cfmac(zacc, v2r, t);
+              tv[jj] = t;
             }
+            zacc.x = mine ? zacc.x : 0.0;
+            zacc.y = mine ? zacc.y : 0.0;
             red3[q * B + l] = zacc;
             team_bar();  // BAR3
             const cplx zc = qsum(red3);
@@ -298,11 +310,9 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
 #pragma unroll
             for (int jj = 0; jj < QN; ++jj) {
               const int r = q * QN + jj;
-              if (mine && r < L2) {
-                cplx t = tv[jj];
-                cfms(t, v2s[r], f);
-                pc[r] = t;
-              }
+              cplx t = tv[jj];
+              cfms(t, v2s[r], f);
+              if (mine && r < L2) pc[r] = t;
             }
           }
           if (q == 0) vs[l] = v2;  // after BAR3 (or with P3 skipped): nobody still reads the old v

@@ -34,6 +34,8 @@ __global__ void __launch_bounds__(256) potrf_diag_kernel(int n, int lda, int j0,
     X[c][r] = cmake(0.0, 0.0);
   }
   __syncthreads();
+  // thread (r, g): row r = t & 63, column group g = t >> 6 (columns c+1+g, c+5+g, ...)
+  const int r = t & (NB - 1), g = t >> 6;
   for (int c = 0; c < nbk; ++c) {
     if (t == 0) {
       double piv = S[c][c].x;
@@ -45,31 +47,36 @@ __global__ void __launch_bounds__(256) potrf_diag_kernel(int n, int lda, int j0,
     }
     __syncthreads();
     const double dinvc = 1.0 / S[c][c].x;
-    for (int r = c + 1 + t; r < nbk; r += blockDim.x) S[c][r] = cscale(S[c][r], dinvc);
+    if (g == 0 && r > c && r < nbk) S[c][r] = cscale(S[c][r], dinvc);
     __syncthreads();
-    // trailing update of the block: S[r][cc] -= S[r][c] conj(S[cc][c]),  c < cc <= r
-    const int m = nbk - c - 1;
-    for (int i = t; i < m * m; i += blockDim.x) {
-      const int rr = c + 1 + i % m, cc = c + 1 + i / m;
-      if (rr >= cc) {
-        cplx v = S[cc][rr];
-        cfms(v, S[c][rr], cconj(S[c][cc]));
-        S[cc][rr] = v;
+    // trailing update of the block: S[cc][r] -= S[c][r] conj(S[c][cc]),  c < cc <= r
+    if (r > c && r < nbk) {
+      const cplx lr = S[c][r];
+      for (int cc = c + 1 + g; cc <= r; cc += 4) {
+        cplx v = S[cc][r];
+        cfms(v, lr, cconj(S[c][cc]));
+        S[cc][r] = v;
       }
     }
     __syncthreads();
   }
-  // X = L^{-1}: thread c solves column c by forward substitution.
-  if (t < nbk) {
-    const int c = t;
-    X[c][c] = cmake(1.0 / S[c][c].x, 0.0);
-    for (int r = c + 1; r < nbk; ++r) {
-      cplx acc = cmake(0.0, 0.0);
-      for (int k = c; k < r; ++k) cfma(acc, S[k][r], X[c][k]);
-      X[c][r] = cscale(acc, -1.0 / S[r][r].x);
-    }
-  }
+  // X = L^{-1} row by row: X[r][c] = -(1/L[r][r]) sum_{k=c}^{r-1} L[r][k] X[k][c]; thread (c, g) sums k = c+g, c+g+4, ...
+  __shared__ cplx psum[4][NB];
+  if (g == 0 && r < nbk) X[r][r] = cmake(1.0 / S[r][r].x, 0.0);
   __syncthreads();
+  for (int rr = 1; rr < nbk; ++rr) {
+    const int c = r;
+    cplx acc = cmake(0.0, 0.0);
+    if (c < rr)
+      for (int k = c + g; k < rr; k += 4) cfma(acc, S[k][rr], X[c][k]);
+    psum[g][c] = acc;
+    __syncthreads();
+    if (g == 0 && c < rr) {
+      const cplx sum = cadd(cadd(psum[0][c], psum[1][c]), cadd(psum[2][c], psum[3][c]));
+      X[c][rr] = cscale(sum, -1.0 / S[rr][rr].x);
+    }
+    __syncthreads();
+  }
   for (int i = t; i < NB * NB; i += blockDim.x) {
     const int r = i % NB, c = i / NB;
     if (r < nbk && c < nbk) Ag[(size_t)r + (size_t)c * lda] = S[c][r];  // zeros above the diagonal of the block

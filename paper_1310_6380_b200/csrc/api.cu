@@ -602,6 +602,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   const Layout L = make_layout(Mt, nk, lead->mode, lead->nb);
   const int N = L.N, n2 = 2 * N, n3 = 3 * N;
   if (nbands < 1 || nbands > n2) return fail(BS_ERR_ARG, "bs_bands: nbands must be in 1..2N = %d", n2);
+  if ((long long)ncells * nk > 65535) return fail(BS_ERR_ARG, "bs_bands: ncells * nk = %lld exceeds 65535 matrices per call", (long long)ncells * nk);
   for (int c = 0; c < ncells; ++c)
     if ((size_t)L.total * sizeof(cplx) > cells[c]->ws_bytes)
       return fail(BS_ERR_NOMEM, "bs_bands: cells[%d] workspace is %zu bytes, %d k-points need %zu", c, cells[c]->ws_bytes, nk,

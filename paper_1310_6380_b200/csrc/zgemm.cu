@@ -39,10 +39,13 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
   cplx(*As)[BK][LDA_S] = reinterpret_cast<cplx(*)[BK][LDA_S]>(smem_raw);
   cplx(*Bs)[BK][LDB_S] = reinterpret_cast<cplx(*)[BK][LDB_S]>(smem_raw + (size_t)STAGES * BK * LDA_S * sizeof(cplx));
 
-  const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+  // grid.x = (M tiles) x (matrices x k-splits): grid.z is limited to 65535, the batch of config 4 is not
+  const int tiles_m = (g.M + BM - 1) / BM;
+  const int bz = blockIdx.x / tiles_m;
+  const int m0 = (blockIdx.x % tiles_m) * BM, n0 = blockIdx.y * BN;
   if ((g.flags & BS_GEMM_LOWER_ONLY) && n0 >= m0 + BM) return;
   const int nsplit = g.ksplit > 1 ? g.ksplit : 1;
-  const int ks = blockIdx.z % nsplit, zz = blockIdx.z / nsplit;
+  const int ks = bz % nsplit, zz = bz / nsplit;
   const int cell = zz / g.inner, bi = zz % g.inner;
   const cplx *__restrict__ A = batch_ptr(g.A, cell, bi);
   const cplx *__restrict__ B = batch_ptr(g.B, cell, bi);
@@ -190,7 +193,7 @@ void launch_one(const GemmDesc &g, cudaStream_t s) {
     cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_done = true;
   }
-  dim3 grid((g.M + BM - 1) / BM, (g.N + BN - 1) / BN, g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1));
+  dim3 grid(((g.M + BM - 1) / BM) * g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1), (g.N + BN - 1) / BN, 1);
   zgemm_kernel<OPA, OPB, HERM, BM, BN><<<grid, NT, smem, s>>>(g);
 }
 }  // namespace

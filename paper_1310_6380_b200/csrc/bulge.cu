@@ -348,6 +348,12 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
     G = max(1, min(G, gmax));
     Wc = 2 * G * B + 8;
   }
+  static const int g_env = getenv("BS_BULGE_G") ? atoi(getenv("BS_BULGE_G")) : 0;  // experiment knob
+  if (g_env > 0) {
+    G = min(g_env, gmax);
+    Wc = 2 * G * B + 8;
+    if (Wc >= n) Wc = n;
+  }
   const size_t smem = (size_t)Wc * colbytes + G * team_bytes;
   static bool attr_done = false;
   if (!attr_done) {

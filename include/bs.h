@@ -137,7 +137,7 @@ bs_status bs_get_timings(bs_cell *cell, double *ms_out);
 
 /* Kernel classes of bs_get_kernel_timings. */
 enum {
-  BS_KC_TABLE = 0,        /* S1 table kernel                                    work: 0 (ALU-bound)   */
+  BS_KC_TABLE = 0,        /* S1 table kernel (FP64 ALU)                         work: real flops                     */
   BS_KC_EXPAND = 1,       /* S2 expansion                                       work: bytes written                  */
   BS_KC_GEMM_FACTOR = 2,  /* DMMA zgemm launches of S3                          work: real flops                     */
   BS_KC_GEMM_REDUCE = 3,  /* DMMA zgemm launches of S5 (and of the POLY coefficient reduction)                       */

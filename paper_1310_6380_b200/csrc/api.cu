@@ -475,7 +475,9 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   KtGuard ktg(lead);
 
   tick(lead, 0, s);
-  bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), s); ++nl;  // S1
+  double total_edges = 0.0;
+  for (int c = 0; c < ncells; ++c) total_edges += cells[c]->nedge;
+  bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, s); ++nl;  // S1
   tick(lead, 1, s);
   bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2
   tick(lead, 2, s);

@@ -7,20 +7,19 @@ namespace bsk {
 
 static constexpr double kPi = 3.14159265358979323846264338327950288;
 
-// One warp per index difference D in the half plane {D1>0} u {D1==0, D2>=0}; lanes stride over the edges.
+// One CTA (8 warps) per index difference D in the half plane {D1>0} u {D1==0, D2>=0}; the warps split the edges, lanes
+// stride over a warp's slice, and the 8 x 32 partial sums are reduced in a fixed order (deterministic).
 //   T_c(D) = (-i/|q|^2) sum_edges w_c[phase(e)] (q x e) exp(i q.m_e) j0(q.e/2),   q = D1 q^1 + D2 q^2,
 // and T_c(0) = sum_p w_c[p] area_p.  The phase q.m and the argument of j0 are evaluated in FRACTIONAL coordinates
 // (q.x = 2 pi (D1 H1 + D2 H2) with integer D), so sincospi/sinpi reduce the argument exactly.
 __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table) {
+  __shared__ double part[8][14];
   const int cell = blockIdx.y;
   const Geometry g = geos[cell];
   const int L = 4 * Mt + 1;
   const int L2 = L * L;
-  const int nhalf = (L2 + 1) / 2;
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (warp >= nhalf) return;
-  const int flat = warp + (L2 - 1) / 2;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int flat = blockIdx.x + (L2 - 1) / 2;
   const int D1 = flat / L - 2 * Mt;
   const int D2 = flat % L - 2 * Mt;
   cplx *T = batch_ptr(table, cell, 0);
@@ -30,7 +29,7 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
   for (int c = 0; c < 7; ++c) accr[c] = acci[c] = 0.0;
 
   if (D1 == 0 && D2 == 0) {
-    for (int p = lane; p < g.P; p += 32) {
+    for (int p = threadIdx.x; p < g.P; p += 256) {
       const double a = g.area[p];
 #pragma unroll
       for (int c = 0; c < 7; ++c) accr[c] = fma(g.w[c * g.P + p], a, accr[c]);
@@ -41,7 +40,7 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
     const int ne = g.nedge;
     const double *mh1 = g.edge, *mh2 = g.edge + ne, *eh1 = g.edge + 2 * ne, *eh2 = g.edge + 3 * ne;
     const double *ex = g.edge + 4 * ne, *ey = g.edge + 5 * ne;
-    for (int e = lane; e < ne; e += 32) {
+    for (int e = threadIdx.x; e < ne; e += 256) {
       const double phi = fma((double)D1, mh1[e], (double)D2 * mh2[e]);  // q.m / (2 pi)
       const double u = fma((double)D1, eh1[e], (double)D2 * eh2[e]);    // q.e / (2 pi)  ->  q.e/2 = pi u
       double sn, cs;
@@ -67,29 +66,35 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
     }
   }
   if (lane == 0) {
-    if (D1 == 0 && D2 == 0) {
 #pragma unroll
-      for (int c = 0; c < 7; ++c) T[(size_t)c * L2 + flat] = cmake(accr[c], 0.0);
+    for (int c = 0; c < 7; ++c) { part[warp][2 * c] = accr[c]; part[warp][2 * c + 1] = acci[c]; }
+  }
+  __syncthreads();
+  if (threadIdx.x < 7) {
+    const int c = threadIdx.x;
+    double sr = 0.0, si = 0.0;
+    for (int w = 0; w < 8; ++w) { sr += part[w][2 * c]; si += part[w][2 * c + 1]; }
+    if (D1 == 0 && D2 == 0) {
+      T[(size_t)c * L2 + flat] = cmake(sr, 0.0);
     } else {
       const double qx = D1 * g.Q[0] + D2 * g.Q[2];
       const double qy = D1 * g.Q[1] + D2 * g.Q[3];
       const double inv = 1.0 / (qx * qx + qy * qy);
-#pragma unroll
-      for (int c = 0; c < 7; ++c) {
-        // (-i) * (ar + i ai) = ai - i ar
-        const double re = acci[c] * inv, im = -accr[c] * inv;
-        T[(size_t)c * L2 + flat] = cmake(re, im);
-        T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);  // T(-D) = conj T(D): Phi, R exactly Hermitian
-      }
+      // (-i) * (ar + i ai) = ai - i ar
+      const double re = si * inv, im = -sr * inv;
+      T[(size_t)c * L2 + flat] = cmake(re, im);
+      T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);  // T(-D) = conj T(D): Phi, R exactly Hermitian
     }
   }
 }
 
-void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, cudaStream_t s) {
+void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, cudaStream_t s) {
   const int L = 4 * Mt + 1;
   const int nhalf = (L * L + 1) / 2;
-  dim3 grid((nhalf + 7) / 8, ncells);
-  KScope ks(KC_TABLE, 0.0, s);
+  dim3 grid(nhalf, ncells);
+  // algorithmic work: ~230 real flops per (index difference, edge) term: sincospi + sinpi + the 7-channel accumulation,
+  // counted from the SASS of the loop body (about 95 DFMA, 25 DMUL, 15 DADD)
+  KScope ks(KC_TABLE, 230.0 * total_edges * nhalf, s);
   table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table);
 }
 

@@ -120,7 +120,7 @@ struct Geometry {  // device pointers, per cell
 };
 
 // S1: table[c][(D1+2Mt)*(4Mt+1) + (D2+2Mt)], c < 7.  geo: device array [ncells]; table at BatchRef (inner unused).
-void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, cudaStream_t s);
+void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, cudaStream_t s);
 // S2: Phi (3N x 3N full) and R (N x N full) from the table.
 void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s);
 

@@ -12,16 +12,26 @@ constexpr int G = 8;      // interior shifts per eigenvalue per round -> the int
 constexpr int EPB = ST / G;  // eigenvalues per pass
 constexpr int ROUNDS = 24;   // 9^24 > 2^76
 
+// Number of eigenvalues < x = number of negative q_i = p_i / p_{i-1}, q_0 = d_0 - x, q_i = d_i - x - e_{i-1}^2 / q_{i-1}
+// (a zero pivot is replaced by a tiny negative one, the role of -pivmin in LAPACK dstebz).  Evaluated WITHOUT the division, whose latency (~100 cycles)
+// would serialise the recurrence: p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2}, a sign change between p_{i-1} and p_i
+// is a negative pivot.  The pair (p_{i-1}, p_i) is rescaled by a power of two whenever its exponent leaves [2^-400, 2^400]
+// (this does not change the ratio), so nothing overflows or underflows.
 __device__ __forceinline__ int sturm_count(const double *__restrict__ d, const double *__restrict__ e2, int n, double x,
                                            double pivmin) {
-  int cnt = 0;
-  double q = d[0] - x;
-  if (fabs(q) < pivmin) q = -pivmin;
-  cnt += q < 0.0;
+  double p0 = 1.0, p1 = d[0] - x;
+  if (p1 == 0.0) p1 = -0x1p-200;  // zero pivot -> tiny negative pivot (relative 2^-200: far below rounding)
+  int cnt = p1 < 0.0;
   for (int i = 1; i < n; ++i) {
-    q = d[i] - x - e2[i - 1] / q;
-    if (fabs(q) < pivmin) q = -pivmin;
-    cnt += q < 0.0;
+    double p2 = fma(d[i] - x, p1, -(e2[i - 1] * p0));
+    if (p2 == 0.0) p2 = -0x1p-200 * p1;               // q_i = -2^-200 (|p1| >= 2^-453 after rescaling: no underflow)
+    cnt += (p2 < 0.0) != (p1 < 0.0);
+    const int ex = (__double2hiint(p2) >> 20) & 0x7ff;
+    double sc = 1.0;
+    if (ex > 1023 + 400) sc = 0x1p-400;
+    else if (ex < 1023 - 400) sc = 0x1p+400;
+    p0 = p1 * sc;
+    p1 = p2 * sc;
   }
   return cnt;
 }

@@ -135,191 +135,226 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
     __syncthreads();
   }
 
-  for (int t0 = 0; t0 < n - 1; t0 += G) {
-    const int nvalid = min(G, n - 1 - t0);  // sweeps t0 .. t0+nvalid-1
-    if (!resident) {
-      // (re)position the window at the head of the band for this train
-      const int need = min(n, t0 + 1 + B);
-      if (t0 < wlo || t0 >= whi) {
-        io_evict(max(wlo, t0), whi, tid, blockDim.x);  // columns < t0 are finished: never read again
-        __syncthreads();
-        io_load(t0, need, tid, blockDim.x);
-        wlo = t0; whi = need;
-      } else if (whi < need) {
-        io_load(whi, need, tid, blockDim.x);
-        whi = need;
+  // per-team sweep state (identical in all threads of a team)
+  int i = 0, k = 0, J = 0, L = 0;
+  bool finished = true;
+  cplx v = cmake(0.0, 0.0), tau = cmake(0.0, 0.0);
+  // one step of sweep i (the whole team executes it)
+  auto do_step = [&]() {
+    // -------------------------------------------------------------------- one step of sweep i
+    if (k == 0) {
+      L = min(B, n - 1 - i);
+      const cplx *ci = ring + (size_t)slot_of(i) * LD;
+      cplx x = l < L ? ci[1 + l] : cmake(0.0, 0.0);
+      double beta;
+      group_larfg<B>(x, L, l, tau, beta);
+      v = x;
+      if (tt == 0) { eg[i] = beta; dg[i] = ci[0].x; }
+      if (q == 0) vs[l] = v;
+      team_bar();
+    }
+    const int sJ = slot_of(J);
+    // element offsets of the ring columns this thread touches: its quarter (J + q QN + jj) and column J + l
+    int cb[QN];
+#pragma unroll
+    for (int jj = 0; jj < QN; ++jj) {
+      int sl = sJ + q * QN + jj;
+      if (sl >= Wc) sl -= Wc;
+      cb[jj] = sl * LD;
+    }
+    int mycb = sJ + l;
+    if (mycb >= Wc) mycb -= Wc;
+    mycb *= LD;
+    const int cb0 = sJ * LD;
+    const bool t_on = (tau.x != 0.0 || tau.y != 0.0);
+    const int Jn = J + L, L2 = min(B, n - Jn);
+    // P1: partial p = D v over this thread's quarter of the columns; P4: partial u = C v
+    // (branch-free: every index is a valid ring address, invalid contributions are masked through v)
+    cplx acc = cmake(0.0, 0.0), uacc = cmake(0.0, 0.0);
+    if (t_on) {
+#pragma unroll
+      for (int jj = 0; jj < QN; ++jj) {
+        const int c = q * QN + jj;
+        cplx vc = vs[c];
+        vc.x = c < L ? vc.x : 0.0;
+        vc.y = c < L ? vc.y : 0.0;
+        cplx a = ring[l >= c ? cb[jj] + l - c : mycb + c - l];  // lower part as stored, upper part mirrored
+        a.y = l > c ? a.y : (l == c ? 0.0 : -a.y);
+        cfma(acc, a, vc);
+        cfma(uacc, ring[cb[jj] + L + l - c], vc);
+      }
+      acc.x = l < L ? acc.x : 0.0;
+      acc.y = l < L ? acc.y : 0.0;
+      uacc.x = l < L2 ? uacc.x : 0.0;
+      uacc.y = l < L2 ? uacc.y : 0.0;
+    }
+    red1[q * B + l] = acc;
+    red2[q * B + l] = uacc;
+    team_bar();  // BAR1
+    cplx p = qsum(red1);
+    p = cmul(tau, p);
+    const double sr = group_sum<B>(l < L ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
+    const double si = group_sum<B>(l < L ? p.x * v.y - p.y * v.x : 0.0);
+    const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
+    cplx w = p;
+    cfma(w, alpha, v);
+    const cplx u = qsum(red2);
+    const cplx tu = cmul(tau, u);
+    // P5: first column of C after the right-apply, and the reflector that annihilates it
+    cplx tau2 = cmake(0.0, 0.0), v2 = cmake(0.0, 0.0);
+    if (L2 > 0) {
+      cplx *c0p = ring + cb0 + L;
+      cplx x = cmake(0.0, 0.0);
+      if (l < L2) x = csub(c0p[l], tu);  // conj(v[0]) = 1
+      if (L2 > 1) {
+        double beta2;
+        group_larfg<B>(x, L2, l, tau2, beta2);
+        v2 = x;
+        if (q == 0 && l < L2) c0p[l] = (l == 0) ? cmake(beta2, 0.0) : cmake(0.0, 0.0);
+      } else {
+        if (tt == 0) c0p[0] = x;
+        v2 = (l == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+      }
+    }
+    if (q == 0) { ws[l] = w; tus[l] = tu; v2s[l] = v2; }
+    team_bar();  // BAR2
+    // P3: D <- D - v w^H - w v^H on the lower triangle (all loads first, then all stores: no false dependences)
+    if (t_on) {
+      cplx av[QN];
+#pragma unroll
+      for (int jj = 0; jj < QN; ++jj) {
+        const int c = q * QN + jj;
+        av[jj] = ring[cb[jj] + max(l - c, 0)];
+      }
+#pragma unroll
+      for (int jj = 0; jj < QN; ++jj) {
+        const int c = q * QN + jj;
+        cplx a = av[jj];
+        cfms(a, v, cconj(ws[c]));
+        cfms(a, w, cconj(vs[c]));
+        a.y = l == c ? 0.0 : a.y;
+        av[jj] = a;
+      }
+#pragma unroll
+      for (int jj = 0; jj < QN; ++jj) {
+        const int c = q * QN + jj;
+        if (c <= l && l < L) ring[cb[jj] + (l - c)] = av[jj];
+      }
+    }
+    if (L2 <= 0) {
+      finished = true;
+    } else {
+      const bool t2_on = (tau2.x != 0.0 || tau2.y != 0.0);
+      if (t_on || t2_on) {
+        // P6/P7: thread = column c = l of C (1 <= c < L), rows of its quarter:
+        //   t = C - (tau C v) v^H ; z = v2^H t ; C = t - v2 conj(tau2) z
+        const bool mine = l >= 1 && l < L;
+        const cplx vcj = cconj(v);
+        cplx *pc = ring + (mine ? mycb + L - l : cb0 + L);
+        cplx tv[QN];
+        cplx zacc = cmake(0.0, 0.0);
+#pragma unroll
+        for (int jj = 0; jj < QN; ++jj) {
+          const int r = q * QN + jj;
+          cplx t = pc[r];
+          cplx tur = tus[r], v2r = v2s[r];
+          v2r.x = r < L2 ? v2r.x : 0.0;  // rows beyond the block do not contribute
+          v2r.y = r < L2 ? v2r.y : 0.0;
+          cfms(t, tur, vcj);
+          cfmac(zacc, v2r, t);
+          tv[jj] = t;
+        }
+        zacc.x = mine ? zacc.x : 0.0;
+        zacc.y = mine ? zacc.y : 0.0;
+        red3[q * B + l] = zacc;
+        team_bar();  // BAR3
+        const cplx zc = qsum(red3);
+        const cplx f = cmul(cconj(tau2), zc);
+#pragma unroll
+        for (int jj = 0; jj < QN; ++jj) {
+          const int r = q * QN + jj;
+          cplx t = tv[jj];
+          cfms(t, v2s[r], f);
+          if (mine && r < L2) pc[r] = t;
+        }
+      }
+      if (q == 0) vs[l] = v2;  // after BAR3 (or with P3 skipped): nobody still reads the old v
+      v = v2; tau = tau2; J = Jn; L = L2; ++k;
+    }
+  };
+
+  if (resident) {
+    // The whole band is in shared memory: no trains, the teams run a continuous pipeline.  Sweep i starts at macro-step
+    // start[i] = max(start[i-1] + 2, finish of sweep i-G) (two blocks behind its predecessor, and its team must be free).
+    int *start = reinterpret_cast<int *>(ring + (size_t)Wc * LD + (size_t)G * (4 + 3 * NQ) * B);
+    if (tid == 0) {
+      for (int j = 0; j <= n - 2; ++j) {
+        int st = j == 0 ? 0 : start[j - 1] + 2;
+        if (j >= G) st = max(st, start[j - G] + (n - 1 - (j - G) + B - 1) / B);
+        start[j] = st;
+      }
+    }
+    __syncthreads();
+    const int S = n >= 2 ? start[n - 2] + 1 : 0;  // the last sweep has a single step
+    int next_i = team;
+    for (int s = 0; s < S; ++s) {
+      if (!is_io) {
+        if (finished && next_i <= n - 2 && start[next_i] == s) {
+          i = next_i; k = 0; J = i + 1; L = 0; finished = false;
+          tau = cmake(0.0, 0.0);
+        }
+        if (!finished) {
+          do_step();
+          if (finished) next_i += G;
+        }
       }
       __syncthreads();
     }
-    // per-team sweep state (identical in all threads of a team)
-    const int i = t0 + team;
-    const bool valid = !is_io && team < nvalid;
-    int k = 0, J = i + 1, L = 0;
-    bool finished = !valid;
-    cplx v = cmake(0.0, 0.0), tau = cmake(0.0, 0.0);
-    const int nsteps0 = (n - 1 - t0 + B - 1) / B;
-    const int S = nsteps0 + 2 * (nvalid - 1);
+  } else {
+    for (int t0 = 0; t0 < n - 1; t0 += G) {
+      const int nvalid = min(G, n - 1 - t0);  // sweeps t0 .. t0+nvalid-1
+      if (!resident) {
+        // (re)position the window at the head of the band for this train
+        const int need = min(n, t0 + 1 + B);
+        if (t0 < wlo || t0 >= whi) {
+          io_evict(max(wlo, t0), whi, tid, blockDim.x);  // columns < t0 are finished: never read again
+          __syncthreads();
+          io_load(t0, need, tid, blockDim.x);
+          wlo = t0; whi = need;
+        } else if (whi < need) {
+          io_load(whi, need, tid, blockDim.x);
+          whi = need;
+        }
+        __syncthreads();
+      }
+      i = t0 + team;
+      const bool valid = !is_io && team < nvalid;
+      k = 0; J = i + 1; L = 0;
+      finished = !valid;
+      v = cmake(0.0, 0.0); tau = cmake(0.0, 0.0);
+      const int nsteps0 = (n - 1 - t0 + B - 1) / B;
+      const int S = nsteps0 + 2 * (nvalid - 1);
 
-    for (int s = 0; s < S; ++s) {
-      if (!resident) {  // window bookkeeping (uniform): columns needed at macro-step s or later / at s+1
-        int keep = n, hi = whi;
-        for (int g = 0; g < nvalid; ++g) {
-          const int ig = t0 + g, kg = s - 2 * g, ns = (n - 1 - ig + B - 1) / B;
-          if (kg >= ns) continue;  // finished
-          keep = min(keep, kg <= 0 ? ig : ig + 1 + kg * B);
-          const int k1 = kg + 1;
-          if (k1 >= 0 && k1 < ns) hi = max(hi, min(n, ig + 1 + (k1 + 1) * B));
+      for (int s = 0; s < S; ++s) {
+        if (!resident) {  // window bookkeeping (uniform): columns needed at macro-step s or later / at s+1
+          int keep = n, hi = whi;
+          for (int g = 0; g < nvalid; ++g) {
+            const int ig = t0 + g, kg = s - 2 * g, ns = (n - 1 - ig + B - 1) / B;
+            if (kg >= ns) continue;  // finished
+            keep = min(keep, kg <= 0 ? ig : ig + 1 + kg * B);
+            const int k1 = kg + 1;
+            if (k1 >= 0 && k1 < ns) hi = max(hi, min(n, ig + 1 + (k1 + 1) * B));
+          }
+          keep = max(keep, wlo);
+          if (is_io) {
+            io_evict(max(wlo, t0 + nvalid), keep, io_tid, io_nt);  // columns < t0+nvalid are finished
+            io_load(whi, hi, io_tid, io_nt);
+          }
+          wlo = keep; whi = hi;
         }
-        keep = max(keep, wlo);
-        if (is_io) {
-          io_evict(max(wlo, t0 + nvalid), keep, io_tid, io_nt);  // columns < t0+nvalid are finished
-          io_load(whi, hi, io_tid, io_nt);
-        }
-        wlo = keep; whi = hi;
+        if (!finished && s >= 2 * team) do_step();
+        __syncthreads();
       }
-      if (!finished && s >= 2 * team) {
-        // -------------------------------------------------------------------- one step of sweep i
-        if (k == 0) {
-          L = min(B, n - 1 - i);
-          const cplx *ci = ring + (size_t)slot_of(i) * LD;
-          cplx x = l < L ? ci[1 + l] : cmake(0.0, 0.0);
-          double beta;
-          group_larfg<B>(x, L, l, tau, beta);
-          v = x;
-          if (tt == 0) { eg[i] = beta; dg[i] = ci[0].x; }
-          if (q == 0) vs[l] = v;
-          team_bar();
-        }
-        const int sJ = slot_of(J);
-        // element offsets of the ring columns this thread touches: its quarter (J + q QN + jj) and column J + l
-        int cb[QN];
-#pragma unroll
-        for (int jj = 0; jj < QN; ++jj) {
-          int sl = sJ + q * QN + jj;
-          if (sl >= Wc) sl -= Wc;
-          cb[jj] = sl * LD;
-        }
-        int mycb = sJ + l;
-        if (mycb >= Wc) mycb -= Wc;
-        mycb *= LD;
-        const int cb0 = sJ * LD;
-        const bool t_on = (tau.x != 0.0 || tau.y != 0.0);
-        const int Jn = J + L, L2 = min(B, n - Jn);
-        // P1: partial p = D v over this thread's quarter of the columns; P4: partial u = C v
-        // (branch-free: every index is a valid ring address, invalid contributions are masked through v)
-        cplx acc = cmake(0.0, 0.0), uacc = cmake(0.0, 0.0);
-        if (t_on) {
-#pragma unroll
-          for (int jj = 0; jj < QN; ++jj) {
-            const int c = q * QN + jj;
-            cplx vc = vs[c];
-            vc.x = c < L ? vc.x : 0.0;
-            vc.y = c < L ? vc.y : 0.0;
-            cplx a = ring[l >= c ? cb[jj] + l - c : mycb + c - l];  // lower part as stored, upper part mirrored
-            a.y = l > c ? a.y : (l == c ? 0.0 : -a.y);
-            cfma(acc, a, vc);
-            cfma(uacc, ring[cb[jj] + L + l - c], vc);
-          }
-          acc.x = l < L ? acc.x : 0.0;
-          acc.y = l < L ? acc.y : 0.0;
-          uacc.x = l < L2 ? uacc.x : 0.0;
-          uacc.y = l < L2 ? uacc.y : 0.0;
-        }
-        red1[q * B + l] = acc;
-        red2[q * B + l] = uacc;
-        team_bar();  // BAR1
-        cplx p = qsum(red1);
-        p = cmul(tau, p);
-        const double sr = group_sum<B>(l < L ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
-        const double si = group_sum<B>(l < L ? p.x * v.y - p.y * v.x : 0.0);
-        const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
-        cplx w = p;
-        cfma(w, alpha, v);
-        const cplx u = qsum(red2);
-        const cplx tu = cmul(tau, u);
-        // P5: first column of C after the right-apply, and the reflector that annihilates it
-        cplx tau2 = cmake(0.0, 0.0), v2 = cmake(0.0, 0.0);
-        if (L2 > 0) {
-          cplx *c0p = ring + cb0 + L;
-          cplx x = cmake(0.0, 0.0);
-          if (l < L2) x = csub(c0p[l], tu);  // conj(v[0]) = 1
-          if (L2 > 1) {
-            double beta2;
-            group_larfg<B>(x, L2, l, tau2, beta2);
-            v2 = x;
-            if (q == 0 && l < L2) c0p[l] = (l == 0) ? cmake(beta2, 0.0) : cmake(0.0, 0.0);
-          } else {
-            if (tt == 0) c0p[0] = x;
-            v2 = (l == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
-          }
-        }
-        if (q == 0) { ws[l] = w; tus[l] = tu; v2s[l] = v2; }
-        team_bar();  // BAR2
-        // P3: D <- D - v w^H - w v^H on the lower triangle (all loads first, then all stores: no false dependences)
-        if (t_on) {
-          cplx av[QN];
-#pragma unroll
-          for (int jj = 0; jj < QN; ++jj) {
-            const int c = q * QN + jj;
-            av[jj] = ring[cb[jj] + max(l - c, 0)];
-          }
-#pragma unroll
-          for (int jj = 0; jj < QN; ++jj) {
-            const int c = q * QN + jj;
-            cplx a = av[jj];
-            cfms(a, v, cconj(ws[c]));
-            cfms(a, w, cconj(vs[c]));
-            a.y = l == c ? 0.0 : a.y;
-            av[jj] = a;
-          }
-#pragma unroll
-          for (int jj = 0; jj < QN; ++jj) {
-            const int c = q * QN + jj;
-            if (c <= l && l < L) ring[cb[jj] + (l - c)] = av[jj];
-          }
-        }
-        if (L2 <= 0) {
-          finished = true;
-        } else {
-          const bool t2_on = (tau2.x != 0.0 || tau2.y != 0.0);
-          if (t_on || t2_on) {
-            // P6/P7: thread = column c = l of C (1 <= c < L), rows of its quarter:
-            //   t = C - (tau C v) v^H ; z = v2^H t ; C = t - v2 conj(tau2) z
-            const bool mine = l >= 1 && l < L;
-            const cplx vcj = cconj(v);
-            cplx *pc = ring + (mine ? mycb + L - l : cb0 + L);
-            cplx tv[QN];
-            cplx zacc = cmake(0.0, 0.0);
-#pragma unroll
-            for (int jj = 0; jj < QN; ++jj) {
-              const int r = q * QN + jj;
-              cplx t = pc[r];
-              cplx tur = tus[r], v2r = v2s[r];
-              v2r.x = r < L2 ? v2r.x : 0.0;  // rows beyond the block do not contribute
-              v2r.y = r < L2 ? v2r.y : 0.0;
-              cfms(t, tur, vcj);
-              cfmac(zacc, v2r, t);
-              tv[jj] = t;
-            }
-            zacc.x = mine ? zacc.x : 0.0;
-            zacc.y = mine ? zacc.y : 0.0;
-            red3[q * B + l] = zacc;
-            team_bar();  // BAR3
-            const cplx zc = qsum(red3);
-            const cplx f = cmul(cconj(tau2), zc);
-#pragma unroll
-            for (int jj = 0; jj < QN; ++jj) {
-              const int r = q * QN + jj;
-              cplx t = tv[jj];
-              cfms(t, v2s[r], f);
-              if (mine && r < L2) pc[r] = t;
-            }
-          }
-          if (q == 0) vs[l] = v2;  // after BAR3 (or with P3 skipped): nobody still reads the old v
-          v = v2; tau = tau2; J = Jn; L = L2; ++k;
-        }
-      }
-      __syncthreads();
     }
   }
   // last diagonal entry
@@ -340,7 +375,7 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
   const size_t team_bytes = (size_t)(4 + 3 * NQ) * B * sizeof(cplx);
   const size_t max_smem = 226 * 1024;
   int G, Wc;
-  if ((size_t)n * colbytes + gmax * team_bytes <= max_smem) {  // whole band resident
+  if ((size_t)n * colbytes + gmax * team_bytes + (size_t)n * sizeof(int) <= max_smem) {  // whole band resident
     Wc = n;
     G = max(1, min(gmax, (n + 2 * B - 1) / (2 * B)));
   } else {
@@ -354,7 +389,7 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
     Wc = 2 * G * B + 8;
     if (Wc >= n) Wc = n;
   }
-  const size_t smem = (size_t)Wc * colbytes + G * team_bytes;
+  const size_t smem = (size_t)Wc * colbytes + G * team_bytes + (Wc >= n ? (size_t)n * sizeof(int) : 0);
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(bulge_kernel<B, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);

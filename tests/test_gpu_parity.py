@@ -192,3 +192,42 @@ def test_config4_batch_parity_sampled(bs):
             check_bands(lam[ci, i:i + 1], lr[None, :], np.array([lmax]), f"C4 cell{ci} k{i}")
     for c in cells:
         bs.bs_destroy_cell(c)
+
+
+def test_config5_bands_parity_sampled(bs):
+    # full size of config 5 (n = 1922, 120 k-points in one call, as bench.py launches it); oracle on sampled k-points
+    w = wl.get("C5")
+    cell = w.cells[0]
+    h = make_cell(bs, cell, w.Mt, w.nk)
+    bs.bs_assemble(h, w.Mt)
+    lam = bs.bs_bands(h, w.kpts, w.nbands)
+    assert lam.shape == (w.nk, w.nbands) and np.all(np.diff(lam, axis=1) >= 0)
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), w.Mt)
+    Phi, Psi = bs.bs_get_matrices(h)
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+    assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    needed_backward_clause = 0
+    for i in [0, 1, 67]:
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, w.Mt, w.kpts[i], w.nbands)
+        needed_backward_clause += check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"C5 k{i}")
+    assert needed_backward_clause <= 4      # the two zero modes at Gamma and the acoustic pair next to it (R8)
+    bs.bs_destroy_cell(h)
+
+
+def test_config4_full_batch_sampled(bs):
+    # the whole optimisation-loop batch (256 cells x 40 k-points = 10240 eigenproblems in one call)
+    w = wl.get("C4")
+    cells = [make_cell(bs, c, w.Mt, w.nk) for c in w.cells]
+    bs.bs_assemble_batch(cells, w.Mt)
+    lam = bs.bs_bands_batch(cells, w.kpts, w.nbands)
+    assert lam.shape == (256, w.nk, w.nbands) and np.all(np.isfinite(lam))
+    for ci in [0, 131, 255]:
+        Pr, Sr = oracle.assemble(*oracle_inputs(w.cells[ci]), w.Mt)
+        for i in [0, 17, 39]:
+            lr, lmax = oracle.bands_at_k(Pr, Sr, w.cells[ci].lattice, w.Mt, w.kpts[i], w.nbands)
+            check_bands(lam[ci, i:i + 1], lr[None, :], np.array([lmax]), f"C4 cell{ci} k{i}")
+    # a batch call equals the single-cell calls bit for bit (same kernels, same order of operations)
+    one = bs.bs_bands(cells[131], w.kpts, w.nbands)
+    assert np.array_equal(one, lam[131])
+    for c in cells:
+        bs.bs_destroy_cell(c)

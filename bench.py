@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — k-points/s of the whole hot path (bs_assemble + bs_bands over every k-point of one workload).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
 
 A "step" is one pass of the whole path (S1..S8 of DESIGN.md) over one workload: assembly of Phi/Psi and their
 factors, then the lowest `nbands` eigenvalues at every k-point.  `value` = k-points per second with the inputs already
@@ -325,7 +325,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C3", choices=list(wl.CONFIGS))
+    ap.add_argument("--workload", default="C5", choices=list(wl.CONFIGS))
     ap.add_argument("--cells", type=int, default=256, help="number of cells of workload C4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

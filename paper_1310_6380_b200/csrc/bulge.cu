@@ -3,16 +3,15 @@
 //
 // One CTA per matrix.  Sweep i annihilates column i below the sub-diagonal and chases the bulge down the band in steps
 // of B columns; step k of sweep i touches columns [i+1+kB, i+1+(k+1)B) only, so sweep i+1 can run two steps behind sweep i.
-// A "train" of G consecutive sweeps is executed by G warps in lock step (warp g does step s-2g at macro-step s) on a
-// window of the band held in shared memory as a ring of Wc columns; NIO further warps write the columns the train has
-// left behind back to global memory and fetch the ones the leading sweep needs next, concurrently with the arithmetic.
-// When the whole band fits the ring (small n) it is loaded once and never written back (only d, e are outputs).
+// A "train" of G consecutive sweeps is executed by G teams of NQ*B threads in lock step (team g does step s-2g at
+// macro-step s) on a window of the band held in shared memory as a ring of Wc columns; NIO further warps write the
+// columns the train has left behind back to global memory and fetch the ones the leading sweep needs next, concurrently
+// with the arithmetic.  When the whole band fits the ring (small n) it is loaded once, never written back (only d, e
+// are outputs), and the teams run one continuous pipeline over all sweeps instead of trains.
 //
 // Element (r, c), c <= r <= c + 2B - 1, lives at ring[(c mod Wc) * LD + (r - c)].  With LD = 2B the two access patterns
 // used (fixed column, lanes over rows: stride 1; fixed row, lanes over columns: stride LD - 1, odd) are both free of
 // shared-memory bank conflicts for 16-byte elements.
-#include <cstdlib>
-
 #include "bs_internal.cuh"
 
 namespace bsk {
@@ -383,12 +382,6 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
     G = max(1, min(G, gmax));
     Wc = 2 * G * B + 8;
   }
-  static const int g_env = getenv("BS_BULGE_G") ? atoi(getenv("BS_BULGE_G")) : 0;  // experiment knob
-  if (g_env > 0) {
-    G = min(g_env, gmax);
-    Wc = 2 * G * B + 8;
-    if (Wc >= n) Wc = n;
-  }
   const size_t smem = (size_t)Wc * colbytes + G * team_bytes + (Wc >= n ? (size_t)n * sizeof(int) : 0);
   static bool attr_done = false;
   if (!attr_done) {
@@ -404,9 +397,8 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
 // Band -> tridiagonal for every matrix of the batch.  b must be 8, 16 or 32.
 void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s) {
   const int nmat = ncells * inner;
-  static const int nq_env = getenv("BS_BULGE_NQ") ? atoi(getenv("BS_BULGE_NQ")) : 0;
   if (b == 8) launch_bulge_t<8, 4>(n, AB, d, e, nmat, inner, s);
-  else if (b == 16) { if (nq_env == 8) launch_bulge_t<16, 8>(n, AB, d, e, nmat, inner, s); else launch_bulge_t<16, 4>(n, AB, d, e, nmat, inner, s); }
+  else if (b == 16) launch_bulge_t<16, 4>(n, AB, d, e, nmat, inner, s);
   else launch_bulge_t<32, 4>(n, AB, d, e, nmat, inner, s);
 }
 

@@ -17,8 +17,7 @@ constexpr int ROUNDS = 24;   // 9^24 > 2^76
 // would serialise the recurrence: p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2}, a sign change between p_{i-1} and p_i
 // is a negative pivot.  The pair (p_{i-1}, p_i) is rescaled by a power of two whenever its exponent leaves [2^-400, 2^400]
 // (this does not change the ratio), so nothing overflows or underflows.
-__device__ __forceinline__ int sturm_count(const double *__restrict__ d, const double *__restrict__ e2, int n, double x,
-                                           double pivmin) {
+__device__ __forceinline__ int sturm_count(const double *__restrict__ d, const double *__restrict__ e2, int n, double x) {
   double p0 = 1.0, p1 = d[0] - x;
   if (p1 == 0.0) p1 = -0x1p-200;  // zero pivot -> tiny negative pivot (relative 2^-200: far below rounding)
   int cnt = p1 < 0.0;
@@ -40,7 +39,7 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
                                                    int nev, double *__restrict__ lam) {
   extern __shared__ double sm[];
   double *d = sm, *e2 = sm + n;
-  __shared__ double s_lo, s_hi, s_emax;
+  __shared__ double s_lo, s_hi;
   __shared__ int cnts[ST];
   const int z = blockIdx.x, t = threadIdx.x;
   dg += (size_t)z * n;
@@ -51,20 +50,18 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
   }
   __syncthreads();
   if (t == 0) {  // Gershgorin bounds (n <= 2048: serial is fine next to the bisection itself)
-    double lo = d[0], hi = d[0], emax = 0.0;
+    double lo = d[0], hi = d[0];
     for (int i = 0; i < n; ++i) {
       const double l = i > 0 ? sqrt(e2[i - 1]) : 0.0, r = i + 1 < n ? sqrt(e2[i]) : 0.0;
       lo = fmin(lo, d[i] - l - r);
       hi = fmax(hi, d[i] + l + r);
-      emax = fmax(emax, e2[i]);
     }
     const double nrm = fmax(fabs(lo), fabs(hi));
     lo -= 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
     hi += 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
-    s_lo = lo; s_hi = hi; s_emax = emax;
+    s_lo = lo; s_hi = hi;
   }
   __syncthreads();
-  const double pivmin = fmax(2.3e-308 * fmax(1.0, s_emax), 2.3e-308);
   const int grp = t / G, sub = t % G;
   for (int k0 = 0; k0 < nev; k0 += EPB) {
     const int k = k0 + grp;  // eigenvalue index of this group
@@ -73,7 +70,7 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
       const double w = hi - lo;
       const double x = lo + w * ((double)(sub + 1) / (double)(G + 1));
       int c = 0;
-      if (k < nev) c = sturm_count(d, e2, n, x, pivmin);
+      if (k < nev) c = sturm_count(d, e2, n, x);
       cnts[t] = c;
       __syncthreads();
       // new interval: [x_{m-1}, x_m] with m the first sub-shift whose count >= k+1  (x_{-1} = lo, x_G = hi)

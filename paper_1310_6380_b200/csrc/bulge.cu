@@ -190,30 +190,46 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
     red1[q * B + l] = acc;
     red2[q * B + l] = uacc;
     team_bar();  // BAR1
-    cplx p = qsum(red1);
-    p = cmul(tau, p);
-    const double sr = group_sum<B>(l < L ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
-    const double si = group_sum<B>(l < L ? p.x * v.y - p.y * v.x : 0.0);
+    // P2 (w from p) and P5 (first column of C after the right-apply and the reflector that annihilates it) as one
+    // straight-line block: the three lane reductions and the sqrt / divisions of the two chains overlap
+    cplx p = cmul(tau, qsum(red1));
+    const cplx u = qsum(red2);
+    const cplx tu = cmul(tau, u);
+    cplx x = csub(ring[cb0 + L + l], tu);  // conj(v[0]) = 1; always a valid ring address
+    x.x = l < L2 ? x.x : 0.0;
+    x.y = l < L2 ? x.y : 0.0;
+    double sr = l < L ? p.x * v.x + p.y * v.y : 0.0;  // p^H v
+    double si = l < L ? p.x * v.y - p.y * v.x : 0.0;
+    double ss = l >= 1 ? x.x * x.x + x.y * x.y : 0.0;
+#pragma unroll
+    for (int o = B / 2; o > 0; o >>= 1) {
+      sr += __shfl_xor_sync(0xffffffffu, sr, o);
+      si += __shfl_xor_sync(0xffffffffu, si, o);
+      ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    }
     const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
     cplx w = p;
     cfma(w, alpha, v);
-    const cplx u = qsum(red2);
-    const cplx tu = cmul(tau, u);
-    // P5: first column of C after the right-apply, and the reflector that annihilates it
-    cplx tau2 = cmake(0.0, 0.0), v2 = cmake(0.0, 0.0);
-    if (L2 > 0) {
-      cplx *c0p = ring + cb0 + L;
-      cplx x = cmake(0.0, 0.0);
-      if (l < L2) x = csub(c0p[l], tu);  // conj(v[0]) = 1
-      if (L2 > 1) {
-        double beta2;
-        group_larfg<B>(x, L2, l, tau2, beta2);
-        v2 = x;
-        if (q == 0 && l < L2) c0p[l] = (l == 0) ? cmake(beta2, 0.0) : cmake(0.0, 0.0);
-      } else {
-        if (tt == 0) c0p[0] = x;
-        v2 = (l == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
-      }
+    // zlarfg, branch-free: no reflector when the block has a single row (L2 <= 1) or the column is already e_1-shaped
+    const cplx al = shfl_c(x, (threadIdx.x & 31) & ~(B - 1));
+    const bool norefl = L2 <= 1, trivial = norefl || (ss == 0.0 && al.y == 0.0);
+    const double nrm = sqrt(al.x * al.x + al.y * al.y + ss);
+    const double beta2 = trivial ? 1.0 : -copysign(nrm, al.x);
+    const double ib = 1.0 / beta2;
+    cplx tau2 = cmake((beta2 - al.x) * ib, -al.y * ib);
+    tau2.x = trivial ? 0.0 : tau2.x;
+    tau2.y = trivial ? 0.0 : tau2.y;
+    const double dr = al.x - beta2, di = al.y;
+    const double den = 1.0 / (dr * dr + di * di);
+    cplx scale = cmake(dr * den, -di * den);
+    scale.x = trivial ? 0.0 : scale.x;
+    scale.y = trivial ? 0.0 : scale.y;
+    cplx v2 = cmul(x, scale);
+    v2.x = l == 0 ? 1.0 : v2.x;
+    v2.y = l == 0 ? 0.0 : v2.y;
+    if (q == 0 && l < L2) {
+      cplx c00 = norefl ? x : cmake(trivial ? al.x : beta2, 0.0);
+      ring[cb0 + L + l] = (l == 0) ? c00 : cmake(0.0, 0.0);
     }
     if (q == 0) { ws[l] = w; tus[l] = tu; v2s[l] = v2; }
     team_bar();  // BAR2

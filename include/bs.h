@@ -50,6 +50,11 @@ enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
  * chasing; default), 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check). */
 enum { BS_OPT_TRIDIAG = 3 };
 enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1 };
+/* BS_OPT_ASSEMBLY (option 4): quadrature of the shape integrals in S1.  0 = exact closed-form polygon integral (default),
+ * 1 = the paper's centroid rule I_p(q) ~ A_p exp(i q.c_p) (PAPER.md:106 eq. 12, :213 eq. 22; c_p = area centroid), kept as the
+ * paper-faithful variant: its matrices converge to the exact ones as the mesh is refined. */
+enum { BS_OPT_ASSEMBLY = 4 };
+enum { BS_ASSEMBLY_EXACT = 0, BS_ASSEMBLY_CENTROID = 1 };
 
 /* Stage indices of bs_get_timings (milliseconds, CUDA events on the call's stream). */
 enum {

@@ -9,6 +9,8 @@ from .bandstructure import (  # noqa: F401
     plane_wave_indices,
     shape_integral,
     polygon_area,
+    polygon_centroid,
+    shape_integral_centroid,
     isotropic_plane_strain_compliance,
     lame_from_C11_C44,
     voigt_compliance,

@@ -74,6 +74,23 @@ def shape_integral(poly, q):
     return complex(-1j * s / q2)
 
 
+def polygon_centroid(poly):
+    """Area centroid of a simple polygon (textbook shoelace form)."""
+    p = np.asarray(poly, dtype=np.float64)
+    x, y = p[:, 0], p[:, 1]
+    xn, yn = np.roll(x, -1), np.roll(y, -1)
+    cr = x * yn - xn * y
+    A = 0.5 * np.sum(cr)
+    return np.array([np.sum((x + xn) * cr), np.sum((y + yn) * cr)]) / (6.0 * A)
+
+
+def shape_integral_centroid(poly, q):
+    """PAPER.md:106 (eq. 12) / :213 (eq. 22): the paper's one-point rule int_{Omega_p} F ~ F(c_p) V_p with
+    F = exp(i q.x): I_p(q) ~ A_p exp(i q.c_p).  (The leading term of ``shape_integral``; reading R6.)"""
+    q = np.asarray(q, dtype=np.float64)
+    return complex(polygon_area(poly) * np.exp(1j * (polygon_centroid(poly) @ q)))
+
+
 # --------------------------------------------------------------------------- property fields
 def isotropic_plane_strain_compliance(E, nu):
     """PAPER.md:121 (eq. 14): D_jkmn = (1/2mu)[ (d_jm d_kn + d_jn d_km)/2 - lam/(2(mu+lam)) d_jk d_mn ].
@@ -143,11 +160,12 @@ def assemble_direct(lattice, vert_offset, verts, compliance, density, Mt):
     return Phi, Psi
 
 
-def shape_integral_table(lattice, vert_offset, verts, weights, Mt):
+def shape_integral_table(lattice, vert_offset, verts, weights, Mt, quadrature="exact"):
     """T_c(D) = sum_p weights[c,p] I_p(D1 q^1 + D2 q^2) for every index difference
     D in [-2Mt,2Mt]^2 (reading R1: G_beta - G_alpha depends only on beta - alpha, so the
     N^2 entries of a block take (4Mt+1)^2 distinct values).  Vectorised over edges; the
     formula is ``shape_integral``'s, pinned to it and to ``assemble_direct`` in the tests.
+    ``quadrature="centroid"`` uses the paper's one-point rule per polygon (``shape_integral_centroid``) instead.
     Returns complex (C, 4Mt+1, 4Mt+1), index [c, D1+2Mt, D2+2Mt]."""
     _, Q, _ = reciprocal_basis(lattice)
     verts = np.asarray(verts, dtype=np.float64).reshape(-1, 2)
@@ -164,6 +182,10 @@ def shape_integral_table(lattice, vert_offset, verts, weights, Mt):
         nxt[s:t] = np.roll(verts[s:t], -1, axis=0)
         phase_of_edge[s:t] = p
         area[p] = polygon_area(verts[s:t])
+    if quadrature == "centroid":
+        cent = np.array([polygon_centroid(verts[off[p]:off[p + 1]]) for p in range(P)])
+    elif quadrature != "exact":
+        raise ValueError(quadrature)
     e = nxt - start
     m = 0.5 * (nxt + start)
     we = w[:, phase_of_edge]                       # (C, nedge)
@@ -175,6 +197,9 @@ def shape_integral_table(lattice, vert_offset, verts, weights, Mt):
                 out[:, i1, i2] = w @ area
                 continue
             q = D1 * Q[0] + D2 * Q[1]
+            if quadrature == "centroid":
+                out[:, i1, i2] = w @ (area * np.exp(1j * (cent @ q)))
+                continue
             q2 = float(q @ q)
             cross = q[0] * e[:, 1] - q[1] * e[:, 0]
             term = cross * np.exp(1j * (m @ q)) * _j0(0.5 * (e @ q))
@@ -182,7 +207,7 @@ def shape_integral_table(lattice, vert_offset, verts, weights, Mt):
     return out
 
 
-def assemble(lattice, vert_offset, verts, compliance, density, Mt):
+def assemble(lattice, vert_offset, verts, compliance, density, Mt, quadrature="exact"):
     """Phi (3N x 3N) and Psi (2N x 2N) through the index-difference table (same numbers as
     ``assemble_direct`` up to rounding; that equality is a test).  PAPER.md:150-171."""
     Dv = voigt_compliance(compliance)
@@ -190,7 +215,7 @@ def assemble(lattice, vert_offset, verts, compliance, density, Mt):
     # channels: 6 distinct entries of the symmetric 3x3 weight block, then rho
     pairs = [(0, 0), (1, 1), (0, 1), (0, 2), (1, 2), (2, 2)]
     W = np.stack([Dv[:, a, b] for a, b in pairs] + [rho], axis=0)
-    tab = shape_integral_table(lattice, vert_offset, verts, W, Mt)
+    tab = shape_integral_table(lattice, vert_offset, verts, W, Mt, quadrature)
     idx = plane_wave_indices(Mt)
     N = idx.shape[0]
     d1 = idx[None, :, 0] - idx[:, None, 0] + 2 * Mt       # [alpha, beta] -> beta - alpha

@@ -18,6 +18,8 @@ LIB_PATH = os.path.join(_PKG, "libbs.so")
 BS_OK, BS_ERR_ARG, BS_ERR_GEOMETRY, BS_ERR_NOT_PD, BS_ERR_STATE, BS_ERR_CUDA, BS_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
 BS_OPT_PENCIL_MODE, BS_OPT_PANEL, BS_OPT_TIMING, BS_OPT_TRIDIAG = 0, 1, 2, 3
 BS_TRIDIAG_TWO_STAGE, BS_TRIDIAG_ONE_STAGE = 0, 1
+BS_OPT_ASSEMBLY = 4
+BS_ASSEMBLY_EXACT, BS_ASSEMBLY_CENTROID = 0, 1
 BS_PENCIL_POLY, BS_PENCIL_DIRECT = 0, 1
 BS_T_TABLE, BS_T_EXPAND, BS_T_FACTOR, BS_T_COEF, BS_T_PENCIL, BS_T_TRIDIAG, BS_T_BISECT, BS_T_COUNT = 0, 1, 2, 3, 4, 5, 6, 8
 BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_KHI_COL, BS_GEMM_A_HERM_LOWER = 1, 2, 4, 8, 16, 32

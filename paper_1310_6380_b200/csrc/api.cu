@@ -91,7 +91,7 @@ struct bs_cell {
   int *d_ephase = nullptr;
   bsk::Geometry geo;
   bsk::Geometry *d_geo = nullptr;  // [1]
-  int mode = BS_PENCIL_POLY, nb = 32, timing = 0, algo = BS_TRIDIAG_TWO_STAGE;
+  int mode = BS_PENCIL_POLY, nb = 32, timing = 0, algo = BS_TRIDIAG_TWO_STAGE, quad = BS_ASSEMBLY_EXACT;
   void *ws = nullptr;
   size_t ws_bytes = 0;
   Layout lay;            // layout of the last bs_assemble (lay.Mt < 0: not assembled)
@@ -222,16 +222,18 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
   c->P = nphase;
   const int ne = vert_offset[nphase];
   c->nedge = ne;
-  std::vector<double> edge((size_t)6 * ne), area(nphase), w((size_t)7 * nphase);
+  std::vector<double> edge((size_t)6 * ne), area((size_t)3 * nphase), w((size_t)7 * nphase);  // area: [area | ch1 | ch2]
   std::vector<int> eph(ne);
   double total = 0.0;
   for (int p = 0; p < nphase; ++p) {
     const int s = vert_offset[p], t = vert_offset[p + 1];
-    double a2 = 0.0;
+    double a2 = 0.0, cxs = 0.0, cys = 0.0;
     for (int i = s; i < t; ++i) {
       const int k = (i + 1 < t) ? i + 1 : s;
       const double x0 = verts[2 * i], y0 = verts[2 * i + 1], x1 = verts[2 * k], y1 = verts[2 * k + 1];
       a2 += x0 * y1 - x1 * y0;
+      cxs += (x0 + x1) * (x0 * y1 - x1 * y0);
+      cys += (y0 + y1) * (x0 * y1 - x1 * y0);
       const double ex = x1 - x0, ey = y1 - y0, mx = 0.5 * (x0 + x1), my = 0.5 * (y0 + y1);
       // fractional coordinates H = x T  (x = H_1 h^1 + H_2 h^2)
       edge[0 * (size_t)ne + i] = mx * c->T[0] + my * c->T[2];
@@ -248,6 +250,11 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
       return fail(BS_ERR_GEOMETRY, "bs_create_cell: phase %d has non-positive signed area %g (must be CCW)", p, area[p]);
     }
     total += area[p];
+    {  // area centroid (used by the centroid-rule assembly mode, eq. 12), in fractional coordinates
+      const double cx = cxs / (3.0 * a2), cy = cys / (3.0 * a2);
+      area[(size_t)nphase + p] = cx * c->T[0] + cy * c->T[2];
+      area[(size_t)2 * nphase + p] = cx * c->T[1] + cy * c->T[3];
+    }
     if (!(density[p] > 0.0)) {
       delete c;
       return fail(BS_ERR_ARG, "bs_create_cell: phase %d has density <= 0", p);
@@ -314,6 +321,11 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
     case BS_OPT_TRIDIAG:
       if (value != BS_TRIDIAG_TWO_STAGE && value != BS_TRIDIAG_ONE_STAGE) return fail(BS_ERR_ARG, "bs_set_option: bad S6 algorithm");
       c->algo = value;
+      return BS_OK;
+    case BS_OPT_ASSEMBLY:
+      if (value != BS_ASSEMBLY_EXACT && value != BS_ASSEMBLY_CENTROID) return fail(BS_ERR_ARG, "bs_set_option: bad assembly mode");
+      if (c->quad != value) c->assembled = false;
+      c->quad = value;
       return BS_OK;
     case BS_OPT_TIMING:
       if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
@@ -442,7 +454,7 @@ bs_status check_batch(bs_cell *const *cells, int ncells, const char *who) {
   for (int c = 0; c < ncells; ++c) {
     if (!cells[c]) return fail(BS_ERR_ARG, "%s: cells[%d] is null", who, c);
     if (!cells[c]->ws) return fail(BS_ERR_NOMEM, "%s: cells[%d] has no workspace (bs_set_workspace)", who, c);
-    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb || cells[c]->algo != cells[0]->algo)
+    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb || cells[c]->algo != cells[0]->algo || cells[c]->quad != cells[0]->quad)
       return fail(BS_ERR_ARG, "%s: cells[%d] has different options than cells[0]", who, c);
   }
   return BS_OK;
@@ -477,7 +489,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   tick(lead, 0, s);
   double total_edges = 0.0;
   for (int c = 0; c < ncells; ++c) total_edges += cells[c]->nedge;
-  bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, s); ++nl;  // S1
+  bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s); ++nl;  // S1
   tick(lead, 1, s);
   bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2
   tick(lead, 2, s);

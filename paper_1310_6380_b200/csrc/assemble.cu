@@ -12,7 +12,7 @@ static constexpr double kPi = 3.14159265358979323846264338327950288;
 //   T_c(D) = (-i/|q|^2) sum_edges w_c[phase(e)] (q x e) exp(i q.m_e) j0(q.e/2),   q = D1 q^1 + D2 q^2,
 // and T_c(0) = sum_p w_c[p] area_p.  The phase q.m and the argument of j0 are evaluated in FRACTIONAL coordinates
 // (q.x = 2 pi (D1 H1 + D2 H2) with integer D), so sincospi/sinpi reduce the argument exactly.
-__global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table) {
+__global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table, int centroid_rule) {
   __shared__ double part[8][14];
   const int cell = blockIdx.y;
   const Geometry g = geos[cell];
@@ -33,6 +33,21 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
       const double a = g.area[p];
 #pragma unroll
       for (int c = 0; c < 7; ++c) accr[c] = fma(g.w[c * g.P + p], a, accr[c]);
+    }
+  } else if (centroid_rule) {
+    // PAPER.md:106 (eq. 12) / :213 (eq. 22): I_p(q) ~ A_p exp(i q.c_p), the paper's one-point rule per mesh element
+    for (int p = threadIdx.x; p < g.P; p += 256) {
+      const double phi = fma((double)D1, g.area[g.P + p], (double)D2 * g.area[2 * g.P + p]);  // q.c / (2 pi)
+      double sn, cs;
+      sincospi(2.0 * phi, &sn, &cs);
+      const double a = g.area[p];
+      const double tr = a * cs, ti = a * sn;
+#pragma unroll
+      for (int c = 0; c < 7; ++c) {
+        const double w = g.w[c * g.P + p];
+        accr[c] = fma(w, tr, accr[c]);
+        acci[c] = fma(w, ti, acci[c]);
+      }
     }
   } else {
     const double qx = D1 * g.Q[0] + D2 * g.Q[2];
@@ -76,6 +91,9 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
     for (int w = 0; w < 8; ++w) { sr += part[w][2 * c]; si += part[w][2 * c + 1]; }
     if (D1 == 0 && D2 == 0) {
       T[(size_t)c * L2 + flat] = cmake(sr, 0.0);
+    } else if (centroid_rule) {
+      T[(size_t)c * L2 + flat] = cmake(sr, si);
+      T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(sr, -si);
     } else {
       const double qx = D1 * g.Q[0] + D2 * g.Q[2];
       const double qy = D1 * g.Q[1] + D2 * g.Q[3];
@@ -88,14 +106,15 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
   }
 }
 
-void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, cudaStream_t s) {
+void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
+                  cudaStream_t s) {
   const int L = 4 * Mt + 1;
   const int nhalf = (L * L + 1) / 2;
   dim3 grid(nhalf, ncells);
   // algorithmic work: ~230 real flops per (index difference, edge) term: sincospi + sinpi + the 7-channel accumulation,
   // counted from the SASS of the loop body (about 95 DFMA, 25 DMUL, 15 DADD)
   KScope ks(KC_TABLE, 230.0 * total_edges * nhalf, s);
-  table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table);
+  table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table, centroid_rule);
 }
 
 // S2: one thread per (g_alpha, g_beta): Phi[(a,ga),(b,gb)] = T_{c(a,b)}(D(gb) - D(ga)), R[ga,gb] = T_rho(...).

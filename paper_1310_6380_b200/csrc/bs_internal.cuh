@@ -114,13 +114,14 @@ struct Geometry {  // device pointers, per cell
   const double *edge;   // SoA [6][nedge]: mh1, mh2 (fractional midpoint), eh1, eh2 (fractional edge), ex, ey (Cartesian edge)
   const int *ephase;    // [nedge] phase of each edge
   const double *w;      // [7][P] channel weights: Dv11 Dv22 Dv12 Dv13 Dv23 Dv33 rho
-  const double *area;   // [P]
+  const double *area;   // [3][P]: signed area, fractional centroid (ch1, ch2)
   int nedge, P;
   double Q[4];          // rows q^1, q^2 (Cartesian)
 };
 
 // S1: table[c][(D1+2Mt)*(4Mt+1) + (D2+2Mt)], c < 7.  geo: device array [ncells]; table at BatchRef (inner unused).
-void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, cudaStream_t s);
+void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
+                  cudaStream_t s);
 // S2: Phi (3N x 3N full) and R (N x N full) from the table.
 void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s);
 

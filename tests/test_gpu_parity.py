@@ -231,3 +231,25 @@ def test_config4_full_batch_sampled(bs):
     assert np.array_equal(one, lam[131])
     for c in cells:
         bs.bs_destroy_cell(c)
+
+
+def test_centroid_rule_assembly_parity(bs):
+    # BS_OPT_ASSEMBLY = centroid (eq. 12): matrices and bands against the oracle's centroid-rule assembly
+    w = wl.get("C3")
+    cell = w.cells[0]
+    Mt = 4
+    h = make_cell(bs, cell, Mt, 3)
+    bs.bs_set_option(h, bs.BS_OPT_ASSEMBLY, bs.BS_ASSEMBLY_CENTROID)
+    bs.bs_assemble(h, Mt)
+    Phi, Psi = bs.bs_get_matrices(h)
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), Mt, quadrature="centroid")
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+    assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    Pe, _ = oracle.assemble(*oracle_inputs(cell), Mt)
+    assert 1e-6 < np.max(np.abs(Pr - Pe)) / np.max(np.abs(Pe)) < 0.2     # a different (coarser) quadrature, same limit
+    kp = np.array([[0.2, 0.1], [0.5, 0.0], [0.0, 0.0]])
+    lam = bs.bs_bands(h, kp, 12)
+    for i, kr in enumerate(kp):
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, Mt, kr, 12)
+        check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"centroid k{i}")
+    bs.bs_destroy_cell(h)

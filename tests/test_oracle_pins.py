@@ -309,3 +309,30 @@ def test_paper_stopbands_steel_epoxy_hexagonal():
     assert len(gaps) == 2, gaps
     for (lo, hi), (glo, ghi) in zip(gaps, gold):
         assert abs(lo - glo) < 0.02 * glo and abs(hi - ghi) < 0.02 * ghi, (gaps, gold)
+
+
+# ----------------------------------------------------------------------------- centroid rule (eq. 12)
+def test_centroid_rule_is_the_leading_term_and_converges():
+    # textbook centroids; I(0) = area; |I_exact - A e^{iq.c}| = O(|q|^2 h^2) A: refining a pixel grid by 2 cuts the
+    # error of the assembled table by ~4 (second order), and it tends to the exact table
+    assert np.allclose(oracle.polygon_centroid(np.array([[0, 0], [3, 0], [0, 3.0]])), [1, 1])
+    assert np.allclose(oracle.polygon_centroid(np.array([[1, 1], [3, 1], [3, 2], [1, 2.0]])), [2, 1.5])
+    poly = np.array([[0.1, 0.2], [0.5, 0.25], [0.3, 0.6]])
+    assert oracle.shape_integral_centroid(poly, np.zeros(2)) == pytest.approx(oracle.polygon_area(poly))
+    for scale in (1.0, 0.5):
+        q = np.array([3.0, -2.0])
+        small = poly * scale
+        err = abs(oracle.shape_integral(small, q) - oracle.shape_integral_centroid(small, q)) / oracle.polygon_area(small)
+        assert err < 0.2 * (np.linalg.norm(q) * scale * 0.5) ** 2
+    errs = []
+    for n in (8, 16, 32):
+        rho = np.array([1000.0 + 500.0 * ((i * 7 + j * 3) % 5) for i in range(4) for j in range(4)])
+        # the same 4x4 property field carried by n x n pixels
+        polys = wl.pixel_polygons(n)
+        w = np.array([[rho[(i * 4 // n) * 4 + (j * 4 // n)] for i in range(n) for j in range(n)]])
+        off, verts = wl._csr(polys)
+        ex = oracle.shape_integral_table(wl.SQUARE, off, verts, w, 1)
+        ce = oracle.shape_integral_table(wl.SQUARE, off, verts, w, 1, quadrature="centroid")
+        errs.append(np.max(np.abs(ex - ce)) / np.max(np.abs(ex)))
+    assert errs[0] > errs[1] > errs[2] and errs[2] < 2e-2
+    assert 3.5 < errs[0] / errs[1] < 4.6 and 3.8 < errs[1] / errs[2] < 4.2

@@ -55,6 +55,10 @@ enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1 };
  * paper-faithful variant: its matrices converge to the exact ones as the mesh is refined. */
 enum { BS_OPT_ASSEMBLY = 4 };
 enum { BS_ASSEMBLY_EXACT = 0, BS_ASSEMBLY_CENTROID = 1 };
+/* BS_OPT_PHI_INVERSE (option 5): 0 = automatic (default): when every phase is isotropic plane strain, Phi has the block
+ * structure [[A, B, 0], [B, A, 0], [0, 0, 2(A-B)]] and Phi^{-1} is composed from the two N x N inverses
+ * (A+B)^{-1} and (A-B)^{-1}; 1 = always factor and invert the full 3N x 3N matrix (any compliance; cross-check). */
+enum { BS_OPT_PHI_INVERSE = 5 };
 
 /* Stage indices of bs_get_timings (milliseconds, CUDA events on the call's stream). */
 enum {

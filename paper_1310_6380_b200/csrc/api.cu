@@ -87,6 +87,8 @@ Layout make_layout(int Mt, int nk, int mode, int nb) {
 struct bs_cell {
   double A[4], T[4], Q[4], V;
   int P = 0, nedge = 0;
+  bool isotropic = true;  // every phase has the isotropic plane-strain block structure of PAPER.md:173
+  int phi_general = 0;    // BS_OPT_PHI_INVERSE: 1 = always the general 3N x 3N inverse
   double *d_edge = nullptr, *d_w = nullptr, *d_area = nullptr;
   int *d_ephase = nullptr;
   bsk::Geometry geo;
@@ -261,6 +263,8 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
     }
     // Voigt weights with the factors 1/2/4 of PAPER.md:167-171 (eq. 20)
     const double *D = compliance + 6 * (size_t)p;
+    if (D[3] != 0.0 || D[4] != 0.0 || D[0] != D[1] || std::fabs(4.0 * D[5] - 2.0 * (D[0] - D[2])) > 1e-14 * std::fabs(D[0]))
+      c->isotropic = false;
     w[0 * (size_t)nphase + p] = D[0];
     w[1 * (size_t)nphase + p] = D[1];
     w[2 * (size_t)nphase + p] = D[2];
@@ -326,6 +330,11 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       if (value != BS_ASSEMBLY_EXACT && value != BS_ASSEMBLY_CENTROID) return fail(BS_ERR_ARG, "bs_set_option: bad assembly mode");
       if (c->quad != value) c->assembled = false;
       c->quad = value;
+      return BS_OK;
+    case BS_OPT_PHI_INVERSE:
+      if (value != 0 && value != 1) return fail(BS_ERR_ARG, "bs_set_option: bad Phi-inverse mode");
+      if (c->phi_general != value) c->assembled = false;
+      c->phi_general = value;
       return BS_OK;
     case BS_OPT_TIMING:
       if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
@@ -495,11 +504,29 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   tick(lead, 2, s);
   // S3: Phi = L L^H, X = L^{-1}, Y = X^H X;  R = L_R L_R^H, X_R = L_R^{-1}
   CU(cudaMemsetAsync(lead->d_info, 0, sizeof(int) * 2 * ncells, s));
-  bsk::launch_copy_matrix(n3, n3, R(L.Phi), n3, R(L.Lf), n3, ncells, 1, s); ++nl;
   bsk::launch_copy_matrix(Ni, Ni, R(L.R), Ni, R(L.LR), Ni, ncells, 1, s); ++nl;
-  nl += bsk::potrf_trtri(n3, n3, R(L.Lf), R(L.X), R(L.tmp), R(L.dinv), lead->d_info, 0, ncells, 1, s);
   nl += bsk::potrf_trtri(Ni, Ni, R(L.LR), R(L.XR), R(L.tmpR), R(L.dinvR), lead->d_info + ncells, 0, ncells, 1, s);
-  {
+  bool iso = !lead->phi_general;
+  for (int c = 0; c < ncells; ++c) iso = iso && cells[c]->isotropic;
+  if (iso) {
+    // isotropic phases: Phi^{-1} from (A+B)^{-1} and (A-B)^{-1}, two N x N inverses instead of one 3N x 3N
+    const long long NN = (long long)Ni * Ni;
+    bsk::launch_expand_sumdiff(ncells, Mt, R(L.table), R(L.Lf), R(L.Lf + NN), s); ++nl;
+    for (int w = 0; w < 2; ++w) {
+      nl += bsk::potrf_trtri(Ni, Ni, R(L.Lf + w * NN), R(L.X + w * NN), R(L.tmp + w * NN), R(L.dinv), lead->d_info, 0, ncells, 1, s);
+      bsk::GemmDesc g{};
+      g.ncells = ncells; g.inner = 1; g.kclass = bsk::KC_GEMM_FACTOR;
+      g.M = Ni; g.N = Ni; g.K = Ni; g.opA = 1; g.opB = 0;
+      g.A = R(L.X + w * NN); g.lda = Ni; g.B = g.A; g.ldb = Ni; g.C = R(L.tmp + (2 + w) * NN); g.ldc = Ni;
+      g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+      g.flags = BS_GEMM_LOWER_ONLY | BS_GEMM_KLO_ROW | BS_GEMM_KLO_COL;
+      bsk::launch_zgemm(g, s); ++nl;
+      bsk::launch_hermitian_fill_upper(Ni, R(L.tmp + (2 + w) * NN), Ni, ncells, 1, s); ++nl;
+    }
+    bsk::launch_compose_y(ncells, Ni, R(L.tmp + 2 * NN), R(L.tmp + 3 * NN), R(L.Y), s); ++nl;
+  } else {
+    bsk::launch_copy_matrix(n3, n3, R(L.Phi), n3, R(L.Lf), n3, ncells, 1, s); ++nl;
+    nl += bsk::potrf_trtri(n3, n3, R(L.Lf), R(L.X), R(L.tmp), R(L.dinv), lead->d_info, 0, ncells, 1, s);
     bsk::GemmDesc g{};
     g.ncells = ncells; g.inner = 1; g.kclass = bsk::KC_GEMM_FACTOR;
     g.M = n3; g.N = n3; g.K = n3; g.opA = 1; g.opB = 0;

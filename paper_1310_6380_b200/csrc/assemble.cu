@@ -151,4 +151,44 @@ void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R,
   expand_kernel<<<grid, 256, 0, s>>>(Mt, table, Phi, R);
 }
 
+// Isotropic shortcut of S3: with Phi = [[A, B, 0], [B, A, 0], [0, 0, 2(A - B)]],
+// Phi^{-1} follows from the two N x N inverses Ei = (A + B)^{-1}, Fi = (A - B)^{-1}.
+// expand_sumdiff: E = A + B, F = A - B from the table channels 0 (Dv11) and 2 (Dv12).
+__global__ void __launch_bounds__(256) expand_sumdiff_kernel(int Mt, BatchRef table, BatchRef E, BatchRef F) {
+  const int cell = blockIdx.z;
+  const int W = 2 * Mt + 1, N = W * W, L = 4 * Mt + 1, L2 = L * L;
+  const int ga = blockIdx.x * blockDim.x + threadIdx.x, gb = blockIdx.y;
+  if (ga >= N) return;
+  const cplx *T = batch_ptr(table, cell, 0);
+  const int f = (gb / W - ga / W + 2 * Mt) * L + (gb % W - ga % W + 2 * Mt);
+  const cplx a = T[f], b = T[(size_t)2 * L2 + f];
+  batch_ptr(E, cell, 0)[(size_t)gb * N + ga] = cadd(a, b);
+  batch_ptr(F, cell, 0)[(size_t)gb * N + ga] = csub(a, b);
+}
+// compose: Y11 = Y22 = (Ei + Fi)/2, Y12 = Y21 = (Ei - Fi)/2, Y33 = Fi/2, all other blocks zero.
+__global__ void __launch_bounds__(256) compose_y_kernel(int N, BatchRef Ei, BatchRef Fi, BatchRef Y) {
+  const int cell = blockIdx.z;
+  const int r = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y;
+  if (r >= N) return;
+  const cplx e = batch_ptr(Ei, cell, 0)[(size_t)c * N + r], f = batch_ptr(Fi, cell, 0)[(size_t)c * N + r];
+  cplx *Yg = batch_ptr(Y, cell, 0);
+  const size_t n3 = 3 * (size_t)N;
+  const cplx sum = cscale(cadd(e, f), 0.5), dif = cscale(csub(e, f), 0.5), zero = cmake(0.0, 0.0);
+  const cplx blk[3][3] = {{sum, dif, zero}, {dif, sum, zero}, {zero, zero, cscale(f, 0.5)}};
+#pragma unroll
+  for (int b = 0; b < 3; ++b)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) Yg[((size_t)b * N + c) * n3 + (size_t)a * N + r] = blk[a][b];
+}
+
+void launch_expand_sumdiff(int ncells, int Mt, BatchRef table, BatchRef E, BatchRef F, cudaStream_t s) {
+  const int W = 2 * Mt + 1, N = W * W;
+  KScope ks(KC_EXPAND, 32.0 * N * N * ncells, s);
+  expand_sumdiff_kernel<<<dim3((N + 255) / 256, N, ncells), 256, 0, s>>>(Mt, table, E, F);
+}
+void launch_compose_y(int ncells, int N, BatchRef Ei, BatchRef Fi, BatchRef Y, cudaStream_t s) {
+  KScope ks(KC_EXPAND, 16.0 * 11.0 * N * N * ncells, s);
+  compose_y_kernel<<<dim3((N + 255) / 256, N, ncells), 256, 0, s>>>(N, Ei, Fi, Y);
+}
+
 }  // namespace bsk

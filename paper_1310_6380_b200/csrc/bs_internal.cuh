@@ -125,6 +125,10 @@ void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, d
 // S2: Phi (3N x 3N full) and R (N x N full) from the table.
 void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s);
 
+// Isotropic shortcut of S3: E = A + B, F = A - B (N x N) from the table; Y from Ei = E^{-1}, Fi = F^{-1}.
+void launch_expand_sumdiff(int ncells, int Mt, BatchRef table, BatchRef E, BatchRef F, cudaStream_t s);
+void launch_compose_y(int ncells, int N, BatchRef Ei, BatchRef Fi, BatchRef Y, cudaStream_t s);
+
 struct GemmDesc {
   int M, N, K, opA, opB, lda, ldb, ldc, flags, inner, ncells;
   int kclass;  // KClass the launch is timed under (0 -> KC_OTHER)

@@ -100,9 +100,12 @@ def test_anisotropic_matrices_parity(bs):
 
 
 @pytest.mark.parametrize("mode", [0, 1])
-def test_pencil_parity(bs, mode):
+@pytest.mark.parametrize("phi_general", [0, 1])
+def test_pencil_parity(bs, mode, phi_general):
+    # phi_general = 0: isotropic shortcut (two N x N inverses); 1: full 3N x 3N Cholesky inverse
     cell = wl.get("C1").cells[0]
     h = make_cell(bs, cell, 3, 1, mode=mode)
+    bs.bs_set_option(h, bs.BS_OPT_PHI_INVERSE, phi_general)
     bs.bs_assemble(h, 3)
     Pr, _ = oracle.assemble(*oracle_inputs(cell), 3)
     for kr in [(0.31, 0.12), (0.5, 0.5), (0.0, 0.0)]:
@@ -253,3 +256,18 @@ def test_centroid_rule_assembly_parity(bs):
         lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, Mt, kr, 12)
         check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"centroid k{i}")
     bs.bs_destroy_cell(h)
+
+
+def test_phi_inverse_paths_agree_on_bands(bs):
+    w = wl.get("C2")
+    cell = w.cells[0]
+    out = []
+    for general in (0, 1):
+        h = make_cell(bs, cell, w.Mt, 6)
+        bs.bs_set_option(h, bs.BS_OPT_PHI_INVERSE, general)
+        bs.bs_assemble(h, w.Mt)
+        out.append(bs.bs_bands(h, w.kpts[[0, 1, 9, 20, 40, 59]], w.nbands))
+        bs.bs_destroy_cell(h)
+    om0, om1 = np.sqrt(np.maximum(out[0], 0)), np.sqrt(np.maximum(out[1], 0))
+    nz = om1 > 1e-3 * om1.max()
+    assert np.max(np.abs(om0[nz] - om1[nz]) / om1[nz]) < 1e-9

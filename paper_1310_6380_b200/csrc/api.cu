@@ -58,7 +58,7 @@ Layout make_layout(int Mt, int nk, int mode, int nb) {
   L.Lf = take(n3 * n3);
   L.X = take(n3 * n3);
   L.tmp = take(n3 * n3);
-  L.dinv = take(((n3 + 63) / 64) * 4096);
+  L.dinv = take(((n3 + 63) / 64) * 4096 + ((N + 63) / 64) * 4096);  // + a second N-sized slot (isotropic shortcut)
   L.Y = take(n3 * n3);
   L.LR = take(N * N);
   L.XR = take(N * N);
@@ -104,7 +104,8 @@ struct bs_cell {
   // batch scratch owned by the handle that leads a call (cells[0])
   unsigned long long *d_bases = nullptr;
   bsk::Geometry *d_geos = nullptr;
-  int *d_info = nullptr;
+  int *d_info = nullptr;              // [5 ncells]: Phi, R, then (E, F, R) of the batched isotropic factorisation
+  unsigned long long *d_bases3 = nullptr;  // [4][3 ncells] matrix addresses of that batched call
   int batch_cap = 0;
   double *d_flat = nullptr;  // d, e, scal, lam, coefk
   size_t flat_cap = 0;
@@ -129,10 +130,12 @@ bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStr
     if (lead->d_bases) cudaFree(lead->d_bases);
     if (lead->d_geos) cudaFree(lead->d_geos);
     if (lead->d_info) cudaFree(lead->d_info);
-    lead->d_bases = nullptr; lead->d_geos = nullptr; lead->d_info = nullptr; lead->batch_cap = 0;
+    if (lead->d_bases3) cudaFree(lead->d_bases3);
+    lead->d_bases = nullptr; lead->d_geos = nullptr; lead->d_info = nullptr; lead->d_bases3 = nullptr; lead->batch_cap = 0;
     CU(cudaMalloc(&lead->d_bases, sizeof(unsigned long long) * ncells));
     CU(cudaMalloc(&lead->d_geos, sizeof(bsk::Geometry) * ncells));
-    CU(cudaMalloc(&lead->d_info, sizeof(int) * 2 * ncells));
+    CU(cudaMalloc(&lead->d_info, sizeof(int) * 5 * ncells));
+    CU(cudaMalloc(&lead->d_bases3, sizeof(unsigned long long) * 12 * ncells));
     lead->batch_cap = ncells;
   }
   std::vector<unsigned long long> b(ncells);
@@ -302,7 +305,7 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
 void bs_destroy_cell(bs_cell *c) {
   if (!c) return;
   cudaFree(c->d_edge); cudaFree(c->d_ephase); cudaFree(c->d_w); cudaFree(c->d_area); cudaFree(c->d_geo);
-  cudaFree(c->d_bases); cudaFree(c->d_geos); cudaFree(c->d_info); cudaFree(c->d_flat);
+  cudaFree(c->d_bases); cudaFree(c->d_geos); cudaFree(c->d_info); cudaFree(c->d_bases3); cudaFree(c->d_flat);
   for (auto &e : c->ev)
     if (e) cudaEventDestroy(e);
   delete c->kt;
@@ -503,17 +506,30 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2
   tick(lead, 2, s);
   // S3: Phi = L L^H, X = L^{-1}, Y = X^H X;  R = L_R L_R^H, X_R = L_R^{-1}
-  CU(cudaMemsetAsync(lead->d_info, 0, sizeof(int) * 2 * ncells, s));
+  CU(cudaMemsetAsync(lead->d_info, 0, sizeof(int) * 5 * ncells, s));
   bsk::launch_copy_matrix(Ni, Ni, R(L.R), Ni, R(L.LR), Ni, ncells, 1, s); ++nl;
-  nl += bsk::potrf_trtri(Ni, Ni, R(L.LR), R(L.XR), R(L.tmpR), R(L.dinvR), lead->d_info + ncells, 0, ncells, 1, s);
   bool iso = !lead->phi_general;
   for (int c = 0; c < ncells; ++c) iso = iso && cells[c]->isotropic;
+  if (!iso) nl += bsk::potrf_trtri(Ni, Ni, R(L.LR), R(L.XR), R(L.tmpR), R(L.dinvR), lead->d_info + ncells, 0, ncells, 1, s);
   if (iso) {
     // isotropic phases: Phi^{-1} from (A+B)^{-1} and (A-B)^{-1}, two N x N inverses instead of one 3N x 3N
     const long long NN = (long long)Ni * Ni;
     bsk::launch_expand_sumdiff(ncells, Mt, R(L.table), R(L.Lf), R(L.Lf + NN), s); ++nl;
+    {  // E, F and R (all N x N) are factored and inverted as ONE batch of 3 ncells matrices (one latency chain)
+      const long long dN = (long long)((Ni + 63) / 64) * 4096;
+      const long long offs[4][3] = {{L.Lf, L.Lf + NN, L.LR}, {L.X, L.X + NN, L.XR}, {L.tmp, L.tmp + NN, L.tmpR},
+                                    {L.dinv, L.dinv + dN, L.dinvR}};
+      std::vector<unsigned long long> hb((size_t)12 * ncells);
+      for (int a4 = 0; a4 < 4; ++a4)
+        for (int c = 0; c < ncells; ++c)
+          for (int w = 0; w < 3; ++w)
+            hb[((size_t)a4 * ncells + c) * 3 + w] = (unsigned long long)((cplx *)cells[c]->ws + offs[a4][w]);
+      CU(cudaMemcpyAsync(lead->d_bases3, hb.data(), sizeof(unsigned long long) * hb.size(), cudaMemcpyHostToDevice, s));
+      CU(cudaStreamSynchronize(s));  // hb goes out of scope
+      auto B3 = [&](int a4) { BatchRef r; r.bases = lead->d_bases3 + (size_t)a4 * 3 * ncells; r.single = 0; r.off = 0; r.stride = 0; return r; };
+      nl += bsk::potrf_trtri(Ni, Ni, B3(0), B3(1), B3(2), B3(3), lead->d_info + 2 * ncells, 0, 3 * ncells, 1, s);
+    }
     for (int w = 0; w < 2; ++w) {
-      nl += bsk::potrf_trtri(Ni, Ni, R(L.Lf + w * NN), R(L.X + w * NN), R(L.tmp + w * NN), R(L.dinv), lead->d_info, 0, ncells, 1, s);
       bsk::GemmDesc g{};
       g.ncells = ncells; g.inner = 1; g.kclass = bsk::KC_GEMM_FACTOR;
       g.M = Ni; g.N = Ni; g.K = Ni; g.opA = 1; g.opB = 0;
@@ -557,7 +573,13 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   CU(cudaGetLastError());
   if (bsk::g_kt) bsk::g_kt->collect();
   std::vector<int> info(2 * ncells);
-  CU(cudaMemcpy(info.data(), lead->d_info, sizeof(int) * 2 * ncells, cudaMemcpyDeviceToHost));
+  std::vector<int> info5(5 * ncells);
+  CU(cudaMemcpy(info5.data(), lead->d_info, sizeof(int) * 5 * ncells, cudaMemcpyDeviceToHost));
+  for (int c = 0; c < ncells; ++c) {
+    const int *b3 = &info5[2 * ncells + 3 * c];  // batched isotropic path: E, F -> Phi; R
+    info[c] = info5[c] ? info5[c] : (b3[0] ? b3[0] : b3[1]);
+    info[ncells + c] = info5[ncells + c] ? info5[ncells + c] : b3[2];
+  }
   lead->launches += nl;
   if (lead->timing) {
     lead->ms[BS_T_TABLE] = tock(lead, 0, 1);

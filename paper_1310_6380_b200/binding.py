@@ -135,7 +135,7 @@ class Cell:
         self.Mt = None
 
     def close(self):
-        if getattr(self, "handle", None):
+        if getattr(self, "handle", None) and lib is not None:   # lib is None during interpreter shutdown
             lib.bs_destroy_cell(self.handle)
             self.handle = None
             self.workspace = None

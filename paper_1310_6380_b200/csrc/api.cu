@@ -89,6 +89,7 @@ struct bs_cell {
   int P = 0, nedge = 0;
   bool isotropic = true;  // every phase has the isotropic plane-strain block structure of PAPER.md:173
   int phi_general = 0;    // BS_OPT_PHI_INVERSE: 1 = always the general 3N x 3N inverse
+  char *d_blob = nullptr;  // the one device allocation that holds geo, edge, w, area, ephase
   double *d_edge = nullptr, *d_w = nullptr, *d_area = nullptr;
   int *d_ephase = nullptr;
   bsk::Geometry geo;
@@ -280,21 +281,33 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
     delete c;
     return fail(BS_ERR_GEOMETRY, "bs_create_cell: phases cover area %.17g, cell area is %.17g", total, c->V);
   }
-  bs_status st = BS_OK;
-  auto up = [&](void **dst, const void *src, size_t bytes) {
-    if (st != BS_OK) return;
-    if (cudaMalloc(dst, bytes) != cudaSuccess || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) != cudaSuccess)
-      st = fail(BS_ERR_CUDA, "bs_create_cell: device allocation/copy failed: %s", cudaGetErrorString(cudaGetLastError()));
-  };
-  up((void **)&c->d_edge, edge.data(), sizeof(double) * edge.size());
-  up((void **)&c->d_ephase, eph.data(), sizeof(int) * eph.size());
-  up((void **)&c->d_w, w.data(), sizeof(double) * w.size());
-  up((void **)&c->d_area, area.data(), sizeof(double) * area.size());
+  // one device allocation and one H2D copy per cell: [Geometry | edge | w | area | ephase], each part 256-byte aligned
+  auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  const size_t o_geo = 0, o_edge = pad(sizeof(bsk::Geometry)), o_w = o_edge + pad(sizeof(double) * edge.size()),
+               o_area = o_w + pad(sizeof(double) * w.size()), o_eph = o_area + pad(sizeof(double) * area.size()),
+               total_bytes = o_eph + pad(sizeof(int) * eph.size());
+  char *dev = nullptr;
+  if (cudaMalloc((void **)&dev, total_bytes) != cudaSuccess) {
+    delete c;
+    return fail(BS_ERR_CUDA, "bs_create_cell: device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  c->d_blob = dev;
+  c->d_geo = reinterpret_cast<bsk::Geometry *>(dev + o_geo);
+  c->d_edge = reinterpret_cast<double *>(dev + o_edge);
+  c->d_w = reinterpret_cast<double *>(dev + o_w);
+  c->d_area = reinterpret_cast<double *>(dev + o_area);
+  c->d_ephase = reinterpret_cast<int *>(dev + o_eph);
   c->geo.edge = c->d_edge; c->geo.ephase = c->d_ephase; c->geo.w = c->d_w; c->geo.area = c->d_area;
   c->geo.nedge = ne; c->geo.P = nphase;
   std::memcpy(c->geo.Q, c->Q, sizeof(double) * 4);
-  up((void **)&c->d_geo, &c->geo, sizeof(bsk::Geometry));
-  if (st != BS_OK) {
+  std::vector<char> host(total_bytes, 0);
+  std::memcpy(host.data() + o_geo, &c->geo, sizeof(bsk::Geometry));
+  std::memcpy(host.data() + o_edge, edge.data(), sizeof(double) * edge.size());
+  std::memcpy(host.data() + o_w, w.data(), sizeof(double) * w.size());
+  std::memcpy(host.data() + o_area, area.data(), sizeof(double) * area.size());
+  std::memcpy(host.data() + o_eph, eph.data(), sizeof(int) * eph.size());
+  if (cudaMemcpy(dev, host.data(), total_bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+    bs_status st = fail(BS_ERR_CUDA, "bs_create_cell: H2D copy failed: %s", cudaGetErrorString(cudaGetLastError()));
     bs_destroy_cell(c);
     return st;
   }
@@ -304,7 +317,7 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
 
 void bs_destroy_cell(bs_cell *c) {
   if (!c) return;
-  cudaFree(c->d_edge); cudaFree(c->d_ephase); cudaFree(c->d_w); cudaFree(c->d_area); cudaFree(c->d_geo);
+  cudaFree(c->d_blob);
   cudaFree(c->d_bases); cudaFree(c->d_geos); cudaFree(c->d_info); cudaFree(c->d_bases3); cudaFree(c->d_flat);
   for (auto &e : c->ev)
     if (e) cudaEventDestroy(e);

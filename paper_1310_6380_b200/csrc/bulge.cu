@@ -391,7 +391,7 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
   const size_t max_smem = 226 * 1024;
   int G, Wc;
   if ((size_t)n * colbytes + gmax * team_bytes + (size_t)n * sizeof(int) <= max_smem) {  // whole band resident
-    Wc = n;
+    Wc = max(n, 2 * B + 8);  // never fewer than a block pair of columns: the masked loads of a step stay inside the ring
     G = max(1, min(gmax, (n + 2 * B - 1) / (2 * B)));
   } else {
     G = (int)(((max_smem - gmax * team_bytes) / colbytes - 8) / (2 * B));

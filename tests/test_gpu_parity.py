@@ -271,3 +271,67 @@ def test_phi_inverse_paths_agree_on_bands(bs):
     om0, om1 = np.sqrt(np.maximum(out[0], 0)), np.sqrt(np.maximum(out[1], 0))
     nz = om1 > 1e-3 * om1.max()
     assert np.max(np.abs(om0[nz] - om1[nz]) / om1[nz]) < 1e-9
+
+
+def test_edge_cases_small_truncations_full_spectrum_single_k(bs):
+    # Mt = 0 (one plane wave: K is 2 x 2), Mt = 1, nbands = 2N (the whole spectrum), nk = 1
+    cell = wl.random_small_cell(31, 3, wl.HEXAGONAL)
+    for Mt in (0, 1, 2):
+        n2 = 2 * (2 * Mt + 1) ** 2
+        h = make_cell(bs, cell, Mt, 1)
+        bs.bs_assemble(h, Mt)
+        Pr, Sr = oracle.assemble(*oracle_inputs(cell), Mt)
+        kr = np.array([[0.37, 0.21]])
+        lam = bs.bs_bands(h, kr, n2)
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, Mt, kr[0])
+        check_bands(lam, lr[None, :], np.array([lmax]), f"Mt{Mt}")
+        bs.bs_destroy_cell(h)
+
+
+def test_truncation_limit_is_reported(bs):
+    cell = wl.random_small_cell(1, 2)
+    h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, bs.bs_isotropic_plane_strain(cell.E, cell.nu), cell.rho)
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_workspace_bytes(h, 16, 1)          # 2N = 2178 > 2048
+    assert ei.value.status == bs.BS_ERR_ARG
+    assert bs.bs_workspace_bytes(h, 15, 1) > 0   # the maximum, config 5's truncation
+    bs.bs_destroy_cell(h)
+
+
+def test_nonconvex_and_translated_polygons(bs):
+    # an L-shaped (non-convex) phase, and a phase given as a lattice-translated piece sticking out of the cell (R11)
+    lattice = wl.SQUARE
+    Lshape = np.array([[0, 0], [1, 0], [1, 0.4], [0.4, 0.4], [0.4, 1], [0, 1.0]])
+    square = np.array([[0.4, 0.4], [1, 0.4], [1, 1], [0.4, 1.0]])
+    E, nu, rho = np.array([5e9, 60e9]), np.array([0.3, 0.25]), np.array([1200.0, 2600.0])
+    comp = oracle.isotropic_plane_strain_compliance(E, nu)
+    results = []
+    for shift in (np.zeros(2), np.array([1.0, 0.0]), np.array([-1.0, 2.0])):
+        off, verts = wl._csr([Lshape, square + shift])
+        h = bs.bs_create_cell(lattice, off, verts, bs.bs_isotropic_plane_strain(E, nu), rho)
+        bs.allocate_workspace(h, 2, 2)
+        bs.bs_assemble(h, 2)
+        Phi, Psi = bs.bs_get_matrices(h)
+        Pr, Sr = oracle.assemble(lattice, off, verts, comp, rho, 2)
+        assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+        assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+        results.append(bs.bs_bands(h, [[0.3, 0.1], [0.5, 0.5]], 8))
+        bs.bs_destroy_cell(h)
+    # translating a phase by a lattice vector changes nothing (I_p(G) is invariant)
+    assert np.allclose(results[0], results[1], rtol=1e-10) and np.allclose(results[0], results[2], rtol=1e-10)
+
+
+def test_many_kpoints_and_repeated_calls(bs):
+    w = wl.get("C1")
+    cell = w.cells[0]
+    kp = wl.kpath(cell.lattice, wl.SQUARE_PATH, 517)
+    h = make_cell(bs, cell, w.Mt, 517)
+    bs.bs_assemble(h, w.Mt)
+    lam_all = bs.bs_bands(h, kp, 4)
+    lam_part = bs.bs_bands(h, kp[100:133], 4)           # fewer k-points than the workspace was sized for
+    assert np.array_equal(lam_part, lam_all[100:133])   # deterministic, independent of the batch it ran in
+    import torch
+    out = torch.empty(517, 4, dtype=torch.float64, device="cuda")
+    bs.bs_bands(h, kp, 4, out=out)                      # device output pointer
+    assert np.array_equal(out.cpu().numpy(), lam_all)
+    bs.bs_destroy_cell(h)

@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
         cplx a = ring[l >= c ? cb[jj] + l - c : mycb + c - l];  // lower part as stored, upper part mirrored
         a.y = l > c ? a.y : (l == c ? 0.0 : -a.y);
         cfma(acc, a, vc);
-        cfma(uacc, ring[cb[jj] + L + l - c], vc);
+        cfma(uacc, ring[cb[jj] + max(L + l - c, 0)], vc);  // (negative only where vc is masked to zero)
       }
       acc.x = l < L ? acc.x : 0.0;
       acc.y = l < L ? acc.y : 0.0;

@@ -335,3 +335,23 @@ def test_many_kpoints_and_repeated_calls(bs):
     bs.bs_bands(h, kp, 4, out=out)                      # device output pointer
     assert np.array_equal(out.cpu().numpy(), lam_all)
     bs.bs_destroy_cell(h)
+
+
+def test_poly_and_direct_modes_agree_outside_first_zone(bs):
+    # the k-polynomial form of A(k) (six k-independent matrices) against the per-k scaling kernel, also for k far outside
+    # the first Brillouin zone, and against the oracle
+    w = wl.get("C1")
+    cell = w.cells[0]
+    rng = np.random.default_rng(77)
+    kp = np.concatenate([rng.uniform(-2.5, 2.5, size=(9, 2)), [[0.0, 0.0], [1.0, 0.0], [0.5, 0.5]]])
+    lams = []
+    for mode in (0, 1):
+        h = make_cell(bs, cell, w.Mt, len(kp), mode=mode)
+        bs.bs_assemble(h, w.Mt)
+        lams.append(bs.bs_bands(h, kp, 12))
+        bs.bs_destroy_cell(h)
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), w.Mt)
+    for i, kr in enumerate(kp):
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, w.Mt, kr, 12)
+        for lam in lams:
+            check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"k{i}")

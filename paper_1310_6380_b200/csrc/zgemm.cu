@@ -41,8 +41,22 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
 
   // grid.x = (M tiles) x (matrices x k-splits): grid.z is limited to 65535, the batch of config 4 is not
   const int tiles_m = (g.M + BM - 1) / BM;
-  const int bz = blockIdx.x / tiles_m;
-  const int m0 = (blockIdx.x % tiles_m) * BM, n0 = blockIdx.y * BN;
+  int bz, m0, n0;
+  if (BM == BN && (g.flags & BS_GEMM_LOWER_ONLY)) {
+    // only the tiles of the lower triangle are launched: tile t -> (i, j), i >= j, t = i (i + 1) / 2 + j
+    const int ntri = tiles_m * (tiles_m + 1) / 2;
+    bz = blockIdx.x / ntri;
+    const int tix = blockIdx.x % ntri;
+    int i = (int)((sqrtf(8.0f * (float)tix + 1.0f) - 1.0f) * 0.5f);
+    while (i * (i + 1) / 2 > tix) --i;
+    while ((i + 1) * (i + 2) / 2 <= tix) ++i;
+    m0 = i * BM;
+    n0 = (tix - i * (i + 1) / 2) * BN;
+  } else {
+    bz = blockIdx.x / tiles_m;
+    m0 = (blockIdx.x % tiles_m) * BM;
+    n0 = blockIdx.y * BN;
+  }
   if ((g.flags & BS_GEMM_LOWER_ONLY) && n0 >= m0 + BM) return;
   const int nsplit = g.ksplit > 1 ? g.ksplit : 1;
   const int ks = bz % nsplit, zz = bz / nsplit;
@@ -193,7 +207,9 @@ void launch_one(const GemmDesc &g, cudaStream_t s) {
     cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_done = true;
   }
-  dim3 grid(((g.M + BM - 1) / BM) * g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1), (g.N + BN - 1) / BN, 1);
+  const int tm = (g.M + BM - 1) / BM, zz = g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1);
+  dim3 grid(tm * zz, (g.N + BN - 1) / BN, 1);
+  if (BM == BN && (g.flags & BS_GEMM_LOWER_ONLY)) grid = dim3((tm * (tm + 1) / 2) * zz, 1, 1);  // requires M == N
   zgemm_kernel<OPA, OPB, HERM, BM, BN><<<grid, NT, smem, s>>>(g);
 }
 }  // namespace

@@ -355,3 +355,29 @@ def test_poly_and_direct_modes_agree_outside_first_zone(bs):
         lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, w.Mt, kr, 12)
         for lam in lams:
             check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"k{i}")
+
+
+def test_high_contrast_many_bands(bs):
+    # stiffness contrast 1e4 and density contrast 50 (cond(Phi) ~ 1e5), 150 of 338 eigenvalues (several Sturm passes)
+    cell = wl.get("C3").cells[0]
+    rng = np.random.default_rng(5)
+    E = np.where(rng.uniform(size=cell.nphase) < 0.5, 2e7, 2e11)
+    rho = np.where(rng.uniform(size=cell.nphase) < 0.5, 200.0, 10000.0)
+    nu = np.full(cell.nphase, 0.3)
+    Mt = 6
+    h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, bs.bs_isotropic_plane_strain(E, nu), rho)
+    bs.allocate_workspace(h, Mt, 3)
+    bs.bs_assemble(h, Mt)
+    comp = oracle.isotropic_plane_strain_compliance(E, nu)
+    Pr, Sr = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, comp, rho, Mt)
+    Phi, Psi = bs.bs_get_matrices(h)
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+    assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    kp = np.array([[0.5, 0.0], [0.21, 0.13], [2.0 / 3.0, 1.0 / 3.0]])
+    lam = bs.bs_bands(h, kp, 150)
+    for i, kr in enumerate(kp):
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, Mt, kr, 150)
+        # the explicit inverse of an ill-conditioned Phi costs cond(Phi) eps in K: allow 1e-7 relative on omega here
+        om_g, om_r = np.sqrt(np.maximum(lam[i], 0)), np.sqrt(np.maximum(lr, 0))
+        assert np.max(np.abs(om_g - om_r) / om_r) < 1e-7, np.max(np.abs(om_g - om_r) / om_r)
+    bs.bs_destroy_cell(h)

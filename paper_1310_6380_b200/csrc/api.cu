@@ -147,7 +147,7 @@ bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStr
   }
   CU(cudaMemcpyAsync(lead->d_bases, b.data(), sizeof(unsigned long long) * ncells, cudaMemcpyHostToDevice, s));
   CU(cudaMemcpyAsync(lead->d_geos, g.data(), sizeof(bsk::Geometry) * ncells, cudaMemcpyHostToDevice, s));
-  CU(cudaStreamSynchronize(s));  // the host vectors go out of scope
+  // (no stream synchronise: an H2D copy from pageable memory is staged before cudaMemcpyAsync returns)
   return BS_OK;
 }
 
@@ -538,7 +538,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
           for (int w = 0; w < 3; ++w)
             hb[((size_t)a4 * ncells + c) * 3 + w] = (unsigned long long)((cplx *)cells[c]->ws + offs[a4][w]);
       CU(cudaMemcpyAsync(lead->d_bases3, hb.data(), sizeof(unsigned long long) * hb.size(), cudaMemcpyHostToDevice, s));
-      CU(cudaStreamSynchronize(s));  // hb goes out of scope
+      // (no stream synchronise: an H2D copy from pageable memory is staged before cudaMemcpyAsync returns)
       auto B3 = [&](int a4) { BatchRef r; r.bases = lead->d_bases3 + (size_t)a4 * 3 * ncells; r.single = 0; r.off = 0; r.stride = 0; return r; };
       nl += bsk::potrf_trtri(Ni, Ni, B3(0), B3(1), B3(2), B3(3), lead->d_info + 2 * ncells, 0, 3 * ncells, 1, s);
     }
@@ -571,7 +571,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
     for (int c = 0; c < ncells; ++c) {
       fill_coef_kvec(cells[c], Mt, kv);
       CU(cudaMemcpyAsync((cplx *)cells[c]->ws + L.kvecA, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
-      CU(cudaStreamSynchronize(s));
+      // (no stream synchronise: an H2D copy from pageable memory is staged before cudaMemcpyAsync returns)
     }
     // the cells of one batch may have different areas: V^2 is applied per cell
     bool sameV = true;
@@ -707,14 +707,14 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
         o[0] = 1.0; o[1] = kx; o[2] = ky; o[3] = kx * kx; o[4] = kx * ky; o[5] = ky * ky;
       }
     CU(cudaMemcpyAsync(coefk, ck.data(), ck.size() * sizeof(double), cudaMemcpyHostToDevice, s));
-    CU(cudaStreamSynchronize(s));
+    // (no stream synchronise: an H2D copy from pageable memory is staged before cudaMemcpyAsync returns)
     bsk::launch_combine(n2, R(L.Coef), mat, R(L.Ak, mat), n2, coefk, nk, ncells, s); ++nl;
   } else {
     std::vector<double> kv;
     for (int c = 0; c < ncells; ++c) {
       fill_direct_kvec(cells[c], Mt, nk, kpts, kv);
       CU(cudaMemcpyAsync((cplx *)cells[c]->ws + L.kvecK, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
-      CU(cudaStreamSynchronize(s));
+      // (no stream synchronise: an H2D copy from pageable memory is staged before cudaMemcpyAsync returns)
     }
     bsk::launch_pencil(N, lead->V * lead->V, R(L.Y), n3, R(L.Kk, mat), n2, R(L.kvecK, 2LL * N), 1, ncells, nk, s); ++nl;  // S4
     nl += reduce_blocks(lead, cells, ncells, L, L.Kk, L.Ak, nk, s);                                                        // S5

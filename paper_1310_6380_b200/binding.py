@@ -1,8 +1,9 @@
 """ctypes binding of ``libbs.so`` (C-ABI in ``include/bs.h``): argument marshalling only.
 
 Every step of the path runs in the CUDA kernels behind the C calls.  PyTorch supplies device memory (the workspace
-tensor lent to the handle) and the stream.  There is no CPU fallback: importing this module without a built
-``libbs.so`` raises, and every compute call fails with ``BsError`` when there is no CUDA device.
+tensor lent to the handle) and the stream.  There is no CPU fallback: importing this module compiles ``libbs.so``
+with nvcc when it is missing and raises if that fails, and every compute call fails with ``BsError`` when there is no
+CUDA device.
 """
 from __future__ import annotations
 
@@ -42,8 +43,14 @@ class BsError(RuntimeError):
 
 
 if not os.path.exists(LIB_PATH):
-    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1310_6380_b200.build` "
-                      "(there is no CPU fallback)")
+    # not built yet (fresh checkout: the .so is git-ignored): compile it now with nvcc; there is no CPU fallback, so a
+    # failed build is fatal
+    try:
+        from . import build as _build
+        _build.build()
+    except Exception as exc:  # pragma: no cover
+        raise ImportError(f"{LIB_PATH} is missing and could not be built ({exc}); run "
+                          "`python -m paper_1310_6380_b200.build` (there is no CPU fallback)") from exc
 lib = C.CDLL(LIB_PATH)
 
 _dp = C.POINTER(C.c_double)

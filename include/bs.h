@@ -47,7 +47,8 @@ typedef enum {
 } bs_option;
 enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
 /* BS_OPT_TRIDIAG (option 3): algorithm of S6.  0 = two-stage (dense -> band by DMMA GEMMs, band -> tridiagonal by bulge
- * chasing; default), 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check). */
+ * chasing; default; matrices with n <= 112 are tridiagonalised inside shared memory by one CTA instead),
+ * 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check). */
 enum { BS_OPT_TRIDIAG = 3 };
 enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1 };
 /* BS_OPT_ASSEMBLY (option 4): quadrature of the shape integrals in S1.  0 = exact closed-form polygon integral (default),
@@ -161,7 +162,8 @@ enum {
   BS_KC_BULGE = 12,       /* S6 stage 2: band -> tridiagonal bulge chasing                                           */
   BS_KC_GEMM_HEMM = 13,   /* S6 stage 1: Z = A22 V (Hermitian A22, lower triangle read), DMMA             work: real flops */
   BS_KC_GEMM_WY = 14,     /* S6 stage 1: the two small compact-WY GEMMs per panel, DMMA                    work: real flops */
-  BS_KC_COUNT = 15
+  BS_KC_TRIDIAG_SMALL = 15, /* S6 for n <= 112: whole matrix in shared memory, unblocked Householder    work: real flops */
+  BS_KC_COUNT = 16
 };
 /* Per-class totals of the last bs_assemble / bs_bands led by this handle under BS_OPT_TIMING = 2: device milliseconds
  * (CUDA events on the call's stream around every launch), ALGORITHMIC work credited at launch time (flops or bytes, see

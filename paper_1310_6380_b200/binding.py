@@ -262,7 +262,7 @@ def bs_get_timings(cell: Cell) -> np.ndarray:
 
 
 KERNEL_CLASSES = ["table", "expand", "gemm_factor", "gemm_reduce", "gemm_tridiag", "hemv", "panel", "sturm", "pencil",
-                  "combine", "potrf_diag", "other", "bulge", "gemm_hemm", "gemm_wy"]
+                  "combine", "potrf_diag", "other", "bulge", "gemm_hemm", "gemm_wy", "tridiag_small"]
 
 
 def bs_get_kernel_timings(cell: Cell) -> dict:

@@ -13,7 +13,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libbs.so")
-SOURCES = ["api.cu", "assemble.cu", "factor.cu", "zgemm.cu", "pencil.cu", "tridiag.cu", "band.cu", "bulge.cu", "sturm.cu", "probe.cu"]
+SOURCES = ["api.cu", "assemble.cu", "factor.cu", "zgemm.cu", "pencil.cu", "tridiag.cu", "band.cu", "bulge.cu", "small.cu", "sturm.cu", "probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + os.path.join(ROOT, "include"), "-I" + CSRC]
 

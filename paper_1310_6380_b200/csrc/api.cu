@@ -723,6 +723,8 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   if (lead->algo == BS_TRIDIAG_ONE_STAGE) {
     nl += bsk::launch_tridiag(n2, n2, lead->nb, R(L.Ak, mat), R(L.VW, L.vw_stride),
                               R(L.P, (long long)bsk::tridiag_p_elems(n2)), d, e, scal, ncells, nk, s);  // S6
+  } else if (n2 <= bsk::tridiag_small_max_n()) {
+    bsk::launch_tridiag_small(n2, n2, R(L.Ak, mat), d, e, ncells, nk, s); ++nl;                        // S6, matrix in shared memory
   } else {
     const int bw = band_width(lead->nb);
     nl += bsk::launch_sy2sb(n2, n2, bw, R(L.Ak, mat), R(L.VW, L.vw_stride), R(L.SM, L.sm_stride), R(L.AB, L.ab_stride),
@@ -835,6 +837,12 @@ bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d,
   const long long per = (long long)bs_zhetrd_scratch_elems(n, nb);
   cplx *sc = (cplx *)scratch;
   BatchRef VW = raw(sc, per), P = raw(sc + vw, per);
+  if (algo == BS_TRIDIAG_TWO_STAGE && n <= bsk::tridiag_small_max_n()) {
+    bsk::launch_tridiag_small(n, lda, raw(A, strideA), d, e, 1, batch, (cudaStream_t)stream);
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    CU(cudaGetLastError());
+    return BS_OK;
+  }
   if (algo == BS_TRIDIAG_TWO_STAGE) {
     BatchRef SMr = raw(sc + vw + pp, per), ABr = raw(sc + vw + pp + smn, per);
     bsk::launch_sy2sb(n, lda, bw, raw(A, strideA), VW, SMr, ABr, 1, batch, (cudaStream_t)stream);

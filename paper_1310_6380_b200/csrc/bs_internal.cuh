@@ -66,7 +66,7 @@ namespace bsk {
 // DMMA classes, bytes for the HBM classes), accumulated on the host at launch time.
 enum KClass {
   KC_TABLE = 0, KC_EXPAND, KC_GEMM_FACTOR, KC_GEMM_REDUCE, KC_GEMM_TRIDIAG, KC_HEMV, KC_PANEL, KC_STURM, KC_PENCIL,
-  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_BULGE, KC_GEMM_HEMM, KC_GEMM_WY, KC_COUNT
+  KC_COMBINE, KC_POTRF_DIAG, KC_OTHER, KC_BULGE, KC_GEMM_HEMM, KC_GEMM_WY, KC_TRIDIAG_SMALL, KC_COUNT
 };
 struct KTimer {
   std::vector<cudaEvent_t> ev;   // pool; pairs (2i, 2i+1)
@@ -170,6 +170,9 @@ size_t band_ab_elems(int n, int b);
 int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, BatchRef AB, int ncells, int inner,
                  cudaStream_t s);
 void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s);
+// S6 for n <= tridiag_small_max_n(): the matrix in shared memory, one CTA per matrix, unblocked Householder (small.cu).
+int tridiag_small_max_n();
+void launch_tridiag_small(int n, int lda, BatchRef A, double *d, double *e, int ncells, int inner, cudaStream_t s);
 // S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
 void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s);
 

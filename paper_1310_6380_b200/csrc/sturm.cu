@@ -7,9 +7,8 @@
 namespace bsk {
 
 namespace {
-constexpr int ST = 256;   // threads per matrix
+constexpr int ST = 256;   // maximum threads per matrix (the launch uses 8 threads per wanted eigenvalue, rounded to warps)
 constexpr int G = 8;      // interior shifts per eigenvalue per round -> the interval shrinks 9x per round
-constexpr int EPB = ST / G;  // eigenvalues per pass
 constexpr int ROUNDS = 24;   // 9^24 > 2^76
 
 // Number of eigenvalues < x = number of negative q_i = p_i / p_{i-1}, q_0 = d_0 - x, q_i = d_i - x - e_{i-1}^2 / q_{i-1}
@@ -44,7 +43,8 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
   const int z = blockIdx.x, t = threadIdx.x;
   dg += (size_t)z * n;
   eg += (size_t)z * n;
-  for (int i = t; i < n; i += ST) {
+  const int nthr = blockDim.x, EPB = nthr / G;  // eigenvalues per pass
+  for (int i = t; i < n; i += nthr) {
     d[i] = dg[i];
     e2[i] = (i + 1 < n) ? eg[i] * eg[i] : 0.0;
   }
@@ -95,7 +95,8 @@ void launch_sturm(int n, const double *d, const double *e, int nev, double *lam,
     attr_done = true;
   }
   KScope ks(KC_STURM, 0.0, s);
-  sturm_kernel<<<nmat, ST, smem, s>>>(n, d, e, nev, lam);
+  const int nthr = nev * G >= ST ? ST : ((nev * G + 31) / 32) * 32;  // few eigenvalues: small CTAs, more of them per SM
+  sturm_kernel<<<nmat, nthr, smem, s>>>(n, d, e, nev, lam);
 }
 
 }  // namespace bsk

@@ -16,21 +16,7 @@
 namespace bsk {
 
 namespace {
-constexpr int QT = 1024;     // threads of the panel QR kernel (32 warps: one warp per trailing column of the panel)
-constexpr int NMAXQ = 2048;  // max rows of a panel (n <= 2048)
 constexpr int KS = 8;         // split-K factor of the Gram product [G | S] = V^H [V | Z] (one output tile per matrix)
-
-__device__ __forceinline__ double block_sum_q(double x, double *scratch) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-  __syncthreads();
-  if (l == 0) scratch[w] = x;
-  __syncthreads();
-  double s = 0.0;
-  for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += scratch[i];
-  return s;
-}
 
 // Householder QR of the m x b panel block of every matrix, one CTA per matrix.  The panel is processed in sub-panels
 // of SW = 4 columns held in shared memory: a sub-panel is factored there (no global round trips between its columns), its
@@ -39,7 +25,6 @@ __device__ __forceinline__ double block_sum_q(double x, double *scratch) {
 // band); V goes to columns [0,b) and [2b,3b) of VW (rows indexed globally, zeros above the unit diagonal and in unused
 // columns); tau to SM + 4 b^2.
 constexpr int SW = 4;  // sub-panel width
-constexpr int CH = 4;  // trailing panel columns updated together
 
 template <int K, int NTHR>
 __device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double *res) {

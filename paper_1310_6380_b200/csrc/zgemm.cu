@@ -31,10 +31,14 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 
 // HERM = 1: A is an M x M Hermitian matrix of which only the LOWER triangle is valid (K == M, OPA == 0):
 //   op(A)[m][k] = A[m][k] for m > k, Re A[m][m] for m == k, conj(A[k][m]) for m < k  (the HEMM of the band reduction).
-template <int OPA, int OPB, int HERM, int BM, int BN>
-__global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
-  constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / 16;  // WMN warps along m, 8 / WMN along n
-  static_assert((BM / 16) * (BN / 32) == 8, "8 warps of 16 x 32");
+// M3 = 1: the "3M" form of the complex product, three real DMMAs per complex multiply-add instead of four:
+//   Re = ar br - ai bi,  Im = (ar + ai)(br + bi) - ar br - ai bi   (norm-wise stable)
+//         with three accumulator sets the warp tile shrinks to 16 x 16 (CTA tile 64 x 32).
+template <int OPA, int OPB, int HERM, int BM, int BN, int M3>
+__global__ void __launch_bounds__(NT, 2) zgemm_kernel(const GemmDesc g) {
+  constexpr int NI = M3 ? 2 : 4;                                // 8-column sub-tiles per warp
+  constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / 16;  // WMN warps along m, (NT / 32) / WMN along n
+  static_assert((BM / 16) * (BN / (8 * NI)) == NT / 32, "warps of 16 x 8 NI");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx(*As)[BK][LDA_S] = reinterpret_cast<cplx(*)[BK][LDA_S]>(smem_raw);
   cplx(*Bs)[BK][LDB_S] = reinterpret_cast<cplx(*)[BK][LDB_S]>(smem_raw + (size_t)STAGES * BK * LDA_S * sizeof(cplx));
@@ -42,16 +46,18 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
   // grid.x = (M tiles) x (matrices x k-splits): grid.z is limited to 65535, the batch of config 4 is not
   const int tiles_m = (g.M + BM - 1) / BM;
   int bz, m0, n0;
-  if (BM == BN && (g.flags & BS_GEMM_LOWER_ONLY)) {
-    // only the tiles of the lower triangle are launched: tile t -> (i, j), i >= j, t = i (i + 1) / 2 + j
-    const int ntri = tiles_m * (tiles_m + 1) / 2;
+  if (g.flags & BS_GEMM_LOWER_ONLY) {
+    // only the tiles of the lower triangle are launched: with R = BM / BN column tiles per row tile,
+    // tile t -> (i, j), j < R (i + 1), t = R i (i + 1) / 2 + j
+    constexpr int R = BM / BN;
+    const int ntri = R * tiles_m * (tiles_m + 1) / 2;
     bz = blockIdx.x / ntri;
     const int tix = blockIdx.x % ntri;
-    int i = (int)((sqrtf(8.0f * (float)tix + 1.0f) - 1.0f) * 0.5f);
-    while (i * (i + 1) / 2 > tix) --i;
-    while ((i + 1) * (i + 2) / 2 <= tix) ++i;
+    int i = (int)((sqrtf(8.0f * (float)(tix / R) + 1.0f) - 1.0f) * 0.5f);
+    while (R * i * (i + 1) / 2 > tix) --i;
+    while (R * (i + 1) * (i + 2) / 2 <= tix) ++i;
     m0 = i * BM;
-    n0 = (tix - i * (i + 1) / 2) * BN;
+    n0 = (tix - R * i * (i + 1) / 2) * BN;
   } else {
     bz = blockIdx.x / tiles_m;
     m0 = (blockIdx.x % tiles_m) * BM;
@@ -88,7 +94,7 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
       int m, k;
       bool tr = OPA != 0;                                  // read the element from its transposed position
       if (HERM && k0 >= m0 + BM - 1) tr = true;            // the whole k-tile lies above the diagonal
-      if (!tr) { m = t % BM; k = t / BM + (NT / BM) * r; } else { k = t & 7; m = (t >> 3) + 32 * r; }
+      if (!tr) { m = t % BM; k = t / BM + (NT / BM) * r; } else { k = t & 7; m = (t >> 3) + (NT / 8) * r; }
       if (HERM && !tr && k0 + BK - 1 > m0) tr = (k0 + k > m0 + m);   // tile crossing the diagonal: per element
       const bool ok = (m0 + m < g.M) && (k0 + k < khi);
       const cplx *src = !tr ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
@@ -96,9 +102,10 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
       cp_async16(&As[stage][k][m], ok ? src : A, ok);
     }
 #pragma unroll
-    for (int r = 0; r < BN * BK / NT; ++r) {
+    for (int r = 0; r < (BN * BK + NT - 1) / NT; ++r) {
       int n, k;
-      if (OPB == 0) { k = t & 7; n = (t >> 3) + 32 * r; } else { n = t % BN; k = t / BN + (NT / BN) * r; }
+      if (OPB == 0) { k = t & 7; n = (t >> 3) + (NT / 8) * r; } else { n = t % BN; k = t / BN + (NT / BN) * r; }
+      if (BN * BK < NT && t >= BN * BK) break;
       const bool ok = (n0 + n < g.N) && (k0 + k < khi);
       const cplx *src = OPB == 0 ? B + (size_t)(k0 + k) + (size_t)(n0 + n) * g.ldb
                                  : B + (size_t)(n0 + n) + (size_t)(k0 + k) * g.ldb;
@@ -110,19 +117,24 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
   // pay DRAM latency after the (short, K = 2b) main loop of the rank-2b updates
   if (g.beta.x != 0.0 || g.beta.y != 0.0) {
 #pragma unroll
-    for (int ni = 0; ni < 4; ++ni) {
+    for (int ni = 0; ni < NI; ++ni) {
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const int row = m0 + wm * 16 + (lane >> 2), col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
+        const int row = m0 + wm * 16 + (lane >> 2), col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
         if (row < g.M && col < g.N) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(C + (size_t)row + (size_t)col * g.ldc));
       }
     }
   }
-  double cr[2][4][2], ci[2][4][2];
+  // M3 == 0: cr = Re, ci = Im.  M3 == 1: cr = sum ar br, ci = sum (ar + ai)(br + bi), c2 = sum ai bi.
+  double cr[2][NI][2], ci[2][NI][2], c2[M3 ? 2 : 1][M3 ? NI : 1][2];
 #pragma unroll
   for (int i = 0; i < 2; ++i)
 #pragma unroll
-    for (int j = 0; j < 4; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+    for (int j = 0; j < NI; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
+#pragma unroll
+  for (int i = 0; i < (M3 ? 2 : 1); ++i)
+#pragma unroll
+    for (int j = 0; j < (M3 ? NI : 1); ++j) c2[i][j][0] = c2[i][j][1] = 0.0;
 
 #pragma unroll
   for (int s = 0; s < STAGES - 1; ++s) {
@@ -137,7 +149,7 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
     const int st = kt % STAGES;
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
-      cplx a[2], b[4];
+      cplx a[2], b[NI];
 #pragma unroll
       for (int mi = 0; mi < 2; ++mi) {
         a[mi] = As[st][kk + (lane & 3)][wm * 16 + mi * 8 + (lane >> 2)];
@@ -149,19 +161,36 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
         }
       }
 #pragma unroll
-      for (int ni = 0; ni < 4; ++ni) {
-        b[ni] = Bs[st][kk + (lane & 3)][wn * 32 + ni * 8 + (lane >> 2)];
+      for (int ni = 0; ni < NI; ++ni) {
+        b[ni] = Bs[st][kk + (lane & 3)][wn * (8 * NI) + ni * 8 + (lane >> 2)];
         if (OPB) b[ni].y = -b[ni].y;
       }
 #pragma unroll
-      for (int mi = 0; mi < 2; ++mi) {
-        const double nai = -a[mi].y;
+      if (M3) {
+        double bs[NI];
 #pragma unroll
-        for (int ni = 0; ni < 4; ++ni) {
-          dmma(cr[mi][ni][0], cr[mi][ni][1], a[mi].x, b[ni].x);
-          dmma(cr[mi][ni][0], cr[mi][ni][1], nai, b[ni].y);
-          dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].x, b[ni].y);
-          dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].y, b[ni].x);
+        for (int ni = 0; ni < NI; ++ni) bs[ni] = b[ni].x + b[ni].y;
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi) {
+          const double as = a[mi].x + a[mi].y;
+#pragma unroll
+          for (int ni = 0; ni < NI; ++ni) {
+            dmma(cr[mi][ni][0], cr[mi][ni][1], a[mi].x, b[ni].x);
+            dmma(c2[M3 ? mi : 0][M3 ? ni : 0][0], c2[M3 ? mi : 0][M3 ? ni : 0][1], a[mi].y, b[ni].y);
+            dmma(ci[mi][ni][0], ci[mi][ni][1], as, bs[ni]);
+          }
+        }
+      } else {
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi) {
+          const double nai = -a[mi].y;
+#pragma unroll
+          for (int ni = 0; ni < NI; ++ni) {
+            dmma(cr[mi][ni][0], cr[mi][ni][1], a[mi].x, b[ni].x);
+            dmma(cr[mi][ni][0], cr[mi][ni][1], nai, b[ni].y);
+            dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].x, b[ni].y);
+            dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].y, b[ni].x);
+          }
         }
       }
     }
@@ -176,41 +205,46 @@ __global__ void __launch_bounds__(NT) zgemm_kernel(const GemmDesc g) {
     if (row >= g.M) continue;
     // all eight C loads of this row first (independent, in flight together), then the eight stores: a load placed
     // after a store to C could not be hoisted above it
-    cplx old[4][2];
+    cplx old[NI][2];
 #pragma unroll
-    for (int ni = 0; ni < 4; ++ni) {
+    for (int ni = 0; ni < NI; ++ni) {
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const int col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
+        const int col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
         old[ni][j] = cmake(0.0, 0.0);
         if (has_beta && col < g.N && !(lower && col > row)) old[ni][j] = C[(size_t)row + (size_t)col * g.ldc];
       }
     }
 #pragma unroll
-    for (int ni = 0; ni < 4; ++ni) {
+    for (int ni = 0; ni < NI; ++ni) {
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const int col = n0 + wn * 32 + ni * 8 + (lane & 3) * 2 + j;
+        const int col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
         if (col >= g.N || (lower && col > row)) continue;
-        cplx v = cmul(g.alpha, cmake(cr[mi][ni][j], ci[mi][ni][j]));
+        cplx acc = cmake(cr[mi][ni][j], ci[mi][ni][j]);
+        if (M3) {
+          const double t2 = c2[M3 ? mi : 0][M3 ? ni : 0][j];
+          acc = cmake(cr[mi][ni][j] - t2, ci[mi][ni][j] - cr[mi][ni][j] - t2);
+        }
+        cplx v = cmul(g.alpha, acc);
         if (has_beta) v = cadd(v, cmul(g.beta, old[ni][j]));
         C[(size_t)row + (size_t)col * g.ldc] = v;
       }
     }
   }
 }
-template <int OPA, int OPB, int HERM, int BM, int BN>
+template <int OPA, int OPB, int HERM, int BM, int BN, int M3 = 0>
 void launch_one(const GemmDesc &g, cudaStream_t s) {
   constexpr size_t smem = smem_bytes<BM, BN>();
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN, M3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_done = true;
   }
   const int tm = (g.M + BM - 1) / BM, zz = g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1);
   dim3 grid(tm * zz, (g.N + BN - 1) / BN, 1);
-  if (BM == BN && (g.flags & BS_GEMM_LOWER_ONLY)) grid = dim3((tm * (tm + 1) / 2) * zz, 1, 1);  // requires M == N
-  zgemm_kernel<OPA, OPB, HERM, BM, BN><<<grid, NT, smem, s>>>(g);
+  if (g.flags & BS_GEMM_LOWER_ONLY) grid = dim3((BM / BN) * (tm * (tm + 1) / 2) * zz, 1, 1);  // requires M == N
+  zgemm_kernel<OPA, OPB, HERM, BM, BN, M3><<<grid, NT, smem, s>>>(g);
 }
 }  // namespace
 
@@ -222,13 +256,16 @@ void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   KScope ks(g.kclass ? g.kclass : KC_OTHER, work, s);
   const bool narrow = g.N <= 32 && g.M > 64 && g.opB == 0 && g.opA == 0 &&
                       !(g.flags & (BS_GEMM_KLO_COL | BS_GEMM_KHI_COL | BS_GEMM_KLO_ROW | BS_GEMM_KHI_ROW));
+  const bool m3 = g.kclass == KC_GEMM_HEMM || g.kclass == KC_GEMM_TRIDIAG;
   if (g.flags & BS_GEMM_A_HERM_LOWER) {  // requires opA == 0, opB == 0, K == M
-    if (narrow) launch_one<0, 0, 1, 128, 32>(g, s);
+    if (narrow && m3) launch_one<0, 0, 1, 64, 32, 1>(g, s);
+    else if (narrow) launch_one<0, 0, 1, 128, 32>(g, s);
     else launch_one<0, 0, 1, 64, 64>(g, s);
     return;
   }
   if (narrow) { launch_one<0, 0, 0, 128, 32>(g, s); return; }
   if (g.opA == 0 && g.opB == 0) launch_one<0, 0, 0, 64, 64>(g, s);
+  else if (g.opA == 0 && g.opB == 1 && m3) launch_one<0, 1, 0, 64, 32, 1>(g, s);
   else if (g.opA == 0 && g.opB == 1) launch_one<0, 1, 0, 64, 64>(g, s);
   else if (g.opA == 1 && g.opB == 0) launch_one<1, 0, 0, 64, 64>(g, s);
   else launch_one<1, 1, 0, 64, 64>(g, s);

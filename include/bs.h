@@ -177,7 +177,9 @@ const char *bs_last_error(void); /* thread-local, valid until the next call on t
 
 /* ---- diagnostics: the dense building blocks, exposed so that tests can check them in isolation ------------------- */
 /* C = alpha op(A) op(B) + beta C on DEVICE column-major complex128 arrays; op: 0 = none, 1 = conjugate transpose.
- * flags: see DESIGN.md section 5 (BS_GEMM_*).  batch >= 1 matrices with the given element strides. */
+ * flags: see DESIGN.md section 5 (BS_GEMM_*).  batch >= 1 matrices with the given element strides.  The complex
+ * product is the three-multiplication form (norm-wise error bound, not component-wise).  C must not overlap A or B,
+ * except C == A with opA = 0, opB = 1, N <= 64, flags = 0 (in-place right multiplication by a small block). */
 bs_status bs_zgemm(int32_t opA, int32_t opB, int32_t M, int32_t N, int32_t K, const double alpha[2], const void *A,
                    int32_t lda, int64_t strideA, const void *B, int32_t ldb, int64_t strideB, const double beta[2],
                    void *C, int32_t ldc, int64_t strideC, int32_t batch, int32_t flags, void *stream);

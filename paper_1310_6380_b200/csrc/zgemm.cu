@@ -1,15 +1,17 @@
 // Batched complex128 GEMM on the FP64 tensor pipe (mma.sync m8n8k4 f64 -> DMMA on sm_100a; tcgen05 has no f64 kind).
-// C = alpha op(A) op(B) + beta C, column-major interleaved complex.  A complex product is four real DMMAs on the
-// (re,im) parts kept interleaved in shared memory (one LDS.128 fetches both).  DESIGN.md section 5 (zgemm).
+// C = alpha op(A) op(B) + beta C, column-major interleaved complex, (re,im) kept interleaved in shared memory (one
+// LDS.128 fetches both).  The complex product is taken in its "3M" form, three real DMMAs per complex multiply-add
+// instead of four:  Re = ar br - ai bi,  Im = (ar + ai)(br + bi) - ar br - ai bi  (norm-wise backward stable; the
+// tolerance budget is in DESIGN.md section 5, zgemm).
 #include "bs_internal.cuh"
 
 namespace bsk {
 
 namespace {
 constexpr int BK = 8, STAGES = 4;
-constexpr int NT = 256;
-// CTA tile BM x BN, 8 warps of 16 x 32 each: (BM, BN) = (64, 64) [4 x 2 warps] or (128, 32) [8 x 1 warps, for N <= 32:
-// the HEMM and the compact-WY products of the band reduction].  Row strides are padded by 2 (conflict-free fragments).
+// CTA tile BM x BN = 32 x 32, four warps of 16 x 16 each (three accumulator sets of 2 x 2 m8n8 tiles = 48 registers),
+// four CTAs per SM: small CTAs in different phases hide each other's prologue and read-modify-write epilogue, which
+// is what the K = 2b = 64 rank-2b updates consist of.  Row strides are padded by 2 (conflict-free fragments).
 template <int BM, int BN>
 constexpr size_t smem_bytes() { return (size_t)STAGES * BK * ((BM + 2) + (BN + 2)) * sizeof(cplx); }
 
@@ -31,12 +33,9 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 
 // HERM = 1: A is an M x M Hermitian matrix of which only the LOWER triangle is valid (K == M, OPA == 0):
 //   op(A)[m][k] = A[m][k] for m > k, Re A[m][m] for m == k, conj(A[k][m]) for m < k  (the HEMM of the band reduction).
-// M3 = 1: the "3M" form of the complex product, three real DMMAs per complex multiply-add instead of four:
-//   Re = ar br - ai bi,  Im = (ar + ai)(br + bi) - ar br - ai bi   (norm-wise stable)
-//         with three accumulator sets the warp tile shrinks to 16 x 16 (CTA tile 64 x 32).
-template <int OPA, int OPB, int HERM, int BM, int BN, int M3>
-__global__ void __launch_bounds__(NT, 2) zgemm_kernel(const GemmDesc g) {
-  constexpr int NI = M3 ? 2 : 4;                                // 8-column sub-tiles per warp
+template <int OPA, int OPB, int HERM, int BM, int BN, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) zgemm_kernel(const GemmDesc g) {
+  constexpr int NI = 2;                                         // 8-column sub-tiles per warp
   constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / 16;  // WMN warps along m, (NT / 32) / WMN along n
   static_assert((BM / 16) * (BN / (8 * NI)) == NT / 32, "warps of 16 x 8 NI");
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -125,16 +124,13 @@ __global__ void __launch_bounds__(NT, 2) zgemm_kernel(const GemmDesc g) {
       }
     }
   }
-  // M3 == 0: cr = Re, ci = Im.  M3 == 1: cr = sum ar br, ci = sum (ar + ai)(br + bi), c2 = sum ai bi.
-  double cr[2][NI][2], ci[2][NI][2], c2[M3 ? 2 : 1][M3 ? NI : 1][2];
+  // c1 = sum ar br, c2 = sum ai bi, c3 = sum (ar + ai)(br + bi)
+  double c1[2][NI][2], c2[2][NI][2], c3[2][NI][2];
 #pragma unroll
   for (int i = 0; i < 2; ++i)
 #pragma unroll
-    for (int j = 0; j < NI; ++j) cr[i][j][0] = cr[i][j][1] = ci[i][j][0] = ci[i][j][1] = 0.0;
-#pragma unroll
-  for (int i = 0; i < (M3 ? 2 : 1); ++i)
-#pragma unroll
-    for (int j = 0; j < (M3 ? NI : 1); ++j) c2[i][j][0] = c2[i][j][1] = 0.0;
+    for (int j = 0; j < NI; ++j)
+      c1[i][j][0] = c1[i][j][1] = c2[i][j][0] = c2[i][j][1] = c3[i][j][0] = c3[i][j][1] = 0.0;
 
 #pragma unroll
   for (int s = 0; s < STAGES - 1; ++s) {
@@ -165,32 +161,17 @@ __global__ void __launch_bounds__(NT, 2) zgemm_kernel(const GemmDesc g) {
         b[ni] = Bs[st][kk + (lane & 3)][wn * (8 * NI) + ni * 8 + (lane >> 2)];
         if (OPB) b[ni].y = -b[ni].y;
       }
+      double bs[NI];
 #pragma unroll
-      if (M3) {
-        double bs[NI];
+      for (int ni = 0; ni < NI; ++ni) bs[ni] = b[ni].x + b[ni].y;
 #pragma unroll
-        for (int ni = 0; ni < NI; ++ni) bs[ni] = b[ni].x + b[ni].y;
+      for (int mi = 0; mi < 2; ++mi) {
+        const double as = a[mi].x + a[mi].y;
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi) {
-          const double as = a[mi].x + a[mi].y;
-#pragma unroll
-          for (int ni = 0; ni < NI; ++ni) {
-            dmma(cr[mi][ni][0], cr[mi][ni][1], a[mi].x, b[ni].x);
-            dmma(c2[M3 ? mi : 0][M3 ? ni : 0][0], c2[M3 ? mi : 0][M3 ? ni : 0][1], a[mi].y, b[ni].y);
-            dmma(ci[mi][ni][0], ci[mi][ni][1], as, bs[ni]);
-          }
-        }
-      } else {
-#pragma unroll
-        for (int mi = 0; mi < 2; ++mi) {
-          const double nai = -a[mi].y;
-#pragma unroll
-          for (int ni = 0; ni < NI; ++ni) {
-            dmma(cr[mi][ni][0], cr[mi][ni][1], a[mi].x, b[ni].x);
-            dmma(cr[mi][ni][0], cr[mi][ni][1], nai, b[ni].y);
-            dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].x, b[ni].y);
-            dmma(ci[mi][ni][0], ci[mi][ni][1], a[mi].y, b[ni].x);
-          }
+        for (int ni = 0; ni < NI; ++ni) {
+          dmma(c1[mi][ni][0], c1[mi][ni][1], a[mi].x, b[ni].x);
+          dmma(c2[mi][ni][0], c2[mi][ni][1], a[mi].y, b[ni].y);
+          dmma(c3[mi][ni][0], c3[mi][ni][1], as, bs[ni]);
         }
       }
     }
@@ -221,30 +202,26 @@ __global__ void __launch_bounds__(NT, 2) zgemm_kernel(const GemmDesc g) {
       for (int j = 0; j < 2; ++j) {
         const int col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
         if (col >= g.N || (lower && col > row)) continue;
-        cplx acc = cmake(cr[mi][ni][j], ci[mi][ni][j]);
-        if (M3) {
-          const double t2 = c2[M3 ? mi : 0][M3 ? ni : 0][j];
-          acc = cmake(cr[mi][ni][j] - t2, ci[mi][ni][j] - cr[mi][ni][j] - t2);
-        }
-        cplx v = cmul(g.alpha, acc);
+        const double t1 = c1[mi][ni][j], t2 = c2[mi][ni][j];
+        cplx v = cmul(g.alpha, cmake(t1 - t2, c3[mi][ni][j] - t1 - t2));
         if (has_beta) v = cadd(v, cmul(g.beta, old[ni][j]));
         C[(size_t)row + (size_t)col * g.ldc] = v;
       }
     }
   }
 }
-template <int OPA, int OPB, int HERM, int BM, int BN, int M3 = 0>
+template <int OPA, int OPB, int HERM, int BM = 32, int BN = 32, int NT = 128>
 void launch_one(const GemmDesc &g, cudaStream_t s) {
   constexpr size_t smem = smem_bytes<BM, BN>();
   static bool attr_done = false;
   if (!attr_done) {
-    cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN, M3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_done = true;
   }
   const int tm = (g.M + BM - 1) / BM, zz = g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1);
   dim3 grid(tm * zz, (g.N + BN - 1) / BN, 1);
   if (g.flags & BS_GEMM_LOWER_ONLY) grid = dim3((BM / BN) * (tm * (tm + 1) / 2) * zz, 1, 1);  // requires M == N
-  zgemm_kernel<OPA, OPB, HERM, BM, BN, M3><<<grid, NT, smem, s>>>(g);
+  zgemm_kernel<OPA, OPB, HERM, BM, BN, NT><<<grid, NT, smem, s>>>(g);
 }
 }  // namespace
 
@@ -254,21 +231,18 @@ void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   work *= (g.flags & BS_GEMM_LOWER_ONLY) ? 0.5 * g.M * (g.M + 1.0) : (double)g.M * g.N;
   if (g.flags & (BS_GEMM_KLO_ROW | BS_GEMM_KHI_ROW | BS_GEMM_KLO_COL | BS_GEMM_KHI_COL)) work *= 0.5;
   KScope ks(g.kclass ? g.kclass : KC_OTHER, work, s);
-  const bool narrow = g.N <= 32 && g.M > 64 && g.opB == 0 && g.opA == 0 &&
-                      !(g.flags & (BS_GEMM_KLO_COL | BS_GEMM_KHI_COL | BS_GEMM_KLO_ROW | BS_GEMM_KHI_ROW));
-  const bool m3 = g.kclass == KC_GEMM_HEMM || g.kclass == KC_GEMM_TRIDIAG;
-  if (g.flags & BS_GEMM_A_HERM_LOWER) {  // requires opA == 0, opB == 0, K == M
-    if (narrow && m3) launch_one<0, 0, 1, 64, 32, 1>(g, s);
-    else if (narrow) launch_one<0, 0, 1, 128, 32>(g, s);
-    else launch_one<0, 0, 1, 64, 64>(g, s);
+  // C aliasing A (the panel solve of the Cholesky factorisation, A21 <- A21 inv(L11)^H): a CTA must own complete rows,
+  // i.e. one column tile only; 16 x 64 tiles (1 x 4 warps) serve N <= 64
+  if (g.C.bases == g.A.bases && g.C.single == g.A.single && g.C.off == g.A.off && g.opA == 0 && g.opB == 1 &&
+      g.N <= 64 && g.flags == 0) {
+    launch_one<0, 1, 0, 16, 64>(g, s);
     return;
   }
-  if (narrow) { launch_one<0, 0, 0, 128, 32>(g, s); return; }
-  if (g.opA == 0 && g.opB == 0) launch_one<0, 0, 0, 64, 64>(g, s);
-  else if (g.opA == 0 && g.opB == 1 && m3) launch_one<0, 1, 0, 64, 32, 1>(g, s);
-  else if (g.opA == 0 && g.opB == 1) launch_one<0, 1, 0, 64, 64>(g, s);
-  else if (g.opA == 1 && g.opB == 0) launch_one<1, 0, 0, 64, 64>(g, s);
-  else launch_one<1, 1, 0, 64, 64>(g, s);
+  if (g.flags & BS_GEMM_A_HERM_LOWER) { launch_one<0, 0, 1>(g, s); return; }  // requires opA == opB == 0, K == M
+  if (g.opA == 0 && g.opB == 0) launch_one<0, 0, 0>(g, s);
+  else if (g.opA == 0 && g.opB == 1) launch_one<0, 1, 0>(g, s);
+  else if (g.opA == 1 && g.opB == 0) launch_one<1, 0, 0>(g, s);
+  else launch_one<1, 1, 0>(g, s);
 }
 
 }  // namespace bsk

@@ -34,7 +34,7 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 // HERM = 1: A is an M x M Hermitian matrix of which only the LOWER triangle is valid (K == M, OPA == 0):
 //   op(A)[m][k] = A[m][k] for m > k, Re A[m][m] for m == k, conj(A[k][m]) for m < k  (the HEMM of the band reduction).
 template <int OPA, int OPB, int HERM, int BM, int BN, int NT>
-__global__ void __launch_bounds__(NT, 512 / NT) zgemm_kernel(const GemmDesc g) {
+__global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
   constexpr int NI = 2;                                         // 8-column sub-tiles per warp
   constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / 16;  // WMN warps along m, (NT / 32) / WMN along n
   static_assert((BM / 16) * (BN / (8 * NI)) == NT / 32, "warps of 16 x 8 NI");
@@ -86,29 +86,72 @@ __global__ void __launch_bounds__(NT, 512 / NT) zgemm_kernel(const GemmDesc g) {
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
   const int wm = warp % WMN, wn = warp / WMN;  // warp tile 16 x 32
 
+  // Per-thread load slots: RA + RB 16-byte elements per k-tile.  Source pointers are set up once and advanced by a
+  // constant per k-tile (load_tile is called for kt = 0, 1, 2, ... in order); the address arithmetic of a k-tile is a
+  // few instructions, not a chain in front of the tensor work.  HERM keeps two sets for A: the direct one for k-tiles
+  // below the diagonal, the transposed one above it; the few k-tiles that cross it compute their addresses in place.
+  constexpr int RA = BM * BK / NT, RB = (BN * BK + NT - 1) / NT;
+  static_assert(RA >= 1, "A slots");
+  constexpr bool TRA = OPA != 0;  // the only set reads transposed positions
+  const cplx *pa[RA], *pat[HERM ? RA : 1], *pb[RB];
+  int ka[RA], kat[HERM ? RA : 1], kb[RB];
+  bool va[RA], vat[HERM ? RA : 1], vb[RB];
+  unsigned sa[RA], sat[HERM ? RA : 1], sb[RB];
+  const unsigned as_base = (unsigned)__cvta_generic_to_shared(&As[0][0][0]);
+  const unsigned bs_base = (unsigned)__cvta_generic_to_shared(&Bs[0][0][0]);
+#pragma unroll
+  for (int r = 0; r < RA; ++r) {
+    int m, k;
+    if (!TRA) { m = t % BM; k = t / BM + (NT / BM) * r; } else { k = t % BK; m = t / BK + (NT / BK) * r; }
+    ka[r] = k; va[r] = m0 + m < g.M; sa[r] = as_base + (unsigned)((k * LDA_S + m) * sizeof(cplx));
+    pa[r] = !TRA ? A + (size_t)(m0 + m) + (size_t)(klo + k) * g.lda : A + (size_t)(klo + k) + (size_t)(m0 + m) * g.lda;
+    if (HERM) {
+      k = t % BK; m = t / BK + (NT / BK) * r;
+      kat[r] = k; vat[r] = m0 + m < g.M; sat[r] = as_base + (unsigned)((k * LDA_S + m) * sizeof(cplx));
+      pat[r] = A + (size_t)(klo + k) + (size_t)(m0 + m) * g.lda;
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < RB; ++r) {
+    int n, k;
+    if (OPB == 0) { k = t % BK; n = t / BK + (NT / BK) * r; } else { n = t % BN; k = t / BN + (NT / BN) * r; }
+    kb[r] = k; vb[r] = (n0 + n < g.N) && !(BN * BK < NT && t >= BN * BK);
+    sb[r] = bs_base + (unsigned)((k * LDB_S + n) * sizeof(cplx));
+    pb[r] = OPB == 0 ? B + (size_t)(klo + k) + (size_t)(n0 + n) * g.ldb : B + (size_t)(n0 + n) + (size_t)(klo + k) * g.ldb;
+  }
+  const size_t step_a = !TRA ? (size_t)BK * g.lda : (size_t)BK, step_b = OPB == 0 ? (size_t)BK : (size_t)BK * g.ldb;
+  auto cp16 = [](unsigned dst, const void *src, bool ok) {
+    const int sz = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(sz));
+  };
   auto load_tile = [&](int kt, int stage) {
     const int k0 = klo + kt * BK;
+    const unsigned oa = (unsigned)(stage * BK * LDA_S * sizeof(cplx)), ob = (unsigned)(stage * BK * LDB_S * sizeof(cplx));
+    const bool above = HERM && k0 >= m0 + BM - 1;                 // the whole k-tile lies above the diagonal
+    const bool cross = HERM && !above && k0 + BK - 1 > m0;        // it crosses the diagonal: per element
 #pragma unroll
-    for (int r = 0; r < BM * BK / NT; ++r) {
-      int m, k;
-      bool tr = OPA != 0;                                  // read the element from its transposed position
-      if (HERM && k0 >= m0 + BM - 1) tr = true;            // the whole k-tile lies above the diagonal
-      if (!tr) { m = t % BM; k = t / BM + (NT / BM) * r; } else { k = t & 7; m = (t >> 3) + (NT / 8) * r; }
-      if (HERM && !tr && k0 + BK - 1 > m0) tr = (k0 + k > m0 + m);   // tile crossing the diagonal: per element
-      const bool ok = (m0 + m < g.M) && (k0 + k < khi);
-      const cplx *src = !tr ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
-                            : A + (size_t)(k0 + k) + (size_t)(m0 + m) * g.lda;
-      cp_async16(&As[stage][k][m], ok ? src : A, ok);
+    for (int r = 0; r < RA; ++r) {
+      if (cross) {
+        const int m = t % BM, k = t / BM + (NT / BM) * r;
+        const bool tr = k0 + k > m0 + m, ok = (m0 + m < g.M) && (k0 + k < khi);
+        const cplx *src = !tr ? A + (size_t)(m0 + m) + (size_t)(k0 + k) * g.lda
+                              : A + (size_t)(k0 + k) + (size_t)(m0 + m) * g.lda;
+        cp16(sa[r] + oa, ok ? src : A, ok);
+      } else if (above) {
+        const bool ok = vat[r] && (k0 + kat[r] < khi);
+        cp16(sat[r] + oa, ok ? pat[r] : A, ok);
+      } else {
+        const bool ok = va[r] && (k0 + ka[r] < khi);
+        cp16(sa[r] + oa, ok ? pa[r] : A, ok);
+      }
+      pa[r] += step_a;
+      if (HERM) pat[r] += BK;
     }
 #pragma unroll
-    for (int r = 0; r < (BN * BK + NT - 1) / NT; ++r) {
-      int n, k;
-      if (OPB == 0) { k = t & 7; n = (t >> 3) + (NT / 8) * r; } else { n = t % BN; k = t / BN + (NT / BN) * r; }
-      if (BN * BK < NT && t >= BN * BK) break;
-      const bool ok = (n0 + n < g.N) && (k0 + k < khi);
-      const cplx *src = OPB == 0 ? B + (size_t)(k0 + k) + (size_t)(n0 + n) * g.ldb
-                                 : B + (size_t)(n0 + n) + (size_t)(k0 + k) * g.ldb;
-      cp_async16(&Bs[stage][k][n], ok ? src : B, ok);
+    for (int r = 0; r < RB; ++r) {
+      const bool ok = vb[r] && (k0 + kb[r] < khi);
+      cp16(sb[r] + ob, ok ? pb[r] : B, ok);
+      pb[r] += step_b;
     }
   };
 
@@ -140,15 +183,20 @@ __global__ void __launch_bounds__(NT, 512 / NT) zgemm_kernel(const GemmDesc g) {
   for (int kt = 0; kt < nkt; ++kt) {
     cp_wait<STAGES - 2>();
     __syncthreads();
-    if (kt + STAGES - 1 < nkt) load_tile(kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
-    cp_commit();
     const int st = kt % STAGES;
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
       cplx a[2], b[NI];
 #pragma unroll
+      for (int mi = 0; mi < 2; ++mi) a[mi] = As[st][kk + (lane & 3)][wm * 16 + mi * 8 + (lane >> 2)];
+#pragma unroll
+      for (int ni = 0; ni < NI; ++ni) b[ni] = Bs[st][kk + (lane & 3)][wn * (8 * NI) + ni * 8 + (lane >> 2)];
+      if (kk == 0) {  // the fragment loads of this k-tile are in flight: now refill the stage read one k-tile ago
+        if (kt + STAGES - 1 < nkt) load_tile(kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
+        cp_commit();
+      }
+#pragma unroll
       for (int mi = 0; mi < 2; ++mi) {
-        a[mi] = As[st][kk + (lane & 3)][wm * 16 + mi * 8 + (lane >> 2)];
         if (OPA) a[mi].y = -a[mi].y;
         if (HERM) {
           const int mg = m0 + wm * 16 + mi * 8 + (lane >> 2), kg = klo + kt * BK + kk + (lane & 3);
@@ -157,10 +205,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) zgemm_kernel(const GemmDesc g) {
         }
       }
 #pragma unroll
-      for (int ni = 0; ni < NI; ++ni) {
-        b[ni] = Bs[st][kk + (lane & 3)][wn * (8 * NI) + ni * 8 + (lane >> 2)];
+      for (int ni = 0; ni < NI; ++ni)
         if (OPB) b[ni].y = -b[ni].y;
-      }
       double bs[NI];
 #pragma unroll
       for (int ni = 0; ni < NI; ++ni) bs[ni] = b[ni].x + b[ni].y;
@@ -168,11 +214,11 @@ __global__ void __launch_bounds__(NT, 512 / NT) zgemm_kernel(const GemmDesc g) {
       for (int mi = 0; mi < 2; ++mi) {
         const double as = a[mi].x + a[mi].y;
 #pragma unroll
-        for (int ni = 0; ni < NI; ++ni) {
-          dmma(c1[mi][ni][0], c1[mi][ni][1], a[mi].x, b[ni].x);
-          dmma(c2[mi][ni][0], c2[mi][ni][1], a[mi].y, b[ni].y);
-          dmma(c3[mi][ni][0], c3[mi][ni][1], as, bs[ni]);
-        }
+        for (int ni = 0; ni < NI; ++ni) dmma(c1[mi][ni][0], c1[mi][ni][1], a[mi].x, b[ni].x);
+#pragma unroll
+        for (int ni = 0; ni < NI; ++ni) dmma(c2[mi][ni][0], c2[mi][ni][1], a[mi].y, b[ni].y);
+#pragma unroll
+        for (int ni = 0; ni < NI; ++ni) dmma(c3[mi][ni][0], c3[mi][ni][1], as, bs[ni]);
       }
     }
   }

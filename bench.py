@@ -263,27 +263,44 @@ def run_ours(args):
     units = nk * ncell * world * args.steps
     value = units / (ms_total * 1e-3)
     hbm_peak, hbm_src = measured_peaks()
-    # ---- roofline of the dominant kernel class (largest share of device time inside the timed region)
+    # ---- roofline of the dominant KERNEL: the timing classes are grouped by the __global__ function they launch (all
+    # DMMA GEMM classes are instantiations of zgemm_kernel, as in the ncu launch list under profiles/); the kernel with
+    # the largest share of device time inside the timed region is the dominant one.  Every kernel's own figures are
+    # listed under "by_kernel", the largest single launch (bulge chasing) included.
     tot_kernel_ms = sum(a[0] for a in kacc.values()) or 1.0
-    dom = max(kacc, key=lambda k: kacc[k][0])
-    ms_d, work_d, cnt_d = kacc[dom]
-    traffic = None
+    groups = {}
+    for k, a in kacc.items():
+        if not a[2]:
+            continue
+        gname = "zgemm_kernel" if k in TENSOR_CLASSES else k
+        gacc = groups.setdefault(gname, [0.0, 0.0, 0, []])
+        gacc[0] += a[0]; gacc[1] += a[1]; gacc[2] += a[2]; gacc[3].append(k)
+    tjson = {}
     tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(w.name, {}).get(dom)
-    if dom in TENSOR_CLASSES:
-        roof = {"bound": "tensor", "achieved": work_d / (ms_d * 1e9), "peak": dmma_peak, "unit": "TFLOP/s",
-                "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-only loop measured in this run by bs_fp64_peak; "
-                               "MEASURED_PEAKS.json has no FP64 entry"}
-    elif dom in HBM_CLASSES:
-        roof = {"bound": "hbm", "achieved": work_d / (ms_d * 1e6), "peak": hbm_peak, "unit": "GB/s", "peak_source": hbm_src}
-    else:
-        roof = {"bound": "alu", "achieved": work_d / (ms_d * 1e9) if work_d else None, "peak": dfma_peak, "unit": "TFLOP/s",
-                "peak_source": "FP64 DFMA register-only loop measured in this run by bs_fp64_peak"}
-    roof["frac"] = (roof["achieved"] / roof["peak"]) if roof["achieved"] else None
-    roof.update({"kernel": dom, "launches_per_step": cnt_d / args.steps, "avg_launch_ms": ms_d / max(cnt_d, 1),
-                 "share_of_kernel_time": ms_d / tot_kernel_ms, "traffic": traffic,
-                 "work_per_launch": work_d / max(cnt_d, 1)})
+        tjson = json.load(open(tpath)).get(w.name, {})
+
+    def roof_of(gname):
+        ms_d, work_d, cnt_d, classes = groups[gname]
+        if gname == "zgemm_kernel":
+            r = {"bound": "tensor", "achieved": work_d / (ms_d * 1e9), "peak": dmma_peak, "unit": "TFLOP/s",
+                 "peak_source": "FP64 DMMA (mma.sync m8n8k4) register-only loop measured in this run by bs_fp64_peak; "
+                                "MEASURED_PEAKS.json has no FP64 entry"}
+        elif gname in HBM_CLASSES:
+            r = {"bound": "hbm", "achieved": work_d / (ms_d * 1e6), "peak": hbm_peak, "unit": "GB/s", "peak_source": hbm_src}
+        else:
+            r = {"bound": "alu", "achieved": work_d / (ms_d * 1e9) if work_d else None, "peak": dfma_peak,
+                 "unit": "TFLOP/s", "peak_source": "FP64 DFMA register-only loop measured in this run by bs_fp64_peak"}
+        r["frac"] = (r["achieved"] / r["peak"]) if r["achieved"] else None
+        r.update({"kernel": gname, "classes": sorted(classes), "launches_per_step": cnt_d / args.steps,
+                  "avg_launch_ms": ms_d / max(cnt_d, 1), "share_of_kernel_time": ms_d / tot_kernel_ms,
+                  "traffic": tjson.get(gname), "work_per_launch": work_d / max(cnt_d, 1)})
+        return r
+
+    dom = max(groups, key=lambda k: groups[k][0])
+    roof = roof_of(dom)
+    roof["by_kernel"] = [{k: v for k, v in roof_of(gname).items() if k != "peak_source"}
+                         for gname in sorted(groups, key=lambda k: -groups[k][0])]
     n = 2 * w.N
     gemm_ms = sum(kacc[k][0] for k in TENSOR_CLASSES if k in kacc)
     gemm_fl = sum(kacc[k][1] for k in TENSOR_CLASSES if k in kacc)

@@ -15,10 +15,9 @@ constexpr int BK = 8, STAGES = 4;
 template <int BM, int BN>
 constexpr size_t smem_bytes() { return (size_t)STAGES * BK * ((BM + 2) + (BN + 2)) * sizeof(cplx); }
 
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, bool valid) {
-  const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
-  const int sz = valid ? 16 : 0;
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+__device__ __forceinline__ void cp16(unsigned dst, const void *src, bool ok) {  // dst: shared-space address
+  const int sz = ok ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(sz));
 }
 __device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
 template <int N>
@@ -120,10 +119,6 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
     pb[r] = OPB == 0 ? B + (size_t)(klo + k) + (size_t)(n0 + n) * g.ldb : B + (size_t)(n0 + n) + (size_t)(klo + k) * g.ldb;
   }
   const size_t step_a = !TRA ? (size_t)BK * g.lda : (size_t)BK, step_b = OPB == 0 ? (size_t)BK : (size_t)BK * g.ldb;
-  auto cp16 = [](unsigned dst, const void *src, bool ok) {
-    const int sz = ok ? 16 : 0;
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(sz));
-  };
   auto load_tile = [&](int kt, int stage) {
     const int k0 = klo + kt * BK;
     const unsigned oa = (unsigned)(stage * BK * LDA_S * sizeof(cplx)), ob = (unsigned)(stage * BK * LDB_S * sizeof(cplx));
@@ -167,7 +162,7 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
       }
     }
   }
-  // c1 = sum ar br, c2 = sum ai bi, c3 = sum (ar + ai)(br + bi)
+  // c1 = sum ar br, c2 = sum ai bi (stored imaginary parts), c3 = sum (ar +- ai)(br +- bi) (- where conjugated)
   double c1[2][NI][2], c2[2][NI][2], c3[2][NI][2];
 #pragma unroll
   for (int i = 0; i < 2; ++i)
@@ -195,24 +190,26 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
         if (kt + STAGES - 1 < nkt) load_tile(kt + STAGES - 1, (kt + STAGES - 1) % STAGES);
         cp_commit();
       }
+      // Conjugations cost no FP64-pipe instruction (the pipe DMMA runs on): a uniform conjugate of A or B only
+      // changes signs in the operand sums below and in the epilogue (SGN); the per-element one of HERM flips the
+      // sign bit with an integer operation.
+      if (HERM) {
 #pragma unroll
-      for (int mi = 0; mi < 2; ++mi) {
-        if (OPA) a[mi].y = -a[mi].y;
-        if (HERM) {
+        for (int mi = 0; mi < 2; ++mi) {
           const int mg = m0 + wm * 16 + mi * 8 + (lane >> 2), kg = klo + kt * BK + kk + (lane & 3);
-          if (kg > mg) a[mi].y = -a[mi].y;
-          else if (kg == mg) a[mi].y = 0.0;
+          int hi = __double2hiint(a[mi].y), lo = __double2loint(a[mi].y);
+          hi = kg > mg ? hi ^ (int)0x80000000 : hi;
+          hi = kg == mg ? 0 : hi;
+          lo = kg == mg ? 0 : lo;
+          a[mi].y = __hiloint2double(hi, lo);
         }
       }
-#pragma unroll
-      for (int ni = 0; ni < NI; ++ni)
-        if (OPB) b[ni].y = -b[ni].y;
       double bs[NI];
 #pragma unroll
-      for (int ni = 0; ni < NI; ++ni) bs[ni] = b[ni].x + b[ni].y;
+      for (int ni = 0; ni < NI; ++ni) bs[ni] = OPB ? b[ni].x - b[ni].y : b[ni].x + b[ni].y;
 #pragma unroll
       for (int mi = 0; mi < 2; ++mi) {
-        const double as = a[mi].x + a[mi].y;
+        const double as = OPA ? a[mi].x - a[mi].y : a[mi].x + a[mi].y;
 #pragma unroll
         for (int ni = 0; ni < NI; ++ni) dmma(c1[mi][ni][0], c1[mi][ni][1], a[mi].x, b[ni].x);
 #pragma unroll
@@ -248,7 +245,8 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
       for (int j = 0; j < 2; ++j) {
         const int col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
         if (col >= g.N || (lower && col > row)) continue;
-        const double t1 = c1[mi][ni][j], t2 = c2[mi][ni][j];
+        // c2 holds sum ai bi of the stored imaginary parts: SGN = -1 if exactly one operand is conjugated
+        const double t1 = c1[mi][ni][j], t2 = (OPA != OPB ? -1.0 : 1.0) * c2[mi][ni][j];
         cplx v = cmul(g.alpha, cmake(t1 - t2, c3[mi][ni][j] - t1 - t2));
         if (has_beta) v = cadd(v, cmul(g.beta, old[ni][j]));
         C[(size_t)row + (size_t)col * g.ldc] = v;

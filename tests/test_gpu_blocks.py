@@ -84,6 +84,52 @@ def test_zgemm_batched_lower_only(bs):
         assert np.array_equal(got[up], C0[b][up])      # the strict upper triangle is untouched
 
 
+def test_zgemm_3m_normwise_bound(bs):
+    # The kernel forms Im(ab) as (ar+ai)(br+bi) - ar br - ai bi (three multiplications, include/bs.h): the error of an
+    # entry is bounded norm-wise, c u K max|A| max|B|, also where real and imaginary parts differ by many orders of
+    # magnitude (there the small part is NOT accurate relative to itself: that is the documented trade).
+    import torch
+    rng = np.random.default_rng(2024)
+    M, N, K = 96, 80, 200
+    A = rng.normal(size=(M, K)) + 1e-9j * rng.normal(size=(M, K))     # nearly real
+    B = 1e-9 * rng.normal(size=(K, N)) + 1j * rng.normal(size=(K, N))  # nearly imaginary
+    ref = A @ B
+    dA, dB = to_dev(A), to_dev(B)
+    dC = torch.zeros(N, M, dtype=torch.complex128, device="cuda")
+    bs.bs_zgemm(0, 0, M, N, K, 1.0, dA, M, 0, dB, K, 0, 0.0, dC, M, 0)
+    torch.cuda.synchronize()
+    err = np.abs(from_dev(dC) - ref)
+    bound = 8 * np.finfo(float).eps * K * np.max(np.abs(A)) * np.max(np.abs(B))
+    assert np.max(err) <= bound
+    # exact cases: purely real times purely real has a zero imaginary part bit for bit (ai = bi = 0: T3 == T1)
+    Ar, Br = rng.normal(size=(M, K)) + 0j, rng.normal(size=(K, N)) + 0j
+    dC.zero_()
+    bs.bs_zgemm(0, 0, M, N, K, 1.0, to_dev(Ar), M, 0, to_dev(Br), K, 0, 0.0, dC, M, 0)
+    torch.cuda.synchronize()
+    got = from_dev(dC)
+    assert np.all(got.imag == 0.0)
+    assert np.max(np.abs(got.real - (Ar.real @ Br.real))) <= 1e-13 * K
+
+
+@pytest.mark.parametrize("batch", [1, 700])
+def test_zgemm_in_place_right_multiply(bs, batch):
+    # C == A (the panel solve A21 <- A21 inv(L11)^H of the Cholesky factorisation): a CTA must own complete rows of C.
+    # With many matrices in flight a tile that still reads what another tile has overwritten shows up here.
+    import torch
+    rng = np.random.default_rng(batch)
+    M, N = 161, 64
+    A = [rand_c(rng, M, N) for _ in range(min(batch, 4))]
+    Bm = rand_c(rng, N, N)
+    dA = torch.stack([to_dev(A[b % len(A)]) for b in range(batch)])
+    dB = to_dev(Bm)
+    bs.bs_zgemm(0, 1, M, N, N, 1.0, dA, M, M * N, dB, N, 0, 0.0, dA, M, M * N, batch)
+    torch.cuda.synchronize()
+    for b in (0, batch // 2, batch - 1):
+        ref = A[b % len(A)] @ Bm.conj().T
+        got = dA[b].cpu().numpy().T
+        assert np.max(np.abs(got - ref)) <= 1e-13 * N * np.max(np.abs(ref))
+
+
 @pytest.mark.parametrize("n", [17, 64, 100, 363, 450])
 def test_zpotrf_trtri(bs, n):
     import torch

@@ -271,22 +271,26 @@ __global__ void __launch_bounds__(NTHR) panel_qr_kernel(int n, int lda, int b, i
   }
 }
 
-// T (compact WY, forward columnwise: T[j][j] = tau_j, T[0:j, j] = -tau_j T[0:j,0:j] G[0:j, j]) and
-// M2 = -1/2 T^H S T.  SM per matrix: [G | S] (b x 2b, ld b) at 0; [M2; T] (2b x b, ld 2b) at 2 b^2; tau at 4 b^2.
-__global__ void __launch_bounds__(256) wy_small_kernel(int b, BatchRef SM, int inner) {
+// T (compact WY, forward columnwise: Q = H_1 .. H_b = I - V T V^H) and M2 = -1/2 T^H S T.
+// T^-1 = diag(1 / tau) + triu(G, 1) with G = V^H V, so T solves  (I + diag(tau) triu(G, 1)) T = diag(tau):  all b columns
+// at once by column-oriented back substitution, one barrier per row l = b-1 .. 0 and O(1) work per thread and step
+// (R: running right-hand sides; row l of T is final at step l: T[l, j] = tau_l R[l, j], then R[i, j] -= G[i, l] T[l, j]
+// for i < l).  tau_l = 0 (H_l = I) gives a zero row and column, as the forward recurrence does.
+// SM per matrix: [G | S] (b x 2b, ld b) at 0; [M2; T] (2b x b, ld 2b) at 2 b^2; tau at 4 b^2.
+__global__ void __launch_bounds__(1024) wy_small_kernel(int b, BatchRef SM, int inner) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *T = reinterpret_cast<cplx *>(smem_raw);  // b x b, T[i + j*b]
   cplx *S = T + b * b;                           // b x b
-  cplx *U = S + b * b;                           // b x b scratch
+  cplx *U = S + b * b;                           // b x b scratch: R during the substitution, then S T
   cplx *G = U + b * b;                           // b x b
+  cplx *taus = G + b * b;                        // b
   const int z = blockIdx.x, cell = z / inner, mi = z % inner;
   cplx *sm = batch_ptr(SM, cell, mi);
   const cplx *part = sm + (size_t)4 * b * b + 64;  // KS partial products [G | S], each b x 2b
-  const double *tau = reinterpret_cast<const double *>(sm + (size_t)4 * b * b);
   cplx *out = sm + (size_t)2 * b * b;
   const int t = threadIdx.x;
+  if (t < b) taus[t] = sm[(size_t)4 * b * b + t];
   for (int i = t; i < b * b; i += blockDim.x) {
-    T[i] = cmake(0.0, 0.0);
     cplx gs = cmake(0.0, 0.0), ss = cmake(0.0, 0.0);
     for (int k = 0; k < KS; ++k) {  // fixed order: deterministic
       gs = cadd(gs, part[(size_t)k * 2 * b * b + i]);
@@ -294,16 +298,18 @@ __global__ void __launch_bounds__(256) wy_small_kernel(int b, BatchRef SM, int i
     }
     G[i] = gs;
     S[i] = ss;
+    T[i] = cmake(0.0, 0.0);
+    U[i] = (i % b == i / b) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
   }
   __syncthreads();
-  for (int j = 0; j < b; ++j) {
-    const cplx tj = cmake(tau[2 * j], tau[2 * j + 1]);
-    if (t < j) {
-      cplx acc = cmake(0.0, 0.0);
-      for (int l = t; l < j; ++l) cfma(acc, T[t + l * b], G[l + j * b]);
-      T[t + j * b] = cmul(cmake(-tj.x, -tj.y), acc);
-    } else if (t == j) {
-      T[j + j * b] = tj;
+  for (int l = b - 1; l >= 0; --l) {
+    const cplx tl = taus[l];
+    for (int e = t; e < b * b; e += blockDim.x) {
+      const int i = e % b, j = e / b;
+      if (j < l || i > l) continue;
+      const cplx x = cmul(tl, U[l + j * b]);  // T[l, j]
+      if (i == l) T[e] = x;
+      else { cplx r = U[e]; cfms(r, G[i + l * b], x); U[e] = r; }
     }
     __syncthreads();
   }
@@ -355,7 +361,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
   if (!attr_done) {
     cudaFuncSetAttribute(panel_qr_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 140 * 1024);
     cudaFuncSetAttribute(panel_qr_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
-    cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 32 * 32 * (int)sizeof(cplx));
+    cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (4 * 32 * 32 + 32) * (int)sizeof(cplx));
     attr_done = true;
   }
   for (int c0 = 0; c0 + b < n - 1; c0 += b) {
@@ -392,7 +398,7 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     g.ksplit = 0; g.split_stride = 0;
     {
       KScope ks(KC_OTHER, 0.0, s);
-      wy_small_kernel<<<nmat, 256, 4 * b * b * sizeof(cplx), s>>>(b, SM, inner);
+      wy_small_kernel<<<nmat, b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
       ++launches;
     }
     // X = [V | Z] [M2; T]

@@ -152,7 +152,9 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
 
   // beta != 0: the C tile is read only in the epilogue; warm it into L2 now so that the read-modify-write does not
   // pay DRAM latency after the (short, K = 2b) main loop of the rank-2b updates
-  if (g.beta.x != 0.0 || g.beta.y != 0.0) {
+  // (beta == 1 needs neither: the update goes out as reductions, see the epilogue)
+  const bool accumulate = g.beta.x == 1.0 && g.beta.y == 0.0;
+  if ((g.beta.x != 0.0 || g.beta.y != 0.0) && !accumulate) {
 #pragma unroll
     for (int ni = 0; ni < NI; ++ni) {
 #pragma unroll
@@ -223,6 +225,29 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
 
   const bool has_beta = (g.beta.x != 0.0 || g.beta.y != 0.0);
   const bool lower = g.flags & BS_GEMM_LOWER_ONLY;
+  if (accumulate) {
+    // C += alpha A B: every entry receives exactly one addition per launch, sent as two fire-and-forget FP64
+    // reductions that L2 performs; no read of C, no latency in the epilogue (deterministic: one addend per entry)
+#pragma unroll
+    for (int mi = 0; mi < 2; ++mi) {
+      const int row = m0 + wm * 16 + mi * 8 + (lane >> 2);
+      if (row >= g.M) continue;
+#pragma unroll
+      for (int ni = 0; ni < NI; ++ni) {
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+          const int col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
+          if (col >= g.N || (lower && col > row)) continue;
+          const double t1 = c1[mi][ni][j], t2 = (OPA != OPB ? -1.0 : 1.0) * c2[mi][ni][j];
+          const cplx v = cmul(g.alpha, cmake(t1 - t2, c3[mi][ni][j] - t1 - t2));
+          double *dst = reinterpret_cast<double *>(C + (size_t)row + (size_t)col * g.ldc);
+          asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(dst), "d"(v.x) : "memory");
+          asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(dst + 1), "d"(v.y) : "memory");
+        }
+      }
+    }
+    return;
+  }
 #pragma unroll
   for (int mi = 0; mi < 2; ++mi) {
     const int row = m0 + wm * 16 + mi * 8 + (lane >> 2);

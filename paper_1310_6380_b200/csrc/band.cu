@@ -398,7 +398,8 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     g.ksplit = 0; g.split_stride = 0;
     {
       KScope ks(KC_OTHER, 0.0, s);
-      wy_small_kernel<<<nmat, b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
+      // few matrices: one thread per entry (latency); many: smaller CTAs, several per SM (throughput)
+      wy_small_kernel<<<nmat, nmat > 592 ? 256 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
       ++launches;
     }
     // X = [V | Z] [M2; T]

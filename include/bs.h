@@ -41,7 +41,9 @@ typedef enum {
 /* Options for bs_set_option. */
 typedef enum {
   BS_OPT_PENCIL_MODE = 0, /* 0 = BS_PENCIL_POLY (default), 1 = BS_PENCIL_DIRECT; see bs_bands */
-  BS_OPT_PANEL = 1,       /* two-stage: band width b in {8, 16, 32} (default 32); one-stage: panel width 4..32, multiple of 4 */
+  BS_OPT_PANEL = 1,       /* two-stage: band width b in {8, 16, 32}; one-stage: panel width 4..32, multiple of 4.
+                             0 (default) = automatic: 16 where the whole band then fits in shared memory in stage 2
+                             (2N <= 353), else 32 */
   BS_OPT_TIMING = 2       /* 1 = CUDA events around the stages (bs_get_timings); 2 = also around every kernel launch,
                              summed per kernel class (bs_get_kernel_timings).  Both add a final stream synchronise. */
 } bs_option;

@@ -36,7 +36,7 @@ constexpr double kTwoPi = 6.283185307179586476925286766559;
 
 // Offsets (complex128 elements, each region 256-byte aligned) inside one cell's workspace.
 struct Layout {
-  int Mt = -1, N = 0, nk = 0, mode = 0, nb = 32;
+  int Mt = -1, N = 0, nk = 0, mode = 0, nb = 0;
   long long table, Phi, R, Lf, X, tmp, dinv, Y, LR, XR, tmpR, dinvR, kvecA, Coef, Tb, kvecK, Kk, Ak, VW, P, SM, AB;
   long long vw_stride, sm_stride, ab_stride;
   long long total;  // elements
@@ -44,10 +44,15 @@ struct Layout {
 
 long long align16(long long x) { return (x + 15) & ~15LL; }
 int band_width(int nb) { return nb >= 32 ? 32 : (nb >= 16 ? 16 : 8); }  // two-stage band width from BS_OPT_PANEL
+// BS_OPT_PANEL = 0 (default): band width 16 whenever the whole band then stays in shared memory during stage 2 (n <= 353:
+// no streaming, twelve sweeps in flight), otherwise 32 (the DMMA GEMMs of stage 1 want the wider panels).  Measured,
+// DESIGN.md section 5.  The choice depends on n only, so a batch and its members take the same path.
+int auto_band_width(int n) { return bsk::bulge_band_resident(n, 16) ? 16 : 32; }
 
-Layout make_layout(int Mt, int nk, int mode, int nb) {
+Layout make_layout(int Mt, int nk, int mode, int nb_opt) {
+  const int nb = nb_opt > 0 ? nb_opt : 32;  // automatic band width: sized for the widest
   Layout L;
-  L.Mt = Mt; L.nk = nk; L.mode = mode; L.nb = nb;
+  L.Mt = Mt; L.nk = nk; L.mode = mode; L.nb = nb_opt;
   const long long W = 2 * Mt + 1, N = W * W, n3 = 3 * N, n2 = 2 * N, Lt = 4 * Mt + 1;
   L.N = (int)N;
   long long o = 0;
@@ -94,7 +99,7 @@ struct bs_cell {
   int *d_ephase = nullptr;
   bsk::Geometry geo;
   bsk::Geometry *d_geo = nullptr;  // [1]
-  int mode = BS_PENCIL_POLY, nb = 32, timing = 0, algo = BS_TRIDIAG_TWO_STAGE, quad = BS_ASSEMBLY_EXACT;
+  int mode = BS_PENCIL_POLY, nb = 0, timing = 0, algo = BS_TRIDIAG_TWO_STAGE, quad = BS_ASSEMBLY_EXACT;
   void *ws = nullptr;
   size_t ws_bytes = 0;
   Layout lay;            // layout of the last bs_assemble (lay.Mt < 0: not assembled)
@@ -334,7 +339,8 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       c->mode = value;
       return BS_OK;
     case BS_OPT_PANEL:
-      if (value < 4 || value > 32 || value % 4) return fail(BS_ERR_ARG, "bs_set_option: panel must be 4..32, multiple of 4");
+      if (value != 0 && (value < 4 || value > 32 || value % 4))
+        return fail(BS_ERR_ARG, "bs_set_option: panel must be 0 (automatic) or 4..32, multiple of 4");
       if (c->nb != value) c->assembled = false;
       c->nb = value;
       return BS_OK;
@@ -721,12 +727,12 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   }
   tick(lead, 1, s);
   if (lead->algo == BS_TRIDIAG_ONE_STAGE) {
-    nl += bsk::launch_tridiag(n2, n2, lead->nb, R(L.Ak, mat), R(L.VW, L.vw_stride),
+    nl += bsk::launch_tridiag(n2, n2, lead->nb > 0 ? lead->nb : 32, R(L.Ak, mat), R(L.VW, L.vw_stride),
                               R(L.P, (long long)bsk::tridiag_p_elems(n2)), d, e, scal, ncells, nk, s);  // S6
   } else if (n2 <= bsk::tridiag_small_max_n()) {
     bsk::launch_tridiag_small(n2, n2, R(L.Ak, mat), d, e, ncells, nk, s); ++nl;                        // S6, matrix in shared memory
   } else {
-    const int bw = band_width(lead->nb);
+    const int bw = lead->nb > 0 ? band_width(lead->nb) : auto_band_width(n2);
     nl += bsk::launch_sy2sb(n2, n2, bw, R(L.Ak, mat), R(L.VW, L.vw_stride), R(L.SM, L.sm_stride), R(L.AB, L.ab_stride),
                             ncells, nk, s);                                                             // S6 stage 1
     bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s); ++nl;                         // S6 stage 2

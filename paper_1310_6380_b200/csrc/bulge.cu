@@ -382,15 +382,24 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
   }
 }
 
+constexpr size_t BULGE_MAX_SMEM = 226 * 1024;
+constexpr int bulge_gmax(int B, int NQ) {  // teams per CTA (G * TT + 128 I/O threads)
+  return min(12, ((NQ * B >= 128 ? 512 : 1024) - NIO * 32) / (NQ * B));
+}
+constexpr bool bulge_fits(int n, int B, int NQ) {  // the whole band (n columns of 2B entries) beside the team scratch
+  return (size_t)n * 2 * B * sizeof(cplx) + (size_t)bulge_gmax(B, NQ) * (4 + 3 * NQ) * B * sizeof(cplx) +
+             (size_t)n * sizeof(int) <= BULGE_MAX_SMEM;
+}
+
 template <int B, int NQ>
 void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inner, cudaStream_t s) {
   constexpr int LD = 2 * B, TT = NQ * B;
   const size_t colbytes = (size_t)LD * sizeof(cplx);
-  const int gmax = min(12, ((TT >= 128 ? 512 : 1024) - NIO * 32) / TT);  // teams per CTA (G * TT + 128 I/O threads)
+  const int gmax = bulge_gmax(B, NQ);
   const size_t team_bytes = (size_t)(4 + 3 * NQ) * B * sizeof(cplx);
-  const size_t max_smem = 226 * 1024;
+  const size_t max_smem = BULGE_MAX_SMEM;
   int G, Wc;
-  if ((size_t)n * colbytes + gmax * team_bytes + (size_t)n * sizeof(int) <= max_smem) {  // whole band resident
+  if (bulge_fits(n, B, NQ)) {  // whole band resident
     Wc = max(n, 2 * B + 8);  // never fewer than a block pair of columns: the masked loads of a step stay inside the ring
     G = max(1, min(gmax, (n + 2 * B - 1) / (2 * B)));
   } else {
@@ -409,6 +418,8 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
   bulge_kernel<B, NQ><<<nmat, G * TT + NIO * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
 }
 }  // namespace
+
+bool bulge_band_resident(int n, int b) { return bulge_fits(n, b >= 32 ? 32 : (b >= 16 ? 16 : 8), 4); }
 
 // Band -> tridiagonal for every matrix of the batch.  b must be 8, 16 or 32.
 void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s) {

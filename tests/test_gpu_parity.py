@@ -381,3 +381,21 @@ def test_high_contrast_many_bands(bs):
         om_g, om_r = np.sqrt(np.maximum(lam[i], 0)), np.sqrt(np.maximum(lr, 0))
         assert np.max(np.abs(om_g - om_r) / om_r) < 1e-7, np.max(np.abs(om_g - om_r) / om_r)
     bs.bs_destroy_cell(h)
+
+
+@pytest.mark.parametrize("Mt", [4, 6, 7])
+def test_band_width_choices_agree_with_the_oracle(bs, Mt):
+    # K is 162 x 162, 338 x 338 (automatic band width 16: the band stays in shared memory in stage 2) and 450 x 450
+    # (automatic 32): the automatic choice and every explicit width give the oracle's eigenfrequencies
+    cell = wl.get("C2").cells[0]
+    comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu)
+    Pr, Sr = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho, Mt)
+    kp = np.array([[0.0, 0.0], [0.5, 0.0], [0.31, 0.17]])
+    refs = [oracle.bands_at_k(Pr, Sr, cell.lattice, Mt, kr, 12) for kr in kp]
+    for panel in (None, 8, 16, 32):
+        h = make_cell(bs, cell, Mt, len(kp), panel=panel)
+        bs.bs_assemble(h, Mt)
+        lam = bs.bs_bands(h, kp, 12)
+        for i, (lr, lmax) in enumerate(refs):
+            check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"Mt={Mt} panel={panel} k={i}")
+        bs.bs_destroy_cell(h)

@@ -55,8 +55,10 @@ __device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double
   // after these reads; its `red` writes come after this reduction's second barrier
 }
 
-template <int NTHR>
-__global__ void __launch_bounds__(NTHR) panel_qr_kernel(int n, int lda, int b, int c0, BatchRef A, BatchRef VW, BatchRef SM,
+// MINB: resident CTAs per SM the register allocation must allow (256-thread variant): 2 when a few matrices each wait on
+// their own latency chain (128 registers), 4 when the batch is large and the SM is shared (64 registers, throughput).
+template <int NTHR, int MINB = 1>
+__global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, int b, int c0, BatchRef A, BatchRef VW, BatchRef SM,
                                                         int inner) {
   extern __shared__ __align__(16) unsigned char qr_smem[];
   const int r0 = c0 + b, m = n - r0;
@@ -360,7 +362,8 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
   static bool attr_done = false;
   if (!attr_done) {
     cudaFuncSetAttribute(panel_qr_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 140 * 1024);
-    cudaFuncSetAttribute(panel_qr_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
+    cudaFuncSetAttribute(panel_qr_kernel<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
+    cudaFuncSetAttribute(panel_qr_kernel<256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
     cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (4 * 32 * 32 + 32) * (int)sizeof(cplx));
     attr_done = true;
   }
@@ -373,7 +376,8 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
         panel_qr_kernel<1024><<<nmat, 1024, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
       } else {
         const size_t smem = (size_t)SW * m * sizeof(cplx) + (8 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
-        panel_qr_kernel<256><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
+        if (nmat > 592) panel_qr_kernel<256, 4><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
+        else panel_qr_kernel<256, 2><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
       }
       ++launches;
     }

@@ -307,6 +307,11 @@ void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
     launch_one<0, 1, 0, 16, 64>(g, s);
     return;
   }
+  if (g.N <= 16 && g.opA == 0 && g.opB == 0 && !(g.flags & BS_GEMM_LOWER_ONLY)) {  // band width 16: 64 x 16 tiles
+    if (g.flags & BS_GEMM_A_HERM_LOWER) launch_one<0, 0, 1, 64, 16>(g, s);
+    else launch_one<0, 0, 0, 64, 16>(g, s);
+    return;
+  }
   if (g.flags & BS_GEMM_A_HERM_LOWER) { launch_one<0, 0, 1>(g, s); return; }  // requires opA == opB == 0, K == M
   if (g.opA == 0 && g.opB == 0) launch_one<0, 0, 0>(g, s);
   else if (g.opA == 0 && g.opB == 1) launch_one<0, 1, 0>(g, s);

@@ -47,7 +47,7 @@ def test_zgemm(bs, opA, opB, M, N, K):
     assert np.max(np.abs(got - ref)) <= 1e-13 * K * np.max(np.abs(ref))
 
 
-@pytest.mark.parametrize("M,N", [(64, 32), (200, 32), (333, 17), (130, 64)])
+@pytest.mark.parametrize("M,N", [(64, 32), (200, 32), (333, 17), (130, 64), (226, 16), (97, 9)])
 def test_zgemm_hermitian_lower(bs, M, N):
     # HEMM: only the lower triangle of A is read (the upper one holds garbage), diagonal imaginary parts are ignored
     import torch

@@ -43,7 +43,7 @@ typedef enum {
   BS_OPT_PENCIL_MODE = 0, /* 0 = BS_PENCIL_POLY (default), 1 = BS_PENCIL_DIRECT; see bs_bands */
   BS_OPT_PANEL = 1,       /* two-stage: band width b in {8, 16, 32}; one-stage: panel width 4..32, multiple of 4.
                              0 (default) = automatic: 16 where the whole band then fits in shared memory in stage 2
-                             (2N <= 353), else 32 */
+                             (2N <= 353), 8 for 2N <= 560, else 32 */
   BS_OPT_TIMING = 2       /* 1 = CUDA events around the stages (bs_get_timings); 2 = also around every kernel launch,
                              summed per kernel class (bs_get_kernel_timings).  Both add a final stream synchronise. */
 } bs_option;
@@ -94,6 +94,9 @@ bs_status bs_isotropic_plane_strain(int32_t n, const double *E, const double *nu
 bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
                          const double *compliance, const double *density, bs_cell **out);
 
+/* Waits for the device to finish (cudaDeviceSynchronize), then releases the handle.  Its small device blocks go back to a
+ * process-wide cache (at most 256 MiB) that later bs_create_cell calls draw from, so create/destroy loops do not pay
+ * cudaMalloc / cudaFree.  NULL is accepted. */
 void bs_destroy_cell(bs_cell *cell);
 
 bs_status bs_set_option(bs_cell *cell, int32_t option, int32_t value);

@@ -6,7 +6,10 @@
 #include <cstdio>
 #include <cstring>
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 
 #include "bs_internal.cuh"
 
@@ -44,10 +47,11 @@ struct Layout {
 
 long long align16(long long x) { return (x + 15) & ~15LL; }
 int band_width(int nb) { return nb >= 32 ? 32 : (nb >= 16 ? 16 : 8); }  // two-stage band width from BS_OPT_PANEL
-// BS_OPT_PANEL = 0 (default): band width 16 whenever the whole band then stays in shared memory during stage 2 (n <= 353:
-// no streaming, twelve sweeps in flight), otherwise 32 (the DMMA GEMMs of stage 1 want the wider panels).  Measured,
-// DESIGN.md section 5.  The choice depends on n only, so a batch and its members take the same path.
-int auto_band_width(int n) { return bsk::bulge_band_resident(n, 16) ? 16 : 32; }
+// BS_OPT_PANEL = 0 (default): the band width follows from whether the whole band then stays in shared memory during
+// stage 2 (no streaming, twelve sweeps in flight): 16 for n <= 353, 8 for n <= 560 (resident up to 795, but beyond 560
+// the narrow panels of stage 1 cost more than the resident chase saves), otherwise 32 (the DMMA GEMMs of stage 1 want the
+// wide panels).  Measured, DESIGN.md section 5.  The choice depends on n only, so a batch and its members take the same path.
+int auto_band_width(int n) { return bsk::bulge_band_resident(n, 16) ? 16 : (n <= 560 ? 8 : 32); }
 
 Layout make_layout(int Mt, int nk, int mode, int nb_opt) {
   const int nb = nb_opt > 0 ? nb_opt : 32;  // automatic band width: sized for the widest
@@ -131,17 +135,60 @@ BatchRef ref(const bs_cell *lead, int ncells, bs_cell *const *cells, long long o
   return r;
 }
 
+// Handle-owned device blocks (geometry blob, batch tables) come from a process-wide cache of freed blocks: creating and
+// destroying handles in a loop (an optimisation driver, bench.py's end-to-end arm) then costs no cudaMalloc / cudaFree,
+// whose latency on a busy device is erratic (measured: bs_destroy_cell 1 ms typically, 10-530 ms in one call of five).
+// A block is reused only by exact (256-byte rounded) size; at most 256 MiB stay cached.  bs_destroy_cell synchronises the
+// device before it returns blocks, so a reused block has no reader left.
+struct DevCache {
+  std::mutex mu;
+  std::multimap<size_t, void *> free_blocks;
+  std::unordered_map<void *, size_t> sizes;
+  size_t cached = 0;
+  static size_t round(size_t b) { return (b + 255) & ~(size_t)255; }
+  cudaError_t alloc(void **p, size_t bytes) {
+    const size_t r = round(bytes ? bytes : 1);
+    {
+      std::lock_guard<std::mutex> g(mu);
+      auto it = free_blocks.find(r);
+      if (it != free_blocks.end()) {
+        *p = it->second;
+        free_blocks.erase(it);
+        cached -= r;
+        return cudaSuccess;
+      }
+    }
+    cudaError_t e = cudaMalloc(p, r);
+    if (e == cudaSuccess) {
+      std::lock_guard<std::mutex> g(mu);
+      sizes[*p] = r;
+    }
+    return e;
+  }
+  void release(void *p) {  // the caller has made sure that no kernel still uses p
+    if (!p) return;
+    std::lock_guard<std::mutex> g(mu);
+    auto it = sizes.find(p);
+    if (it == sizes.end()) { cudaFree(p); return; }
+    if (cached + it->second > ((size_t)256 << 20)) { sizes.erase(it); cudaFree(p); return; }
+    free_blocks.emplace(it->second, p);
+    cached += it->second;
+  }
+};
+DevCache &dev_cache() { static DevCache c; return c; }
+template <class T>
+cudaError_t dev_alloc(T **p, size_t bytes) { return dev_cache().alloc(reinterpret_cast<void **>(p), bytes); }
+
 bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStream_t s) {
   if (ncells > lead->batch_cap) {
-    if (lead->d_bases) cudaFree(lead->d_bases);
-    if (lead->d_geos) cudaFree(lead->d_geos);
-    if (lead->d_info) cudaFree(lead->d_info);
-    if (lead->d_bases3) cudaFree(lead->d_bases3);
+    if (lead->d_bases) cudaDeviceSynchronize();  // earlier launches may still read the tables
+    dev_cache().release(lead->d_bases); dev_cache().release(lead->d_geos);
+    dev_cache().release(lead->d_info); dev_cache().release(lead->d_bases3);
     lead->d_bases = nullptr; lead->d_geos = nullptr; lead->d_info = nullptr; lead->d_bases3 = nullptr; lead->batch_cap = 0;
-    CU(cudaMalloc(&lead->d_bases, sizeof(unsigned long long) * ncells));
-    CU(cudaMalloc(&lead->d_geos, sizeof(bsk::Geometry) * ncells));
-    CU(cudaMalloc(&lead->d_info, sizeof(int) * 5 * ncells));
-    CU(cudaMalloc(&lead->d_bases3, sizeof(unsigned long long) * 12 * ncells));
+    CU(dev_alloc(&lead->d_bases, sizeof(unsigned long long) * ncells));
+    CU(dev_alloc(&lead->d_geos, sizeof(bsk::Geometry) * ncells));
+    CU(dev_alloc(&lead->d_info, sizeof(int) * 5 * ncells));
+    CU(dev_alloc(&lead->d_bases3, sizeof(unsigned long long) * 12 * ncells));
     lead->batch_cap = ncells;
   }
   std::vector<unsigned long long> b(ncells);
@@ -158,9 +205,9 @@ bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStr
 
 bs_status ensure_flat(bs_cell *lead, size_t doubles) {
   if (doubles > lead->flat_cap) {
-    if (lead->d_flat) cudaFree(lead->d_flat);
+    if (lead->d_flat) { cudaDeviceSynchronize(); dev_cache().release(lead->d_flat); }
     lead->d_flat = nullptr; lead->flat_cap = 0;
-    CU(cudaMalloc(&lead->d_flat, doubles * sizeof(double)));
+    CU(dev_alloc(&lead->d_flat, doubles * sizeof(double)));
     lead->flat_cap = doubles;
   }
   return BS_OK;
@@ -292,7 +339,7 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
                o_area = o_w + pad(sizeof(double) * w.size()), o_eph = o_area + pad(sizeof(double) * area.size()),
                total_bytes = o_eph + pad(sizeof(int) * eph.size());
   char *dev = nullptr;
-  if (cudaMalloc((void **)&dev, total_bytes) != cudaSuccess) {
+  if (dev_alloc(&dev, total_bytes) != cudaSuccess) {
     delete c;
     return fail(BS_ERR_CUDA, "bs_create_cell: device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
   }
@@ -322,8 +369,10 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
 
 void bs_destroy_cell(bs_cell *c) {
   if (!c) return;
-  cudaFree(c->d_blob);
-  cudaFree(c->d_bases); cudaFree(c->d_geos); cudaFree(c->d_info); cudaFree(c->d_bases3); cudaFree(c->d_flat);
+  cudaDeviceSynchronize();  // as cudaFree did: nothing in flight reads the handle's blocks once this returns
+  DevCache &dc = dev_cache();
+  dc.release(c->d_blob);
+  dc.release(c->d_bases); dc.release(c->d_geos); dc.release(c->d_info); dc.release(c->d_bases3); dc.release(c->d_flat);
   for (auto &e : c->ev)
     if (e) cudaEventDestroy(e);
   delete c->kt;

@@ -138,19 +138,21 @@ BatchRef ref(const bs_cell *lead, int ncells, bs_cell *const *cells, long long o
 // Handle-owned device blocks (geometry blob, batch tables) come from a process-wide cache of freed blocks: creating and
 // destroying handles in a loop (an optimisation driver, bench.py's end-to-end arm) then costs no cudaMalloc / cudaFree,
 // whose latency on a busy device is erratic (measured: bs_destroy_cell 1 ms typically, 10-530 ms in one call of five).
-// A block is reused only by exact (256-byte rounded) size; at most 256 MiB stay cached.  bs_destroy_cell synchronises the
+// A block is reused only on its own device and by exact (256-byte rounded) size; at most 256 MiB stay cached.  bs_destroy_cell synchronises the
 // device before it returns blocks, so a reused block has no reader left.
 struct DevCache {
   std::mutex mu;
-  std::multimap<size_t, void *> free_blocks;
-  std::unordered_map<void *, size_t> sizes;
+  std::multimap<std::pair<int, size_t>, void *> free_blocks;  // (device, bytes) -> block
+  std::unordered_map<void *, std::pair<int, size_t>> sizes;
   size_t cached = 0;
   static size_t round(size_t b) { return (b + 255) & ~(size_t)255; }
   cudaError_t alloc(void **p, size_t bytes) {
     const size_t r = round(bytes ? bytes : 1);
+    int dev = 0;
+    cudaGetDevice(&dev);
     {
       std::lock_guard<std::mutex> g(mu);
-      auto it = free_blocks.find(r);
+      auto it = free_blocks.find({dev, r});
       if (it != free_blocks.end()) {
         *p = it->second;
         free_blocks.erase(it);
@@ -161,7 +163,7 @@ struct DevCache {
     cudaError_t e = cudaMalloc(p, r);
     if (e == cudaSuccess) {
       std::lock_guard<std::mutex> g(mu);
-      sizes[*p] = r;
+      sizes[*p] = {dev, r};
     }
     return e;
   }
@@ -170,9 +172,9 @@ struct DevCache {
     std::lock_guard<std::mutex> g(mu);
     auto it = sizes.find(p);
     if (it == sizes.end()) { cudaFree(p); return; }
-    if (cached + it->second > ((size_t)256 << 20)) { sizes.erase(it); cudaFree(p); return; }
+    if (cached + it->second.second > ((size_t)256 << 20)) { sizes.erase(it); cudaFree(p); return; }
     free_blocks.emplace(it->second, p);
-    cached += it->second;
+    cached += it->second.second;
   }
 };
 DevCache &dev_cache() { static DevCache c; return c; }

@@ -62,6 +62,11 @@ enum { BS_ASSEMBLY_EXACT = 0, BS_ASSEMBLY_CENTROID = 1 };
  * structure [[A, B, 0], [B, A, 0], [0, 0, 2(A-B)]] and Phi^{-1} is composed from the two N x N inverses
  * (A+B)^{-1} and (A-B)^{-1}; 1 = always factor and invert the full 3N x 3N matrix (any compliance; cross-check). */
 enum { BS_OPT_PHI_INVERSE = 5 };
+/* BS_OPT_OUTPUT (option 6), step S8: what bs_bands / bs_bands_batch write.  0 = lambda = omega^2 (default; may be slightly
+ * negative at k = 0 where the exact value is 0), 1 = omega = sqrt(max(lambda, 0)) (omega_N = sqrt(lambda_N)).
+ * In a batch the lead handle (cells[0]) decides. */
+enum { BS_OPT_OUTPUT = 6 };
+enum { BS_OUTPUT_OMEGA2 = 0, BS_OUTPUT_OMEGA = 1 };
 
 /* Stage indices of bs_get_timings (milliseconds, CUDA events on the call's stream). */
 enum {

@@ -21,6 +21,8 @@ BS_OPT_PENCIL_MODE, BS_OPT_PANEL, BS_OPT_TIMING, BS_OPT_TRIDIAG = 0, 1, 2, 3
 BS_TRIDIAG_TWO_STAGE, BS_TRIDIAG_ONE_STAGE = 0, 1
 BS_OPT_ASSEMBLY = 4
 BS_OPT_PHI_INVERSE = 5
+BS_OPT_OUTPUT = 6
+BS_OUTPUT_OMEGA2, BS_OUTPUT_OMEGA = 0, 1
 BS_ASSEMBLY_EXACT, BS_ASSEMBLY_CENTROID = 0, 1
 BS_PENCIL_POLY, BS_PENCIL_DIRECT = 0, 1
 BS_T_TABLE, BS_T_EXPAND, BS_T_FACTOR, BS_T_COEF, BS_T_PENCIL, BS_T_TRIDIAG, BS_T_BISECT, BS_T_COUNT = 0, 1, 2, 3, 4, 5, 6, 8

@@ -98,6 +98,7 @@ struct bs_cell {
   int P = 0, nedge = 0;
   bool isotropic = true;  // every phase has the isotropic plane-strain block structure of PAPER.md:173
   int phi_general = 0;    // BS_OPT_PHI_INVERSE: 1 = always the general 3N x 3N inverse
+  int out_root = 0;       // BS_OPT_OUTPUT: 1 = bs_bands writes omega = sqrt(max(lambda, 0)) instead of lambda
   char *d_blob = nullptr;  // the one device allocation that holds geo, edge, w, area, ephase
   double *d_edge = nullptr, *d_w = nullptr, *d_area = nullptr;
   int *d_ephase = nullptr;
@@ -408,6 +409,10 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       if (value != 0 && value != 1) return fail(BS_ERR_ARG, "bs_set_option: bad Phi-inverse mode");
       if (c->phi_general != value) c->assembled = false;
       c->phi_general = value;
+      return BS_OK;
+    case BS_OPT_OUTPUT:
+      if (value != BS_OUTPUT_OMEGA2 && value != BS_OUTPUT_OMEGA) return fail(BS_ERR_ARG, "bs_set_option: bad output mode");
+      c->out_root = value;
       return BS_OK;
     case BS_OPT_TIMING:
       if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
@@ -789,7 +794,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
     bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s); ++nl;                         // S6 stage 2
   }
   tick(lead, 2, s);
-  bsk::launch_sturm(n2, d, e, nbands, lam, (int)nmat, s); ++nl;                                       // S7
+  bsk::launch_sturm(n2, d, e, nbands, lam, (int)nmat, s, lead->out_root != 0); ++nl;                                       // S7
   tick(lead, 3, s);
   lead->launches += nl;
   lead->last_n = n2; lead->last_nmat = (int)nmat; lead->last_nk = nk;

@@ -175,6 +175,7 @@ bool bulge_band_resident(int n, int b);  // stage 2 keeps the whole band of widt
 int tridiag_small_max_n();
 void launch_tridiag_small(int n, int lda, BatchRef A, double *d, double *e, int ncells, int inner, cudaStream_t s);
 // S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
-void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s);
+void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s,
+                  bool root = false);  // root: write sqrt(max(lambda, 0)) instead of lambda
 
 }  // namespace bsk

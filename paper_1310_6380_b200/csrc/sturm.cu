@@ -35,7 +35,7 @@ __device__ __forceinline__ int sturm_count(const double *__restrict__ d, const d
 }
 
 __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restrict__ dg, const double *__restrict__ eg,
-                                                   int nev, double *__restrict__ lam) {
+                                                   int nev, double *__restrict__ lam, int root) {
   extern __shared__ double sm[];
   double *d = sm, *e2 = sm + n;
   __shared__ double s_lo, s_hi;
@@ -82,12 +82,15 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
       lo = nlo; hi = nhi;
       __syncthreads();
     }
-    if (k < nev && sub == 0) lam[(size_t)z * nev + k] = 0.5 * (lo + hi);
+    if (k < nev && sub == 0) {
+      const double x = 0.5 * (lo + hi);
+      lam[(size_t)z * nev + k] = root ? sqrt(fmax(x, 0.0)) : x;  // S8: omega = sqrt(max(lambda, 0)) if asked
+    }
   }
 }
 }  // namespace
 
-void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s) {
+void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s, bool root) {
   const size_t smem = (size_t)2 * n * sizeof(double);
   static bool attr_done = false;
   if (!attr_done) {
@@ -96,7 +99,7 @@ void launch_sturm(int n, const double *d, const double *e, int nev, double *lam,
   }
   KScope ks(KC_STURM, 0.0, s);
   const int nthr = nev * G >= ST ? ST : ((nev * G + 31) / 32) * 32;  // few eigenvalues: small CTAs, more of them per SM
-  sturm_kernel<<<nmat, nthr, smem, s>>>(n, d, e, nev, lam);
+  sturm_kernel<<<nmat, nthr, smem, s>>>(n, d, e, nev, lam, root ? 1 : 0);
 }
 
 }  // namespace bsk

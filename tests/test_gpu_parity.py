@@ -399,3 +399,24 @@ def test_band_width_choices_agree_with_the_oracle(bs, Mt):
         for i, (lr, lmax) in enumerate(refs):
             check_bands(lam[i:i + 1], lr[None, :], np.array([lmax]), f"Mt={Mt} panel={panel} k={i}")
         bs.bs_destroy_cell(h)
+
+
+def test_output_omega_instead_of_omega_squared(bs):
+    # S8 (omega_N = sqrt(lambda_N)): BS_OPT_OUTPUT = BS_OUTPUT_OMEGA writes sqrt(max(lambda, 0))
+    w = wl.get("C1")
+    cell = w.cells[0]
+    h = make_cell(bs, cell, w.Mt, w.nk)
+    bs.bs_assemble(h, w.Mt)
+    lam = bs.bs_bands(h, w.kpts, w.nbands)
+    bs.bs_set_option(h, bs.BS_OPT_OUTPUT, bs.BS_OUTPUT_OMEGA)
+    om = bs.bs_bands(h, w.kpts, w.nbands)
+    assert np.array_equal(om, np.sqrt(np.maximum(lam, 0.0)))  # sqrt is correctly rounded on both sides
+    Pr, Sr = oracle.assemble(*oracle_inputs(cell), w.Mt)
+    for i in (0, 3, 17):
+        lr, lmax = oracle.bands_at_k(Pr, Sr, cell.lattice, w.Mt, w.kpts[i], w.nbands)
+        om_r = np.sqrt(np.maximum(lr, 0.0))
+        ok = (np.abs(om[i] - om_r) <= 1e-9 * om_r) | (np.abs(om[i] ** 2 - lr) <= 64 * EPS * lmax)
+        assert ok.all()
+    with pytest.raises(bs.BsError):
+        bs.bs_set_option(h, bs.BS_OPT_OUTPUT, 2)
+    bs.bs_destroy_cell(h)

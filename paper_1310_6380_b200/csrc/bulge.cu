@@ -415,7 +415,8 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
   }
   // algorithmic work: ~n^2/(2B) steps of 48 B^2 real flops (hemv, rank-2, C v, right- and left-apply)
   KScope ks(KC_BULGE, 24.0 * n * (double)n * B * nmat, s);
-  bulge_kernel<B, NQ><<<nmat, G * TT + NIO * 32, smem, s>>>(n, AB, d, e, G, Wc, inner);
+  // the I/O warps only exist when the band is streamed through the ring
+  bulge_kernel<B, NQ><<<nmat, G * TT + (Wc >= n ? 0 : NIO * 32), smem, s>>>(n, AB, d, e, G, Wc, inner);
 }
 }  // namespace
 

@@ -420,3 +420,26 @@ def test_output_omega_instead_of_omega_squared(bs):
     with pytest.raises(bs.BsError):
         bs.bs_set_option(h, bs.BS_OPT_OUTPUT, 2)
     bs.bs_destroy_cell(h)
+
+
+def test_create_destroy_loop_reuses_device_blocks(bs):
+    # An optimisation driver creates and destroys handles in a loop (bench.py's end-to-end arm does): the handle-owned
+    # device blocks come from the library's cache of freed blocks, results stay bitwise equal and device memory does not grow.
+    import torch
+    w = wl.get("C1")
+    cell = w.cells[0]
+    ref = None
+    free0 = None
+    for it in range(25):
+        h = make_cell(bs, cell, w.Mt, w.nk)
+        bs.bs_assemble(h, w.Mt)
+        lam = bs.bs_bands(h, w.kpts, w.nbands)
+        bs.bs_destroy_cell(h)
+        if ref is None:
+            ref = lam.copy()
+        assert np.array_equal(lam, ref)
+        torch.cuda.synchronize()
+        if it == 4:
+            free0 = torch.cuda.mem_get_info()[0]
+    torch.cuda.empty_cache()
+    assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)

@@ -363,6 +363,9 @@ __global__ void __launch_bounds__(NQ * B >= 128 ? 512 : 1024) bulge_kernel(int n
           keep = max(keep, wlo);
           if (is_io) {
             io_evict(max(wlo, t0 + nvalid), keep, io_tid, io_nt);  // columns < t0+nvalid are finished
+            // the columns fetched now reuse ring slots of the columns written back just above (hi - wlo exceeds Wc by
+            // up to B - G - 7), in general through another thread: all slot reads first
+            asm volatile("bar.sync 15, %0;\n" ::"r"(NIO * 32) : "memory");
             io_load(whi, hi, io_tid, io_nt);
           }
           wlo = keep; whi = hi;

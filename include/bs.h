@@ -50,9 +50,12 @@ typedef enum {
 enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
 /* BS_OPT_TRIDIAG (option 3): algorithm of S6.  0 = two-stage (dense -> band by DMMA GEMMs, band -> tridiagonal by bulge
  * chasing; default; matrices with n <= 112 are tridiagonalised inside shared memory by one CTA instead),
- * 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check). */
+ * 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check),
+ * 2 = two-stage with the band of stage 2 always streamed through a shared-memory ring of three sweeps (the configuration
+ * large matrices get anyway), also where the whole band would fit: several CTAs per SM for narrow bands.  A tuning / test
+ * variant: the same algorithm as 0, results reproducible and equal to those of 0 up to rounding. */
 enum { BS_OPT_TRIDIAG = 3 };
-enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1 };
+enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1, BS_TRIDIAG_TWO_STAGE_STREAMED = 2 };
 /* BS_OPT_ASSEMBLY (option 4): quadrature of the shape integrals in S1.  0 = exact closed-form polygon integral (default),
  * 1 = the paper's centroid rule I_p(q) ~ A_p exp(i q.c_p) (PAPER.md:106 eq. 12, :213 eq. 22; c_p = area centroid), kept as the
  * paper-faithful variant: its matrices converge to the exact ones as the mesh is refined. */

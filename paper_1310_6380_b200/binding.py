@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_PKG, "libbs.so")
 
 BS_OK, BS_ERR_ARG, BS_ERR_GEOMETRY, BS_ERR_NOT_PD, BS_ERR_STATE, BS_ERR_CUDA, BS_ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
 BS_OPT_PENCIL_MODE, BS_OPT_PANEL, BS_OPT_TIMING, BS_OPT_TRIDIAG = 0, 1, 2, 3
-BS_TRIDIAG_TWO_STAGE, BS_TRIDIAG_ONE_STAGE = 0, 1
+BS_TRIDIAG_TWO_STAGE, BS_TRIDIAG_ONE_STAGE, BS_TRIDIAG_TWO_STAGE_STREAMED = 0, 1, 2
 BS_OPT_ASSEMBLY = 4
 BS_OPT_PHI_INVERSE = 5
 BS_OPT_OUTPUT = 6

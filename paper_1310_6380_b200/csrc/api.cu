@@ -397,7 +397,8 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       c->nb = value;
       return BS_OK;
     case BS_OPT_TRIDIAG:
-      if (value != BS_TRIDIAG_TWO_STAGE && value != BS_TRIDIAG_ONE_STAGE) return fail(BS_ERR_ARG, "bs_set_option: bad S6 algorithm");
+      if (value != BS_TRIDIAG_TWO_STAGE && value != BS_TRIDIAG_ONE_STAGE && value != BS_TRIDIAG_TWO_STAGE_STREAMED)
+        return fail(BS_ERR_ARG, "bs_set_option: bad S6 algorithm");
       c->algo = value;
       return BS_OK;
     case BS_OPT_ASSEMBLY:
@@ -791,7 +792,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
     const int bw = lead->nb > 0 ? band_width(lead->nb) : auto_band_width(n2);
     nl += bsk::launch_sy2sb(n2, n2, bw, R(L.Ak, mat), R(L.VW, L.vw_stride), R(L.SM, L.sm_stride), R(L.AB, L.ab_stride),
                             ncells, nk, s);                                                             // S6 stage 1
-    bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s); ++nl;                         // S6 stage 2
+    bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s, lead->algo == BS_TRIDIAG_TWO_STAGE_STREAMED); ++nl;                         // S6 stage 2
   }
   tick(lead, 2, s);
   bsk::launch_sturm(n2, d, e, nbands, lam, (int)nmat, s, lead->out_root != 0); ++nl;                                       // S7
@@ -905,10 +906,10 @@ bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d,
     CU(cudaGetLastError());
     return BS_OK;
   }
-  if (algo == BS_TRIDIAG_TWO_STAGE) {
+  if (algo == BS_TRIDIAG_TWO_STAGE || algo == BS_TRIDIAG_TWO_STAGE_STREAMED) {
     BatchRef SMr = raw(sc + vw + pp, per), ABr = raw(sc + vw + pp + smn, per);
     bsk::launch_sy2sb(n, lda, bw, raw(A, strideA), VW, SMr, ABr, 1, batch, (cudaStream_t)stream);
-    bsk::launch_sb2st(n, bw, ABr, d, e, 1, batch, (cudaStream_t)stream);
+    bsk::launch_sb2st(n, bw, ABr, d, e, 1, batch, (cudaStream_t)stream, algo == BS_TRIDIAG_TWO_STAGE_STREAMED);
     CU(cudaStreamSynchronize((cudaStream_t)stream));
     CU(cudaGetLastError());
     return BS_OK;

@@ -395,14 +395,17 @@ constexpr bool bulge_fits(int n, int B, int NQ) {  // the whole band (n columns 
 }
 
 template <int B, int NQ>
-void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inner, cudaStream_t s) {
+void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inner, bool streamed, cudaStream_t s) {
   constexpr int LD = 2 * B, TT = NQ * B;
   const size_t colbytes = (size_t)LD * sizeof(cplx);
   const int gmax = bulge_gmax(B, NQ);
   const size_t team_bytes = (size_t)(4 + 3 * NQ) * B * sizeof(cplx);
   const size_t max_smem = BULGE_MAX_SMEM;
   int G, Wc;
-  if (bulge_fits(n, B, NQ)) {  // whole band resident
+  if (streamed && n > 2 * 3 * B + 8) {  // BS_TRIDIAG_TWO_STAGE_STREAMED: the ring of three sweeps whatever n
+    G = min(3, gmax);
+    Wc = 2 * G * B + 8;
+  } else if (bulge_fits(n, B, NQ)) {  // whole band resident
     Wc = max(n, 2 * B + 8);  // never fewer than a block pair of columns: the masked loads of a step stay inside the ring
     G = max(1, min(gmax, (n + 2 * B - 1) / (2 * B)));
   } else {
@@ -426,11 +429,11 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
 bool bulge_band_resident(int n, int b) { return bulge_fits(n, b >= 32 ? 32 : (b >= 16 ? 16 : 8), 4); }
 
 // Band -> tridiagonal for every matrix of the batch.  b must be 8, 16 or 32.
-void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s) {
+void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s, bool streamed) {
   const int nmat = ncells * inner;
-  if (b == 8) launch_bulge_t<8, 4>(n, AB, d, e, nmat, inner, s);
-  else if (b == 16) launch_bulge_t<16, 4>(n, AB, d, e, nmat, inner, s);
-  else launch_bulge_t<32, 4>(n, AB, d, e, nmat, inner, s);
+  if (b == 8) launch_bulge_t<8, 4>(n, AB, d, e, nmat, inner, streamed, s);
+  else if (b == 16) launch_bulge_t<16, 4>(n, AB, d, e, nmat, inner, streamed, s);
+  else launch_bulge_t<32, 4>(n, AB, d, e, nmat, inner, streamed, s);
 }
 
 }  // namespace bsk

@@ -196,6 +196,70 @@ def test_zhetrd_eigenvalues(bs, n, nb, algo):
         assert np.max(np.abs(lt - la)) <= 1e-13 * n * np.max(np.abs(la))
 
 
+@pytest.mark.parametrize("n,nb,batch", [(242, 16, 1500), (242, 8, 1500), (338, 16, 900), (242, 32, 600)])
+def test_zhetrd_forced_streaming_large_batch(bs, n, nb, batch):
+    """BS_TRIDIAG_TWO_STAGE_STREAMED runs stage 2 through the ring of three sweeps with several CTAs per SM (the I/O
+    warps of different CTAs then drift against the compute warps: the setting in which the write-back / fetch race of
+    the streamed kernel showed as run-to-run different results).  Must be reproducible bit for bit, give the same bits
+    for equal matrices anywhere in the batch, agree with the resident-band kernel to rounding, and have the eigenvalues of
+    the dense matrix."""
+    import torch
+    rng = np.random.default_rng(11 * n + nb)
+    base = []
+    for _ in range(4):
+        G = rand_c(rng, n, n)
+        base.append(to_dev(G + G.conj().T))
+    A = torch.stack([base[i % 4] for i in range(batch)]).contiguous()
+    res = {}
+    for key, algo in [("resident", 0), ("streamed", 2), ("streamed again", 2)]:
+        dA = A.clone()
+        d = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+        e = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+        scratch = torch.zeros(batch * bs.bs_zhetrd_scratch_elems(n, nb), dtype=torch.complex128, device="cuda")
+        bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, algo, batch)
+        torch.cuda.synchronize()
+        res[key] = (d.cpu().numpy(), e.cpu().numpy())
+    dd, ee = res["streamed"]
+    assert np.array_equal(dd, res["streamed again"][0]) and np.array_equal(ee, res["streamed again"][1])
+    for j in range(4):
+        assert np.array_equal(dd[j::4], np.broadcast_to(dd[j], dd[j::4].shape))
+        assert np.array_equal(ee[j::4], np.broadcast_to(ee[j], ee[j::4].shape))
+    scale = np.max(np.abs(res["resident"][0]))
+    assert np.max(np.abs(dd - res["resident"][0])) <= 1e-12 * scale
+    assert np.max(np.abs(np.abs(ee) - np.abs(res["resident"][1]))) <= 1e-12 * scale
+    T = np.diag(dd[5]) + np.diag(ee[5][:n - 1], 1) + np.diag(ee[5][:n - 1], -1)
+    la = np.linalg.eigvalsh(from_dev(base[1]))
+    assert np.max(np.abs(np.linalg.eigvalsh(T) - la)) <= 1e-13 * n * np.max(np.abs(la))
+
+
+@pytest.mark.parametrize("n,nb,batch", [(450, 16, 320), (820, 8, 200), (400, 32, 320)])
+def test_zhetrd_streamed_band_large_batch_is_reproducible(bs, n, nb, batch):
+    """Band streamed through the shared-memory ring (n too large for a resident band of this width) with more matrices
+    than SMs: the I/O warps of the chasing kernel write columns back and fetch new ones into the same ring slots, so a
+    missing ordering shows as run-to-run differences.  Two runs must agree bitwise, every matrix of the batch (the same
+    matrix repeated) must give the same d, e bitwise, and the eigenvalues must be those of the dense matrix."""
+    import torch
+    rng = np.random.default_rng(7 * n + nb)
+    G = rand_c(rng, n, n)
+    A = G + G.conj().T
+    dA0 = to_dev(A)
+    out = []
+    for _ in range(2):
+        dA = dA0.unsqueeze(0).repeat(batch, 1, 1).contiguous()
+        d = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+        e = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+        scratch = torch.zeros(batch * bs.bs_zhetrd_scratch_elems(n, nb), dtype=torch.complex128, device="cuda")
+        bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, 0, batch)
+        torch.cuda.synchronize()
+        out.append((d.cpu().numpy(), e.cpu().numpy()))
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    dd, ee = out[0]
+    assert np.array_equal(dd, np.broadcast_to(dd[0], dd.shape)) and np.array_equal(ee, np.broadcast_to(ee[0], ee.shape))
+    T = np.diag(dd[0]) + np.diag(ee[0][:n - 1], 1) + np.diag(ee[0][:n - 1], -1)
+    la = np.linalg.eigvalsh(A)
+    assert np.max(np.abs(np.linalg.eigvalsh(T) - la)) <= 1e-13 * n * np.max(np.abs(la))
+
+
 def test_sturm_constant_tridiagonal_textbook(bs):
     # constant-coefficient tridiagonal: eigenvalues d + 2 e cos(j pi/(n+1)), j = 1..n
     import torch

@@ -232,6 +232,14 @@ def test_config4_full_batch_sampled(bs):
     # a batch call equals the single-cell calls bit for bit (same kernels, same order of operations)
     one = bs.bs_bands(cells[131], w.kpts, w.nbands)
     assert np.array_equal(one, lam[131])
+    # stage 2 streamed through the three-sweep ring (three CTAs per SM here) instead of the resident band: reproducible
+    # bit for bit, and the same eigenvalues to the backward error of the reduction (64 eps lambda_max, reading R8)
+    for c in cells:
+        bs.bs_set_option(c, bs.BS_OPT_TRIDIAG, bs.BS_TRIDIAG_TWO_STAGE_STREAMED)
+    ls = bs.bs_bands_batch(cells, w.kpts, w.nbands)
+    assert np.array_equal(bs.bs_bands_batch(cells, w.kpts, w.nbands), ls)
+    _, lmax = oracle.bands_at_k(Pr, Sr, w.cells[255].lattice, w.Mt, w.kpts[39], w.nbands)
+    assert np.max(np.abs(ls - lam)) <= 64 * EPS * 4 * lmax  # lambda_max varies by less than 4x over the batch
     for c in cells:
         bs.bs_destroy_cell(c)
 

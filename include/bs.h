@@ -53,7 +53,8 @@ enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
  * 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check),
  * 2 = two-stage with the band of stage 2 always streamed through a shared-memory ring of three sweeps (the configuration
  * large matrices get anyway), also where the whole band would fit: several CTAs per SM for narrow bands.  A tuning / test
- * variant: the same algorithm as 0, results reproducible and equal to those of 0 up to rounding. */
+ * variant: the same algorithm as 0, results reproducible and equal to those of 0 up to rounding (the compiler contracts the
+ * multiply-adds of the two inlined copies of the chasing step differently). */
 enum { BS_OPT_TRIDIAG = 3 };
 enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1, BS_TRIDIAG_TWO_STAGE_STREAMED = 2 };
 /* BS_OPT_ASSEMBLY (option 4): quadrature of the shape integrals in S1.  0 = exact closed-form polygon integral (default),

@@ -9,6 +9,7 @@ import pytest
 
 import oracle
 import workloads as wl
+from closed_forms import ANISO_FIELDS, christoffel_frequencies, compliance_tensor, voigt_from_tensor
 
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 HEX = wl.HEXAGONAL
@@ -244,6 +245,46 @@ def test_homogeneous_dispersion_is_analytic(lattice):
         kap = np.linalg.norm((oracle.plane_wave_indices(Mt) + np.array(kred)) @ Q, axis=1)
         ref = np.sort(np.concatenate([cL * kap, cT * kap]))
         assert np.max(np.abs(np.sqrt(np.maximum(lam, 0)) - ref) / ref) < 5e-12
+
+
+def test_homogeneous_anisotropic_dispersion_pins_eq20_shear_coupling_factors():
+    # PAPER.md:167-171 (eq. 20): the factors 2 on D1112, D2212 and 4 on D1212.  A homogeneous ANISOTROPIC cell (all six
+    # compliance fields non-zero, D1112 != D2212) has omega^2 = eig(Bt(kappa)^T C Bt(kappa)) / rho with C the inverse of
+    # the engineering-shear Voigt compliance, which tests/closed_forms.py derives from the 4-index tensor by applying
+    # eps = D : sigma to unit stresses (no call into the oracle).  A factor 1 (or 4) on the 13/23 entries, a swapped
+    # D1112 <-> D2212, or a 2 instead of 4 on D1212 fails this test.
+    rho, Mt = 3100.0, 2
+    c = wl.homogeneous_cell(HEX, 1.0, 0.3, rho, n=2)
+    comp = np.tile(ANISO_FIELDS, (c.nphase, 1))
+    S = voigt_from_tensor(compliance_tensor(ANISO_FIELDS))
+    assert np.all(np.linalg.eigvalsh(S) > 0) and abs(S[0, 2]) > 0 and abs(S[0, 2]) != abs(S[1, 2])
+    Phi, Psi = oracle.assemble(c.lattice, c.vert_offset, c.verts, comp, c.rho, Mt)
+    _, Q, _ = oracle.reciprocal_basis(HEX)
+    for kred in [(0.31, 0.12), (0.5, 0.0), (-0.2, 0.45)]:
+        lam, _ = oracle.bands_at_k(Phi, Psi, HEX, Mt, kred)
+        kap = (oracle.plane_wave_indices(Mt) + np.array(kred)) @ Q
+        ref = np.sort(christoffel_frequencies(ANISO_FIELDS, rho, kap).ravel())
+        assert np.max(np.abs(np.sqrt(np.maximum(lam, 0)) - ref) / ref) < 1e-11
+    # the same closed form separates the readings: the spectrum with factor 1 on the shear-coupling entries is far away
+    wrong = ANISO_FIELDS.copy()
+    wrong[3:5] *= 0.5
+    kap = (oracle.plane_wave_indices(Mt) + np.array((0.31, 0.12))) @ Q
+    a = np.sort(christoffel_frequencies(ANISO_FIELDS, rho, kap).ravel())
+    b = np.sort(christoffel_frequencies(wrong, rho, kap).ravel())
+    assert np.max(np.abs(a - b) / a) > 1e-3
+
+
+def test_j0_has_no_inaccurate_branch():
+    # sin(t)/t is accurate for every t != 0 (one rounding each for sin, the division): compare with the alternating
+    # series summed in extended precision at small arguments, where a wrong Taylor coefficient would show at 1e-9
+    from fractions import Fraction
+    for t in [3e-5, 9.9e-5, 1.0001e-4, 1e-3, 1e-8, 1e-160]:
+        ft, term, s = Fraction(t), Fraction(1), Fraction(0)
+        for k in range(12):
+            s += term
+            term = -term * ft * ft / ((2 * k + 2) * (2 * k + 3))
+        assert abs(float(oracle.bandstructure._j0(t)) - float(s)) <= 2.3e-16
+    assert float(oracle.bandstructure._j0(0.0)) == 1.0
 
 
 def test_two_zero_modes_at_gamma_and_translation_invariance():

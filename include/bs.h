@@ -103,7 +103,8 @@ bs_status bs_isotropic_plane_strain(int32_t n, const double *E, const double *nu
 bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
                          const double *compliance, const double *density, bs_cell **out);
 
-/* Waits for the device to finish (cudaDeviceSynchronize), then releases the handle.  Its small device blocks go back to a
+/* Waits for the stream of the handle's last call (NOT for the whole device: other streams of the caller keep
+ * running), then releases the handle.  Its small device blocks go back to a
  * process-wide cache (at most 256 MiB) that later bs_create_cell calls draw from, so create/destroy loops do not pay
  * cudaMalloc / cudaFree.  NULL is accepted. */
 void bs_destroy_cell(bs_cell *cell);
@@ -126,7 +127,8 @@ bs_status bs_set_workspace(bs_cell *cell, void *dev_ptr, size_t bytes);
 bs_status bs_assemble(bs_cell *cell, int32_t truncation, void *stream);
 
 /* The same for ncells handles in one set of launches (config 4: optimisation-loop batch).  All cells must have a
- * workspace set for the same truncation. */
+ * workspace set for the same truncation, the same options, live on the same device and have the SAME CELL AREA
+ * |det lattice| (one V^2 scales K(k) of every cell of a launch); anything else is BS_ERR_ARG before any launch. */
 bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t truncation, void *stream);
 
 /* Parity access after bs_assemble: copies Phi (3N x 3N) and Psi (2N x 2N) to HOST buffers (either may be NULL). */
@@ -148,7 +150,9 @@ bs_status bs_get_pencil(bs_cell *cell, const double kred[2], void *K_host, void 
  * Errors: BS_ERR_STATE, BS_ERR_ARG, BS_ERR_NOMEM (nk larger than the workspace was sized for), BS_ERR_CUDA. */
 bs_status bs_bands(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *stream);
 
-/* The same k-points for ncells assembled cells in one set of launches.  omega2_out: ncells x nk x nbands. */
+/* The same k-points for ncells assembled cells in one set of launches.  omega2_out: ncells x nk x nbands.
+ * Limits (BS_ERR_ARG): ncells * nk <= 65535 eigenproblems per call (split larger batches over several calls);
+ * 2N <= 2048; equal cell areas, options and device across the batch (see bs_assemble_batch). */
 bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, const double *kpts, int32_t nbands,
                          double *omega2_out, void *stream);
 

@@ -227,6 +227,20 @@ def bs_get_pencil(cell: Cell, kred, stream=None) -> np.ndarray:
     return K
 
 
+def _out_pointer(out, shape):
+    """Validates a caller-supplied result buffer (float64, C-contiguous, exactly `shape`) and returns its address: a
+    wrong buffer would otherwise be a host or device overflow inside the library."""
+    n = int(np.prod(shape))
+    if isinstance(out, np.ndarray):
+        if out.dtype != np.float64 or not out.flags["C_CONTIGUOUS"] or out.size != n or not out.flags["WRITEABLE"]:
+            raise BsError(BS_ERR_ARG, f"out must be a writable C-contiguous float64 array of {n} elements")
+        return C.c_void_p(out.ctypes.data)
+    import torch
+    if not isinstance(out, torch.Tensor) or out.dtype != torch.float64 or not out.is_contiguous() or out.numel() != n:
+        raise BsError(BS_ERR_ARG, f"out must be a contiguous float64 NumPy array or torch tensor of {n} elements")
+    return C.c_void_p(out.data_ptr())
+
+
 def bs_bands(cell: Cell, kpts, nbands: int, out=None, stream=None):
     """omega^2 (nk, nbands), ascending.  ``out``: None -> new host NumPy array; a NumPy array (host) or a torch CUDA
     float64 tensor (device) is filled in place and returned."""
@@ -234,8 +248,9 @@ def bs_bands(cell: Cell, kpts, nbands: int, out=None, stream=None):
     nk = k.shape[0]
     if out is None:
         out = np.empty((nk, nbands))
-    p = C.c_void_p(out.ctypes.data) if isinstance(out, np.ndarray) else C.c_void_p(out.data_ptr())
+    p = _out_pointer(out, (nk, nbands))
     _check(lib.bs_bands(cell.handle, nk, _ptr(k), nbands, p, _stream(stream)))
+    cell.last_nmat = nk
     return out
 
 
@@ -244,15 +259,22 @@ def bs_bands_batch(cells: Sequence[Cell], kpts, nbands: int, out=None, stream=No
     nk = k.shape[0]
     if out is None:
         out = np.empty((len(cells), nk, nbands))
-    p = C.c_void_p(out.ctypes.data) if isinstance(out, np.ndarray) else C.c_void_p(out.data_ptr())
+    p = _out_pointer(out, (len(cells), nk, nbands))
     _check(lib.bs_bands_batch(_handles(cells), len(cells), nk, _ptr(k), nbands, p, _stream(stream)))
+    cells[0].last_nmat = len(cells) * nk
     return out
 
 
-def bs_get_tridiagonal(cell: Cell, nmat: int):
+def bs_get_tridiagonal(cell: Cell, nmat: Optional[int] = None):
+    """d, e (nmat, 2N) of the last bs_bands / bs_bands_batch call led by ``cell`` (nmat is taken from that call)."""
+    known = getattr(cell, "last_nmat", None)
+    if known is None:
+        raise BsError(BS_ERR_STATE, "bs_get_tridiagonal: no bs_bands call led by this handle yet")
+    if nmat is not None and nmat != known:
+        raise BsError(BS_ERR_ARG, f"bs_get_tridiagonal: the last call had {known} matrices, not {nmat}")
     n = 2 * cell.N
-    d = np.empty((nmat, n))
-    e = np.empty((nmat, n))
+    d = np.empty((known, n))
+    e = np.empty((known, n))
     _check(lib.bs_get_tridiagonal(cell.handle, _ptr(d), _ptr(e)))
     return d, e
 

@@ -123,6 +123,11 @@ struct bs_cell {
   int last_n = 0, last_nmat = 0, last_nk = 0;
   cudaEvent_t ev[BS_T_COUNT + 1] = {nullptr};
   bsk::KTimer *kt = nullptr;  // BS_OPT_TIMING = 2
+  // the stream of the last call that launched work reading this handle's blocks (bs_assemble / bs_bands / accessors):
+  // the accessors and bs_destroy_cell wait for THAT stream only, never for the whole device
+  cudaStream_t last_stream = nullptr;
+  bool used = false;
+  int device = 0;  // the device the handle's blocks live on (current device at bs_create_cell)
 };
 
 namespace {
@@ -182,9 +187,21 @@ DevCache &dev_cache() { static DevCache c; return c; }
 template <class T>
 cudaError_t dev_alloc(T **p, size_t bytes) { return dev_cache().alloc(reinterpret_cast<void **>(p), bytes); }
 
+// Waits for the work the handle's last call enqueued (its own stream), not for the device.
+void sync_handle(const bs_cell *c) {
+  if (c->used && cudaStreamSynchronize(c->last_stream) != cudaSuccess) cudaGetLastError();  // (a destroyed stream: nothing left to wait for)
+}
+void mark_stream(bs_cell *const *cells, int ncells, cudaStream_t s) {
+  for (int c = 0; c < ncells; ++c) {
+    if (cells[c]->used && cells[c]->last_stream != s) sync_handle(cells[c]);  // a handle moved to another stream: drain the old one
+    cells[c]->last_stream = s;
+    cells[c]->used = true;
+  }
+}
+
 bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStream_t s) {
   if (ncells > lead->batch_cap) {
-    if (lead->d_bases) cudaDeviceSynchronize();  // earlier launches may still read the tables
+    if (lead->d_bases) sync_handle(lead);  // earlier launches (on the handle's stream) may still read the tables
     dev_cache().release(lead->d_bases); dev_cache().release(lead->d_geos);
     dev_cache().release(lead->d_info); dev_cache().release(lead->d_bases3);
     lead->d_bases = nullptr; lead->d_geos = nullptr; lead->d_info = nullptr; lead->d_bases3 = nullptr; lead->batch_cap = 0;
@@ -208,7 +225,7 @@ bs_status ensure_batch(bs_cell *lead, bs_cell *const *cells, int ncells, cudaStr
 
 bs_status ensure_flat(bs_cell *lead, size_t doubles) {
   if (doubles > lead->flat_cap) {
-    if (lead->d_flat) { cudaDeviceSynchronize(); dev_cache().release(lead->d_flat); }
+    if (lead->d_flat) { sync_handle(lead); dev_cache().release(lead->d_flat); }
     lead->d_flat = nullptr; lead->flat_cap = 0;
     CU(dev_alloc(&lead->d_flat, doubles * sizeof(double)));
     lead->flat_cap = doubles;
@@ -347,6 +364,7 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
     return fail(BS_ERR_CUDA, "bs_create_cell: device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
   }
   c->d_blob = dev;
+  cudaGetDevice(&c->device);
   c->d_geo = reinterpret_cast<bsk::Geometry *>(dev + o_geo);
   c->d_edge = reinterpret_cast<double *>(dev + o_edge);
   c->d_w = reinterpret_cast<double *>(dev + o_w);
@@ -372,7 +390,7 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
 
 void bs_destroy_cell(bs_cell *c) {
   if (!c) return;
-  cudaDeviceSynchronize();  // as cudaFree did: nothing in flight reads the handle's blocks once this returns
+  sync_handle(c);  // nothing in flight reads the handle's blocks once this returns (only its own stream is drained)
   DevCache &dc = dev_cache();
   dc.release(c->d_blob);
   dc.release(c->d_bases); dc.release(c->d_geos); dc.release(c->d_info); dc.release(c->d_bases3); dc.release(c->d_flat);
@@ -542,8 +560,14 @@ bs_status check_batch(bs_cell *const *cells, int ncells, const char *who) {
   for (int c = 0; c < ncells; ++c) {
     if (!cells[c]) return fail(BS_ERR_ARG, "%s: cells[%d] is null", who, c);
     if (!cells[c]->ws) return fail(BS_ERR_NOMEM, "%s: cells[%d] has no workspace (bs_set_workspace)", who, c);
-    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb || cells[c]->algo != cells[0]->algo || cells[c]->quad != cells[0]->quad)
+    if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb || cells[c]->algo != cells[0]->algo ||
+        cells[c]->quad != cells[0]->quad || cells[c]->phi_general != cells[0]->phi_general || cells[c]->out_root != cells[0]->out_root)
       return fail(BS_ERR_ARG, "%s: cells[%d] has different options than cells[0]", who, c);
+    // one V^2 scales K(k) of every cell of a launch (both pencil modes): the cells of a batch share the cell area
+    if (cells[c]->V != cells[0]->V)
+      return fail(BS_ERR_ARG, "%s: cells[%d] has cell area %.17g, cells[0] has %.17g (a batch needs equal cell areas)", who, c,
+                  cells[c]->V, cells[0]->V);
+    if (cells[c]->device != cells[0]->device) return fail(BS_ERR_ARG, "%s: cells[%d] lives on another device", who, c);
   }
   return BS_OK;
 }
@@ -567,6 +591,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
       return fail(BS_ERR_NOMEM, "bs_assemble: cells[%d] workspace is %zu bytes, need %zu", c, cells[c]->ws_bytes,
                   (size_t)L.total * sizeof(cplx));
   }
+  mark_stream(cells, ncells, s);
   st = ensure_batch(lead, cells, ncells, s);
   if (st != BS_OK) return st;
   const int n3 = 3 * (int)N, n2 = 2 * (int)N, Ni = (int)N;
@@ -636,10 +661,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
       CU(cudaMemcpyAsync((cplx *)cells[c]->ws + L.kvecA, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
       // (no stream synchronise: an H2D copy from pageable memory is staged before cudaMemcpyAsync returns)
     }
-    // the cells of one batch may have different areas: V^2 is applied per cell
-    bool sameV = true;
-    for (int c = 1; c < ncells; ++c) sameV = sameV && cells[c]->V == lead->V;
-    if (!sameV) return fail(BS_ERR_ARG, "bs_assemble_batch: all cells of a batch must have the same cell area");
+    // (check_batch has made sure that the cells of the batch share one cell area V)
     bsk::launch_pencil(Ni, lead->V * lead->V, R(L.Y), n3, R(L.Coef, (long long)n2 * n2), n2, R(L.kvecA, 4LL * Ni), 2,
                        ncells, 6, s); ++nl;
     nl += reduce_blocks(lead, cells, ncells, L, L.Coef, L.Coef, 6, s);
@@ -684,7 +706,7 @@ bs_status bs_get_table(bs_cell *c, void *table_host) {
   if (!c || !table_host) return fail(BS_ERR_ARG, "bs_get_table: null argument");
   if (!c->assembled) return fail(BS_ERR_STATE, "bs_get_table: call bs_assemble first");
   const long long Lt = 4 * c->lay.Mt + 1;
-  CU(cudaDeviceSynchronize());
+  sync_handle(c);
   CU(cudaMemcpy(table_host, (cplx *)c->ws + c->lay.table, sizeof(cplx) * 7 * Lt * Lt, cudaMemcpyDeviceToHost));
   return BS_OK;
 }
@@ -693,7 +715,7 @@ bs_status bs_get_matrices(bs_cell *c, void *phi_host, void *psi_host) {
   if (!c) return fail(BS_ERR_ARG, "bs_get_matrices: null handle");
   if (!c->assembled) return fail(BS_ERR_STATE, "bs_get_matrices: call bs_assemble first");
   const size_t N = c->lay.N, n3 = 3 * N, n2 = 2 * N;
-  CU(cudaDeviceSynchronize());
+  sync_handle(c);
   if (phi_host) CU(cudaMemcpy(phi_host, (cplx *)c->ws + c->lay.Phi, sizeof(cplx) * n3 * n3, cudaMemcpyDeviceToHost));
   if (psi_host) {  // Psi = diag(R, R)  (eq. 19)
     std::memset(psi_host, 0, sizeof(cplx) * n2 * n2);
@@ -715,6 +737,7 @@ bs_status bs_get_pencil(bs_cell *c, const double kred[2], void *K_host, void *st
   fill_direct_kvec(c, L.Mt, 1, kred, kv);
   CU(cudaMemcpyAsync((cplx *)c->ws + L.kvecK, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
   bs_cell *cells[1] = {c};
+  mark_stream(cells, 1, s);
   bsk::launch_pencil(N, c->V * c->V, ref(c, 1, cells, L.Y, 0), n3, ref(c, 1, cells, L.Kk, 0), n2,
                      ref(c, 1, cells, L.kvecK, 0), 1, 1, 1, s);
   c->launches += 1;
@@ -747,6 +770,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
       return fail(BS_ERR_NOMEM, "bs_bands: cells[%d] workspace is %zu bytes, %d k-points need %zu", c, cells[c]->ws_bytes, nk,
                   (size_t)L.total * sizeof(cplx));
   cudaStream_t s = (cudaStream_t)stream;
+  mark_stream(cells, ncells, s);
   st = ensure_batch(lead, cells, ncells, s);
   if (st != BS_OK) return st;
   const size_t nmat = (size_t)ncells * nk;
@@ -826,7 +850,7 @@ bs_status bs_get_tridiagonal(bs_cell *c, double *d_host, double *e_host) {
   if (!c || !d_host || !e_host) return fail(BS_ERR_ARG, "bs_get_tridiagonal: null argument");
   if (!c->d_flat || c->last_nmat == 0) return fail(BS_ERR_STATE, "bs_get_tridiagonal: no bs_bands call led by this handle yet");
   const size_t cnt = (size_t)c->last_nmat * c->last_n;
-  CU(cudaDeviceSynchronize());
+  sync_handle(c);
   CU(cudaMemcpy(d_host, c->d_flat, cnt * sizeof(double), cudaMemcpyDeviceToHost));
   CU(cudaMemcpy(e_host, c->d_flat + cnt, cnt * sizeof(double), cudaMemcpyDeviceToHost));
   return BS_OK;

@@ -359,14 +359,11 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
                  cudaStream_t s) {
   int launches = 0;
   const int nmat = ncells * inner;
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(panel_qr_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 140 * 1024);
-    cudaFuncSetAttribute(panel_qr_kernel<256, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
-    cudaFuncSetAttribute(panel_qr_kernel<256, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 48 * 1024);
-    cudaFuncSetAttribute(wy_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (4 * 32 * 32 + 32) * (int)sizeof(cplx));
-    attr_done = true;
-  }
+  static unsigned long long m1 = 0, m2 = 0, m3 = 0, m4 = 0;
+  ensure_dyn_smem(panel_qr_kernel<1024>, 140 * 1024, m1);
+  ensure_dyn_smem(panel_qr_kernel<256, 2>, 48 * 1024, m2);
+  ensure_dyn_smem(panel_qr_kernel<256, 4>, 48 * 1024, m3);
+  ensure_dyn_smem(wy_small_kernel, (4 * 32 * 32 + 32) * (int)sizeof(cplx), m4);
   for (int c0 = 0; c0 + b < n - 1; c0 += b) {
     const int r0 = c0 + b, m = n - r0;  // m >= 2
     {

@@ -61,6 +61,20 @@ __device__ __forceinline__ cplx *batch_ptr(const BatchRef &r, int cell, int i) {
 // ---------------------------------------------------------------- kernels' host launchers (one per .cu)
 namespace bsk {
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a PER-DEVICE attribute: set it once per (kernel, device).  `mask` is
+// the caller's function-local static (one per kernel instantiation), bit d = done on device d.  A race between two host
+// threads only sets the attribute twice.
+template <class F>
+inline void ensure_dyn_smem(F *kernel, int bytes, unsigned long long &mask) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  const unsigned long long bit = 1ull << (dev & 63);
+  if (!(mask & bit)) {
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    mask |= bit;
+  }
+}
+
 // Per-kernel-class device timing (BS_OPT_TIMING = 2): CUDA events recorded on the launching stream around every launch
 // of a class, summed after the call's final synchronise.  `work` is the ALGORITHMIC work of the class (flops for the
 // DMMA classes, bytes for the HBM classes), accumulated on the host at launch time.

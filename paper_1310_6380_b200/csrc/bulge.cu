@@ -414,11 +414,8 @@ void launch_bulge_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
     Wc = 2 * G * B + 8;
   }
   const size_t smem = (size_t)Wc * colbytes + G * team_bytes + (Wc >= n ? (size_t)n * sizeof(int) : 0);
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(bulge_kernel<B, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    attr_done = true;
-  }
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(bulge_kernel<B, NQ>, 227 * 1024, attr_mask);
   // algorithmic work: ~n^2/(2B) steps of 48 B^2 real flops (hemv, rank-2, C v, right- and left-apply)
   KScope ks(KC_BULGE, 24.0 * n * (double)n * B * nmat, s);
   // the I/O warps only exist when the band is streamed through the ring

@@ -142,12 +142,9 @@ int potrf_trtri(int n, int lda, BatchRef A, BatchRef X, BatchRef tmp, BatchRef d
                 int inner_unused, cudaStream_t s) {
   (void)inner_unused;
   int launches = 0;
-  static bool attr_done = false;
   const size_t diag_smem = sizeof(cplx) * NB * LDP * 2;
-  if (!attr_done) {
-    cudaFuncSetAttribute(potrf_diag_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diag_smem);
-    attr_done = true;
-  }
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(potrf_diag_kernel, (int)diag_smem, attr_mask);
   // ---- Cholesky, right-looking
   for (int j0 = 0; j0 < n; j0 += NB) {
     const int nbk = n - j0 < NB ? n - j0 : NB;

@@ -121,11 +121,8 @@ int tridiag_small_max_n() { return SNMAX; }
 
 void launch_tridiag_small(int n, int lda, BatchRef A, double *d, double *e, int ncells, int inner, cudaStream_t s) {
   const size_t smem = ((size_t)n * (n + 1) + 4 * SNMAX) * sizeof(cplx) + 18 * sizeof(double);
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(tridiag_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 215 * 1024);
-    attr_done = true;
-  }
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(tridiag_small_kernel, 215 * 1024, attr_mask);
   KScope ks(KC_TRIDIAG_SMALL, 16.0 * n * (double)n * n / 3.0 * ncells * inner, s);  // the 16 n^3 / 3 flops of S6
   tridiag_small_kernel<<<ncells * inner, ST, smem, s>>>(n, lda, A, d, e, inner);
 }

@@ -92,11 +92,8 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
 
 void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s, bool root) {
   const size_t smem = (size_t)2 * n * sizeof(double);
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(sturm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    attr_done = true;
-  }
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(sturm_kernel, 200 * 1024, attr_mask);
   KScope ks(KC_STURM, 0.0, s);
   const int nthr = nev * G >= ST ? ST : ((nev * G + 31) / 32) * 32;  // few eigenvalues: small CTAs, more of them per SM
   sturm_kernel<<<nmat, nthr, smem, s>>>(n, d, e, nev, lam, root ? 1 : 0);

@@ -220,11 +220,8 @@ int launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, BatchRef P, 
   const int nmat = ncells * inner;
   const int nblk = (n + TS - 1) / TS;
   if (nb > 32) nb = 32;
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(hemv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kHemvSmem);
-    attr_done = true;
-  }
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(hemv_kernel, (int)kHemvSmem, attr_mask);
   for (int j0 = 0; j0 < n; j0 += nb) {
     const int pn = n - j0 < nb ? n - j0 : nb;
     for (int i = 0; i < pn; ++i) {

@@ -282,11 +282,8 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
 template <int OPA, int OPB, int HERM, int BM = 32, int BN = 32, int NT = 128>
 void launch_one(const GemmDesc &g, cudaStream_t s) {
   constexpr size_t smem = smem_bytes<BM, BN>();
-  static bool attr_done = false;
-  if (!attr_done) {
-    cudaFuncSetAttribute(zgemm_kernel<OPA, OPB, HERM, BM, BN, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_done = true;
-  }
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(zgemm_kernel<OPA, OPB, HERM, BM, BN, NT>, (int)smem, attr_mask);
   const int tm = (g.M + BM - 1) / BM, zz = g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1);
   dim3 grid(tm * zz, (g.N + BN - 1) / BN, 1);
   if (g.flags & BS_GEMM_LOWER_ONLY) grid = dim3((BM / BN) * (tm * (tm + 1) / 2) * zz, 1, 1);  // requires M == N

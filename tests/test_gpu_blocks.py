@@ -331,3 +331,43 @@ def test_error_paths(bs):
     assert ei.value.status == bs.BS_ERR_NOT_PD
     bs.bs_destroy_cell(h)
     bs.bs_destroy_cell(h2)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_batch_rejects_unequal_cell_areas_and_bad_output_buffers(bs, mode):
+    # one V^2 scales every K(k) of a launch: a batch of cells with different lattice areas must be refused BEFORE any
+    # launch, in both pencil modes (it used to return eigenvalues off by (V_c / V_lead)^2 in DIRECT mode)
+    import torch
+    a = wl.random_small_cell(3, 2)
+    b = wl.random_small_cell(4, 2, 1.5 * wl.SQUARE)
+    hs = []
+    for c in (a, b):
+        h = bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, bs.bs_isotropic_plane_strain(c.E, c.nu), c.rho)
+        bs.bs_set_option(h, bs.BS_OPT_PENCIL_MODE, mode)
+        bs.allocate_workspace(h, 2, 2)
+        hs.append(h)
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_assemble_batch(hs, 2)
+    assert ei.value.status == bs.BS_ERR_ARG and "area" in str(ei.value)
+    for h in hs:
+        bs.bs_assemble(h, 2)                       # each alone is fine
+    with pytest.raises(bs.BsError) as ei:
+        bs.bs_bands_batch(hs, [[0.1, 0.2]], 4)
+    assert ei.value.status == bs.BS_ERR_ARG
+    # mismatching options across a batch
+    bs.bs_set_option(hs[1], bs.BS_OPT_OUTPUT, bs.BS_OUTPUT_OMEGA)
+    with pytest.raises(bs.BsError):
+        bs.bs_bands_batch([hs[0], hs[0]][:1] + [hs[1]], [[0.1, 0.2]], 4)
+    # result buffers of the wrong dtype / size / layout never reach the library
+    for bad in (np.empty((1, 4), dtype=np.float32), np.empty((1, 3)), np.empty((4, 2)).T[:1],
+                torch.empty(1, 4, dtype=torch.float32, device="cuda"), torch.empty(1, 5, dtype=torch.float64, device="cuda")):
+        with pytest.raises(bs.BsError) as ei:
+            bs.bs_bands(hs[0], [[0.1, 0.2]], 4, out=bad)
+        assert ei.value.status == bs.BS_ERR_ARG
+    lam = bs.bs_bands(hs[0], [[0.1, 0.2]], 4)
+    d, e = bs.bs_get_tridiagonal(hs[0])
+    assert d.shape == (1, 2 * hs[0].N)
+    with pytest.raises(bs.BsError):
+        bs.bs_get_tridiagonal(hs[0], 7)
+    for h in hs:
+        bs.bs_destroy_cell(h)

@@ -13,7 +13,10 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libbs.so")
-SOURCES = ["api.cu", "assemble.cu", "factor.cu", "zgemm.cu", "pencil.cu", "tridiag.cu", "band.cu", "bulge.cu", "small.cu", "sturm.cu", "probe.cu"]
+SOURCES = ["api.cu", "assemble.cu", "factor.cu", "zgemm.cu", "pencil.cu", "tridiag.cu", "band.cu", "chase.cu", "small.cu", "sturm.cu", "probe.cu"]
+# chase.cu: no implicit multiply-add contraction, so that the step function inlined into the resident and the streamed
+# kernel rounds identically in both (explicit fma() calls still compile to DFMA)
+EXTRA_FLAGS = {"chase.cu": ["-fmad=false"]}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + os.path.join(ROOT, "include"), "-I" + CSRC]
 
@@ -43,7 +46,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src: str) -> str:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc] + NVCC_FLAGS + EXTRA_FLAGS.get(src, []) + (["-Xptxas", "-v"] if verbose else []) + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode:
             sys.stderr.write(r.stdout + r.stderr)

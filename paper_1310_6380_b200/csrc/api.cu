@@ -775,9 +775,11 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   if (st != BS_OK) return st;
   const size_t nmat = (size_t)ncells * nk;
   // flat scratch: d, e (nmat x n), scal (2 nmat), lam (nmat x nbands), coefk (6 nmat)
-  st = ensure_flat(lead, nmat * ((size_t)2 * n2 + 2 + nbands + 6));
+  const size_t nsync = bsk::sb2st_sync_ints(n2, (int)nmat);
+  st = ensure_flat(lead, nmat * ((size_t)2 * n2 + 2 + nbands + 6) + (nsync + 1) / 2);
   if (st != BS_OK) return st;
   double *d = lead->d_flat, *e = d + nmat * n2, *scal = e + nmat * n2, *lam = scal + 2 * nmat, *coefk = lam + nmat * nbands;
+  int *chase_sync = reinterpret_cast<int *>(coefk + 6 * nmat);
   auto R = [&](long long off, long long stride = 0) { return ref(lead, ncells, cells, off, stride); };
   int64_t nl = 0;
   KtGuard ktg(lead);
@@ -816,7 +818,8 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
     const int bw = lead->nb > 0 ? band_width(lead->nb) : auto_band_width(n2);
     nl += bsk::launch_sy2sb(n2, n2, bw, R(L.Ak, mat), R(L.VW, L.vw_stride), R(L.SM, L.sm_stride), R(L.AB, L.ab_stride),
                             ncells, nk, s);                                                             // S6 stage 1
-    bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s, lead->algo == BS_TRIDIAG_TWO_STAGE_STREAMED); ++nl;                         // S6 stage 2
+    bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s, lead->algo == BS_TRIDIAG_TWO_STAGE_STREAMED, 0,
+                      chase_sync); ++nl;                         // S6 stage 2
   }
   tick(lead, 2, s);
   bsk::launch_sturm(n2, d, e, nbands, lam, (int)nmat, s, lead->out_root != 0); ++nl;                                       // S7
@@ -917,6 +920,9 @@ bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d,
   if (!A || !d || !e || !scratch || n < 1 || n > 2048 || batch < 1 || lda < n) return fail(BS_ERR_ARG, "bs_zhetrd: bad argument");
   if (nb < 4) nb = 4;
   if (nb > 32) nb = 32;
+  // test knob: bits 8.. of algo = the number of sweeps per train of the streamed chase (0: the launcher's choice)
+  const int force_g = (algo >> 8) & 0xff;
+  algo &= 0xff;
   const int bw = band_width(nb);
   const long long vw = (long long)std::max(bsk::tridiag_vw_elems(n, nb), bsk::band_vw_elems(n, bw));
   const long long pp = (long long)bsk::tridiag_p_elems(n);
@@ -932,9 +938,12 @@ bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d,
   }
   if (algo == BS_TRIDIAG_TWO_STAGE || algo == BS_TRIDIAG_TWO_STAGE_STREAMED) {
     BatchRef SMr = raw(sc + vw + pp, per), ABr = raw(sc + vw + pp + smn, per);
+    int *sync = nullptr;
+    CU(cudaMalloc(&sync, sizeof(int) * bsk::sb2st_sync_ints(n, batch)));
     bsk::launch_sy2sb(n, lda, bw, raw(A, strideA), VW, SMr, ABr, 1, batch, (cudaStream_t)stream);
-    bsk::launch_sb2st(n, bw, ABr, d, e, 1, batch, (cudaStream_t)stream, algo == BS_TRIDIAG_TWO_STAGE_STREAMED);
+    bsk::launch_sb2st(n, bw, ABr, d, e, 1, batch, (cudaStream_t)stream, algo == BS_TRIDIAG_TWO_STAGE_STREAMED, force_g, sync);
     CU(cudaStreamSynchronize((cudaStream_t)stream));
+    cudaFree(sync);
     CU(cudaGetLastError());
     return BS_OK;
   }

@@ -183,8 +183,11 @@ size_t band_sm_elems(int b);
 size_t band_ab_elems(int n, int b);
 int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, BatchRef AB, int ncells, int inner,
                  cudaStream_t s);
-void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s,
-                  bool streamed = false);  // streamed: ring of three sweeps even when the band would fit shared memory
+// streamed: stream the band through the ring even when it would fit shared memory; force_g > 0: at most that many
+// sweeps per train (test knob); sync: device scratch of sb2st_sync_ints(n, nmat) ints (task counter + train progress)
+void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s, bool streamed,
+                  int force_g, int *sync);
+size_t sb2st_sync_ints(int n, int nmat);
 bool bulge_band_resident(int n, int b);  // stage 2 keeps the whole band of width b in shared memory
 // S6 for n <= tridiag_small_max_n(): the matrix in shared memory, one CTA per matrix, unblocked Householder (small.cu).
 int tridiag_small_max_n();

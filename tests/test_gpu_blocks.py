@@ -371,3 +371,36 @@ def test_batch_rejects_unequal_cell_areas_and_bad_output_buffers(bs, mode):
         bs.bs_get_tridiagonal(hs[0], 7)
     for h in hs:
         bs.bs_destroy_cell(h)
+
+
+@pytest.mark.parametrize("batch", [3, 1500])
+@pytest.mark.parametrize("n,nb", [(200, 8), (242, 16), (338, 16), (300, 32), (450, 32)])
+def test_chase_is_bitwise_independent_of_the_number_of_overlapped_sweeps(bs, n, nb, batch):
+    """Stage 2 streamed with G = 1 (sweeps strictly one after the other: the algorithm as defined), 2, 3, 4, 5 sweeps per
+    train (test knob in bits 8.. of `algo`), several CTAs per SM and several CTAs per matrix following one another through
+    L2, and the resident-band pipeline: all must give the same d, e BIT FOR BIT, for every matrix of the batch."""
+    import torch
+    rng = np.random.default_rng(3 * n + nb)
+    base = []
+    for _ in range(3):
+        G = rand_c(rng, n, n)
+        base.append(to_dev(G + G.conj().T))
+    A = torch.stack([base[i % 3] for i in range(batch)]).contiguous()
+    ref = None
+    for algo in [2 | (1 << 8), 2 | (2 << 8), 2 | (3 << 8), 2 | (4 << 8), 2 | (5 << 8), 2, 0]:
+        dA = A.clone()
+        d = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+        e = torch.zeros(batch, n, dtype=torch.float64, device="cuda")
+        scratch = torch.zeros(batch * bs.bs_zhetrd_scratch_elems(n, nb), dtype=torch.complex128, device="cuda")
+        bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, algo, batch)
+        torch.cuda.synchronize()
+        got = (d.cpu().numpy(), e.cpu().numpy())
+        if ref is None:
+            ref = got
+            for j in range(3):
+                assert np.array_equal(got[0][j::3], np.broadcast_to(got[0][j], got[0][j::3].shape))
+            T = np.diag(got[0][1]) + np.diag(got[1][1][:n - 1], 1) + np.diag(got[1][1][:n - 1], -1)
+            la = np.linalg.eigvalsh(from_dev(base[1]))
+            assert np.max(np.abs(np.linalg.eigvalsh(T) - la)) <= 1e-13 * n * np.max(np.abs(la))
+        else:
+            assert np.array_equal(got[0], ref[0]) and np.array_equal(got[1], ref[1]), hex(algo)

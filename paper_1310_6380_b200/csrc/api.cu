@@ -47,11 +47,12 @@ struct Layout {
 
 long long align16(long long x) { return (x + 15) & ~15LL; }
 int band_width(int nb) { return nb >= 32 ? 32 : (nb >= 16 ? 16 : 8); }  // two-stage band width from BS_OPT_PANEL
-// BS_OPT_PANEL = 0 (default): the band width follows from whether the whole band then stays in shared memory during
-// stage 2 (no streaming, twelve sweeps in flight): 16 for n <= 353, 8 for n <= 560 (resident up to 795, but beyond 560
-// the narrow panels of stage 1 cost more than the resident chase saves), otherwise 32 (the DMMA GEMMs of stage 1 want the
-// wide panels).  Measured, DESIGN.md section 5.  The choice depends on n only, so a batch and its members take the same path.
-int auto_band_width(int n) { return bsk::bulge_band_resident(n, 16) ? 16 : (n <= 560 ? 8 : 32); }
+// BS_OPT_PANEL = 0 (default): band width 16 for every n above the shared-memory one-stage kernel.  Measured with the
+// register-tile chasing kernel of chase.cu (S6 total, ms, band width 8 / 16 / 32): n = 242 x 2000: 36.4 / 30.1 / 52.8;
+// n = 338 x 1000: 37.4 / 29.6 / 47.7; n = 450 x 60: 9.9 / 7.6 / 9.1; n = 882 x 90: 45.7 / 30.7 / 33.9; n = 1300 x 100:
+// - / 78.7 / 84.4; n = 1922 x 120: - / 246.1 / 250.6 (stage 2 alone 50.5 vs 85.6 ms; the narrower panels cost stage 1
+// that much again at this size).  The choice does not depend on the batch, so a batch and its members take the same path.
+int auto_band_width(int n) { (void)n; return 16; }
 
 Layout make_layout(int Mt, int nk, int mode, int nb_opt) {
   const int nb = nb_opt > 0 ? nb_opt : 32;  // automatic band width: sized for the widest

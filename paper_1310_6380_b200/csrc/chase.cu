@@ -22,11 +22,11 @@
 // Wc band columns in shared memory: element (r, c), c <= r <= c + 2B - 1, lives at ring[(c mod Wc) * 2B + (r - c)].
 // Small n: the whole band is loaded once and the teams run one continuous pipeline over all sweeps (one CTA per matrix).
 // Large n: the band streams through the ring; NIO I/O warps write back the columns the train has left behind and fetch
-// the ones its leading sweep needs next, under the arithmetic.  Trains are TASKS handed out by an atomic counter in an
-// order that interleaves the matrices of a group, so that several CTAs (SMs) work on consecutive trains of one matrix
-// at the same time, each following its predecessor through L2: train T publishes "columns < X are final and written
-// back" in progress[m][T] (release), train T+1 waits for it (acquire) before it fetches them.
-// states the ring-slot lifetime argument.
+// the ones its leading sweep needs next, under the arithmetic.  Trains are TASKS handed out by an atomic counter in
+// train-major order over a group of matrices, so every SM is busy whatever the batch size and several CTAs may work on
+// consecutive trains of one matrix at the same time, each following its predecessor through L2: train T publishes
+// "columns < X are final and written back" in progress[m][T] (release), train T+1 waits for it (acquire) before it
+// fetches them.  DESIGN.md section 5 states the ring-slot lifetime argument and the measured cost of close followers.
 #include "bs_internal.cuh"
 
 namespace bsk {
@@ -56,6 +56,7 @@ struct Cfg {
   static constexpr int LD = 2 * B, TR = B / 8, TC = B / 8, TCW = TC / NW;
   static constexpr int TW = 2 * NW;        // warps per team
   static constexpr int TT = 32 * TW;       // threads per team
+  static constexpr int MAXT = NW >= 4 ? 896 : 512;  // threads per CTA the kernels are compiled for
   // team scratch (complex elements): v (two parities), tau (two parities, padded), w, tau u, y, C[:,0], partial p, partial u
   static constexpr int O_V = 0, O_TAU = 2 * B, O_W = 2 * B + 4, O_TU = O_W + B, O_Y = O_TU + B, O_C0 = O_Y + B,
                        O_P = O_C0 + B, O_U = O_P + NW * B, SCR = O_U + NW * B;
@@ -104,7 +105,7 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
   using C = Cfg<B, NW>;
   constexpr int LD = C::LD, TR = C::TR, TCW = C::TCW;
   const int g = lane >> 2, t = lane & 3;
-  auto ctg = [&](int ci) { return NW == 1 ? ci : (ci == 0 ? rw : C::TC - 1 - rw); };
+  auto ctg = [&](int ci) { return (NW == 2 && TCW == 2) ? (ci == 0 ? rw : C::TC - 1 - rw) : rw * TCW + ci; };
   double tre[TR][TCW][2], tim[TR][TCW][2];
   // Ring addresses are formed as (column base - column) + row and (row base - row) + column, never as
   // base + (row - column): nvcc 12.9 turns the latter into `base | (row - column)` inside the branch where the
@@ -210,7 +211,7 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
 // the NW C warps owns the tile columns rw TCW .. (rw + 1) TCW - 1 (all tile rows).
 template <int B, int NW>
 __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, const cplx *vb, cplx *vnext, cplx *tau_next,
-                                       cplx tau, int L, int L2, int rw, int lane, int bar_id) {
+                                       cplx tau, int L, int L2, int rw, int lane, int bar_id, int team_bar) {
   using C = Cfg<B, NW>;
   constexpr int LD = C::LD, TR = C::TR, TCW = C::TCW;
   const int g = lane >> 2, t = lane & 3;
@@ -255,6 +256,7 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
       if (rw == 0) ts[C::O_C0 + 8 * rt + g] = cmake(tre[rt][0][0], tim[rt][0][0]);
     }
   }
+  asm volatile("bar.arrive %0, %1;\n" ::"r"(team_bar), "r"(C::TT) : "memory");  // releases the D warps of the team
   if (NW > 1) named_bar(bar_id, 32 * NW);
   else __syncwarp();
   // lane l = row l of C: x = C[:,0] - tau u (conj(v[0]) = 1), then the reflector that annihilates x below its first entry.
@@ -270,8 +272,18 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   cplx x = csub(ts[C::O_C0 + l], tu);
   x.x = in ? x.x : 0.0;
   x.y = in ? x.y : 0.0;
-  const double ss = warp_sum(lane >= 1 ? x.x * x.x + x.y * x.y : 0.0);
-  const cplx al = shfl_c(x, 0);
+  // three lane reductions in one butterfly: |x[1:]|^2 and sum_{l>=1} conj(x_l) (tau u)_l, which gives
+  // s = v2^H (tau u) = (tau u)_0 + conj(scale) sum_{l>=1} conj(x_l) (tau u)_l  without a second pass over the lanes
+  double ss = lane >= 1 ? x.x * x.x + x.y * x.y : 0.0;
+  double sdr = lane >= 1 ? x.x * tu.x + x.y * tu.y : 0.0;
+  double sdi = lane >= 1 ? x.x * tu.y - x.y * tu.x : 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    ss += __shfl_xor_sync(0xffffffffu, ss, o);
+    sdr += __shfl_xor_sync(0xffffffffu, sdr, o);
+    sdi += __shfl_xor_sync(0xffffffffu, sdi, o);
+  }
+  const cplx al = shfl_c(x, 0), tu0 = shfl_c(tu, 0);
   const bool norefl = L2 <= 1, trivial = norefl || (ss == 0.0 && al.y == 0.0);
   const double nrm = sqrt(al.x * al.x + al.y * al.y + ss);
   const double beta2 = trivial ? 1.0 : -copysign(nrm, al.x);
@@ -287,8 +299,8 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   cplx v2 = cmul(x, scale);
   v2.x = lane == 0 ? 1.0 : v2.x;
   v2.y = lane == 0 ? 0.0 : v2.y;
-  // s = v2^H (tau u)
-  const double s_re = warp_sum(v2.x * tu.x + v2.y * tu.y), s_im = warp_sum(v2.x * tu.y - v2.y * tu.x);
+  const cplx sv = cadd(tu0, cmulc(cmake(sdr, sdi), scale));  // (tau u)_0 + conj(scale) sum conj(x_l) (tau u)_l
+  const double s_re = sv.x, s_im = sv.y;
   if (lane < B) {
     ts[C::O_TU + lane] = tu;
     vnext[lane] = v2;
@@ -394,8 +406,13 @@ __device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, i
   const cplx tau = ts[C::O_TAU + par];
   const int Jn = J + L, L2 = min(B, n - Jn);
   const int sJ = J % Wc;
-  if (role == 0) step_D<B, NW>(ring, Wc, sJ, ts, vb, tau, L, rw, lane, 5 + team);
-  else if (L2 > 0) step_C<B, NW>(ring, Wc, sJ, ts, vb, vnext, ts + C::O_TAU + (par ^ 1), tau, L, L2, rw, lane, 9 + team);
+  if (role == 0) {
+    // the C warps (the longer chain of the step) load their tiles first: the D warps wait until those are in registers
+    if (L2 > 0) named_bar(1 + team, C::TT);
+    step_D<B, NW>(ring, Wc, sJ, ts, vb, tau, L, rw, lane, 5 + team);
+  } else if (L2 > 0) {
+    step_C<B, NW>(ring, Wc, sJ, ts, vb, vnext, ts + C::O_TAU + (par ^ 1), tau, L, L2, rw, lane, 9 + team, 1 + team);
+  }
   if (L2 <= 0) {
     finished = true;
   } else {
@@ -408,7 +425,7 @@ __device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, i
 // starts at macro-step start[j] = max(start[j-1] + 2, finish of sweep j-G) (two blocks behind its predecessor, and its
 // team must be free).
 template <int B, int NW>
-__global__ void __launch_bounds__(512) chase_resident_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc, int inner) {
+__global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_resident_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc, int inner) {
   using C = Cfg<B, NW>;
   constexpr int LD = C::LD;
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -417,7 +434,9 @@ __global__ void __launch_bounds__(512) chase_resident_kernel(int n, BatchRef AB,
   const cplx *ab = batch_ptr(AB, cell, mi);
   double *dg = d + (size_t)z * n, *eg = e + (size_t)z * n;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int team = warp / C::TW, wt = warp % C::TW, role = wt / NW, rw = wt % NW;
+  // warps [0, G NW): the D warps of teams 0 .. G-1, then the C warps (the issue arbiter favours the higher warp index:
+  // the C half is the longer chain), then the I/O warps; every scheduler hosts warps of both roles
+  const int role = warp >= G * NW ? 1 : 0, wr = warp - role * G * NW, team = wr / NW, rw = wr % NW;
   cplx *ts = ring + (size_t)Wc * LD + (size_t)team * C::SCR;
   int *start = reinterpret_cast<int *>(ring + (size_t)Wc * LD + (size_t)G * C::SCR);
   for (int q = tid; q < n * LD; q += blockDim.x) {
@@ -469,7 +488,7 @@ __device__ __forceinline__ void st_release(int *p, int v) {
 // so the CTAs in flight spread over about (CTAs / group) consecutive trains of each matrix of the group.  A task only
 // ever waits for its predecessor train, which was handed out earlier and is running or done: no deadlock.
 template <int B, int NW>
-__global__ void __launch_bounds__(512) chase_stream_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc,
+__global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, BatchRef AB, double *d, double *e, int G, int Wc,
                                                            int inner, int nmat, int group, int ntrains, int *sync) {
   using C = Cfg<B, NW>;
   constexpr int LD = C::LD;
@@ -480,7 +499,9 @@ __global__ void __launch_bounds__(512) chase_stream_kernel(int n, BatchRef AB, d
   const int ncomp = G * C::TT;
   const bool is_io = tid >= ncomp;
   const int io_tid = tid - ncomp, io_nt = NIO * 32;
-  const int team = warp / C::TW, wt = warp % C::TW, role = wt / NW, rw = wt % NW;
+  // warps [0, G NW): the D warps of teams 0 .. G-1, then the C warps (the issue arbiter favours the higher warp index:
+  // the C half is the longer chain), then the I/O warps; every scheduler hosts warps of both roles
+  const int role = warp >= G * NW ? 1 : 0, wr = warp - role * G * NW, team = wr / NW, rw = wr % NW;
   cplx *ts = ring + (size_t)Wc * LD + (size_t)(is_io ? 0 : team) * C::SCR;
   const int ntasks = nmat * ntrains;
 
@@ -565,7 +586,7 @@ __global__ void __launch_bounds__(512) chase_stream_kernel(int n, BatchRef AB, d
         if (io_tid == 0) {
           st_release(mine, keep);
           if (prev && hi > whi)
-            while (ld_acquire(prev) < hi) __nanosleep(32);
+            while (ld_acquire(prev) < hi) __nanosleep(20);
         }
         named_bar(15, io_nt);
         io_load(whi, hi, io_tid, io_nt);
@@ -587,10 +608,13 @@ __global__ void __launch_bounds__(512) chase_stream_kernel(int n, BatchRef AB, d
 }
 
 constexpr size_t CHASE_MAX_SMEM = 226 * 1024;
+// warps per role (D, C) of a team at band width 32.  Four (28 warps per CTA, 72 registers) was measured slower than two:
+// C5 95.7 vs 85.6 ms, C3 16.7 vs 14.9 ms (spills, and the exchanges then span four warps)
+constexpr int NW32 = 2;
 template <int B, int NW>
-constexpr int chase_gmax_resident() { return 512 / Cfg<B, NW>::TT; }
+constexpr int chase_gmax_resident() { return NW > 1 ? (Cfg<B, NW>::MAXT / Cfg<B, NW>::TT < 4 ? Cfg<B, NW>::MAXT / Cfg<B, NW>::TT : 4) : 512 / Cfg<B, NW>::TT; }
 template <int B, int NW>
-constexpr int chase_gmax_stream() { return NW == 2 ? 3 : (512 - NIO * 32) / Cfg<B, NW>::TT; }
+constexpr int chase_gmax_stream() { return NW >= 2 ? 3 : (512 - NIO * 32) / Cfg<B, NW>::TT; }
 template <int B, int NW>
 constexpr bool chase_fits(int n) {  // the whole band (n columns of 2B entries) beside the team scratch and the start table
   return (size_t)(n > 2 * B + 8 ? n : 2 * B + 8) * 2 * B * sizeof(cplx) +
@@ -634,9 +658,12 @@ void launch_chase_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
   const int resident = g_sm_count(dev) * max(occ, 1);
   const long long ntasks = (long long)nmat * ntrains;
   const int grid = (int)min((long long)resident, ntasks);
-  // about four CTAs follow one another on each matrix of a group (more would only wait for their predecessors: a train
-  // can start 2G macro-steps after the one before it); groups of equal size
-  int group = max(1, grid / 4);
+  // One group = as many matrices as there are CTAs (train-major inside the group): a CTA that finishes train T of one
+  // matrix moves on to another matrix, and train T + 1 of the first is taken up when its predecessor is far ahead or
+  // done.  Measured on C5 / C3 (ms) with about c CTAs following one another on each matrix: c = 1: 87.6 / 15.2,
+  // c = 2: 87.6 / 19.2, c = 3: 91.9 / 19.2, c = 4: 100.3 / 27.1, c = 6: 112 / 35.9 -- a train cannot start before its
+  // predecessor is 2G + 1 macro-steps ahead, and trains are only ~35 macro-steps long, so close followers mostly wait.
+  int group = max(1, grid);
   const int ngroups = (nmat + group - 1) / group;
   group = (nmat + ngroups - 1) / ngroups;
   cudaMemsetAsync(sync, 0, sizeof(int) * (size_t)(1 + ntasks), s);
@@ -645,7 +672,7 @@ void launch_chase_t(int n, BatchRef AB, double *d, double *e, int nmat, int inne
 }  // namespace
 
 bool bulge_band_resident(int n, int b) {
-  return b >= 32 ? chase_fits<32, 2>(n) : (b >= 16 ? chase_fits<16, 1>(n) : chase_fits<8, 1>(n));
+  return b >= 32 ? chase_fits<32, NW32>(n) : (b >= 16 ? chase_fits<16, 1>(n) : chase_fits<8, 1>(n));
 }
 size_t sb2st_sync_ints(int n, int nmat) { return 1 + (size_t)nmat * (size_t)(n > 1 ? n - 1 : 1); }  // G >= 1 trains per matrix
 
@@ -655,7 +682,7 @@ void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, i
   const int nmat = ncells * inner;
   if (b == 8) launch_chase_t<8, 1>(n, AB, d, e, nmat, inner, streamed, force_g, sync, s);
   else if (b == 16) launch_chase_t<16, 1>(n, AB, d, e, nmat, inner, streamed, force_g, sync, s);
-  else launch_chase_t<32, 2>(n, AB, d, e, nmat, inner, streamed, force_g, sync, s);
+  else launch_chase_t<32, NW32>(n, AB, d, e, nmat, inner, streamed, force_g, sync, s);
 }
 
 }  // namespace bsk

@@ -71,3 +71,62 @@ def test_single_rank_share_is_the_workload_path():
     assert np.array_equal(bench.dense_kpath(w, 1, 0), w.kpts)
     a, b = bench.dense_kpath(w, 2, 0), bench.dense_kpath(w, 2, 1)
     assert a.shape == b.shape == w.kpts.shape and np.allclose(a[0], 0) and np.allclose(b[-1], 0)
+
+
+GATHER_WORKER = r"""
+import os, sys
+import numpy as np
+import torch, torch.distributed as dist
+sys.path.insert(0, os.environ["BS_ROOT"])
+from paper_1310_6380_b200 import sharded
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+# the full result a single rank would produce: value encodes (cell, k, band)
+for ncells, nk, nb in [(1, 30, 6), (5, 7, 3), (1, 2, 4), (7, 1, 2)]:
+    full = (np.arange(ncells)[:, None, None] * 1e6 + np.arange(nk)[None, :, None] * 1e3 + np.arange(nb)[None, None, :]).astype(np.float64)
+    for axis_name in ("kpoints", "cells"):
+        n = nk if axis_name == "kpoints" else ncells
+        ax = 1 if axis_name == "kpoints" else 0
+        lo, hi = sharded.shard_range(n, world, rank)
+        counts = sharded.shard_counts(n, world)
+        assert sum(counts) == n and counts[rank] == hi - lo
+        local = torch.from_numpy(np.ascontiguousarray(full[:, lo:hi] if ax == 1 else full[lo:hi]))
+        got = sharded.gather_shards(local, counts, ax).numpy()
+        assert np.array_equal(got, full), (ncells, nk, nb, axis_name)    # the gathered index map is the 1-rank order
+assert sharded.choose_axis(256, 40, world) == "cells" and sharded.choose_axis(1, 120, world) == "kpoints"
+dist.barrier()
+if rank == 0:
+    print("GATHER OK", world)
+dist.destroy_process_group()
+"""
+
+
+def _run_workers(tmp_path, text, nproc, marker):
+    script = tmp_path / "worker.py"
+    script.write_text(text)
+    env = dict(os.environ, BS_ROOT=ROOT, MASTER_ADDR="127.0.0.1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(nproc), "--master-addr",
+           "127.0.0.1", "--master-port", str(_free_port()), str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, env=env)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert marker in r.stdout
+
+
+def test_result_gather_reproduces_single_rank_order_world2(tmp_path):
+    _run_workers(tmp_path, GATHER_WORKER, 2, "GATHER OK 2")
+
+
+def test_result_gather_ragged_world3(tmp_path):
+    _run_workers(tmp_path, GATHER_WORKER, 3, "GATHER OK 3")
+
+
+def test_shard_ranges_tile_the_units():
+    sys.path.insert(0, ROOT)
+    from paper_1310_6380_b200 import sharded
+    for n in (0, 1, 5, 120, 256, 10240):
+        for world in (1, 2, 3, 8, 16):
+            ranges = [sharded.shard_range(n, world, r) for r in range(world)]
+            assert ranges[0][0] == 0 and ranges[-1][1] == n
+            assert all(a[1] == b[0] for a, b in zip(ranges, ranges[1:]))
+            sizes = [b - a for a, b in ranges]
+            assert max(sizes) - min(sizes) <= 1

@@ -206,8 +206,17 @@ def measure(bs, torch, w, kpts, steps, warmup, local, barrier, e2e=True):
     nk, ncell = len(kpts), len(w.cells)
     comps = [bs.bs_isotropic_plane_strain(c.E, c.nu) for c in w.cells]
 
+    # cells that share one geometry (config 4: every cell is the same 8 x 8 pixel grid with other materials) are created
+    # through bs_create_cells_shared: S1 integrates the polygons once and forms every cell's table as T = W I
+    c0 = w.cells[0]
+    same_geometry = ncell > 1 and all(np.array_equal(c.lattice, c0.lattice) and np.array_equal(c.vert_offset, c0.vert_offset)
+                                      and np.array_equal(c.verts, c0.verts) for c in w.cells)
+
     def create(timing):
-        hs = [bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, comp, c.rho) for c, comp in zip(w.cells, comps)]
+        if same_geometry:
+            hs = bs.bs_create_cells_shared(c0.lattice, c0.vert_offset, c0.verts, np.stack(comps), np.stack([c.rho for c in w.cells]))
+        else:
+            hs = [bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, comp, c.rho) for c, comp in zip(w.cells, comps)]
         bs.bs_set_option(hs[0], bs.BS_OPT_TIMING, timing)
         return hs
 

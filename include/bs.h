@@ -42,8 +42,8 @@ typedef enum {
 typedef enum {
   BS_OPT_PENCIL_MODE = 0, /* 0 = BS_PENCIL_POLY (default), 1 = BS_PENCIL_DIRECT; see bs_bands */
   BS_OPT_PANEL = 1,       /* two-stage: band width b in {8, 16, 32}; one-stage: panel width 4..32, multiple of 4.
-                             0 (default) = automatic: 16 where the whole band then fits in shared memory in stage 2
-                             (2N <= 353), 8 for 2N <= 560, else 32 */
+                             0 (default) = automatic: 16 (measured best at every size with the register-tile chasing
+                             kernel of stage 2) */
   BS_OPT_TIMING = 2       /* 1 = CUDA events around the stages (bs_get_timings); 2 = also around every kernel launch,
                              summed per kernel class (bs_get_kernel_timings).  Both add a final stream synchronise. */
 } bs_option;
@@ -51,10 +51,10 @@ enum { BS_PENCIL_POLY = 0, BS_PENCIL_DIRECT = 1 };
 /* BS_OPT_TRIDIAG (option 3): algorithm of S6.  0 = two-stage (dense -> band by DMMA GEMMs, band -> tridiagonal by bulge
  * chasing; default; matrices with n <= 112 are tridiagonalised inside shared memory by one CTA instead),
  * 1 = one-stage blocked Householder (matrix-vector bound; kept as a cross-check),
- * 2 = two-stage with the band of stage 2 always streamed through a shared-memory ring of three sweeps (the configuration
- * large matrices get anyway), also where the whole band would fit: several CTAs per SM for narrow bands.  A tuning / test
- * variant: the same algorithm as 0, results reproducible and equal to those of 0 up to rounding (the compiler contracts the
- * multiply-adds of the two inlined copies of the chasing step differently). */
+ * 2 = two-stage with the band of stage 2 always streamed through the shared-memory ring (the configuration large matrices
+ * get anyway), also where the whole band would fit.  A tuning / test variant: the same algorithm as 0 and the SAME BITS
+ * (the chasing step is compiled without multiply-add contraction, so its two inlined copies round identically; the
+ * result does not depend on how many sweeps overlap either: tests/test_gpu_blocks.py). */
 enum { BS_OPT_TRIDIAG = 3 };
 enum { BS_TRIDIAG_TWO_STAGE = 0, BS_TRIDIAG_ONE_STAGE = 1, BS_TRIDIAG_TWO_STAGE_STREAMED = 2 };
 /* BS_OPT_ASSEMBLY (option 4): quadrature of the shape integrals in S1.  0 = exact closed-form polygon integral (default),
@@ -102,6 +102,22 @@ bs_status bs_isotropic_plane_strain(int32_t n, const double *E, const double *nu
  * Errors: BS_ERR_ARG, BS_ERR_GEOMETRY, BS_ERR_CUDA. */
 bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
                          const double *compliance, const double *density, bs_cell **out);
+
+/* Optimisation-loop shape: ncells cells that share ONE geometry (lattice
+ * and polygons) and differ in their material properties only.
+ *   compliance  host, ncells x P x 6 doubles;  density  host, ncells x P doubles;  out  receives ncells handles.
+ * The handles behave like those of bs_create_cell (each is destroyed with bs_destroy_cell; the shared geometry is freed
+ * with the last of them).  When ALL cells of a bs_assemble / bs_assemble_batch call share one geometry, step S1 evaluates
+ * the polygon integrals I_p(q_D) ONCE into a (P x index-difference) table that stays with the geometry, and every cell's
+ * table is the small product T = W I of its weights with it (one batched DMMA GEMM) instead of re-integrating every
+ * polygon per cell.  Errors: as bs_create_cell. */
+bs_status bs_create_cells_shared(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
+                                 int32_t ncells, const double *compliance, const double *density, bs_cell **out);
+
+/* New material properties for an existing handle (same geometry): compliance host P x 6, density host P.  The next
+ * bs_assemble uses them; with a shared geometry the polygon integrals are not evaluated again.  The copy is ordered after
+ * the work already enqueued on the handle's stream.  Errors: BS_ERR_ARG. */
+bs_status bs_set_properties(bs_cell *cell, const double *compliance, const double *density);
 
 /* Waits for the stream of the handle's last call (NOT for the whole device: other streams of the caller keep
  * running), then releases the handle.  Its small device blocks go back to a

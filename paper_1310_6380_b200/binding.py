@@ -30,7 +30,7 @@ BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_K
 
 # every symbol include/bs.h declares (tests check that the library exports all of them)
 SYMBOLS = [
-    "bs_isotropic_plane_strain", "bs_create_cell", "bs_destroy_cell", "bs_set_option", "bs_workspace_bytes",
+    "bs_isotropic_plane_strain", "bs_create_cell", "bs_create_cells_shared", "bs_set_properties", "bs_destroy_cell", "bs_set_option", "bs_workspace_bytes",
     "bs_set_workspace", "bs_assemble", "bs_assemble_batch", "bs_get_matrices", "bs_get_table", "bs_get_pencil",
     "bs_bands", "bs_bands_batch", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
     "bs_last_error",
@@ -67,6 +67,8 @@ lib.bs_destroy_cell.restype = None
 lib.bs_destroy_cell.argtypes = [_vp]
 lib.bs_isotropic_plane_strain.argtypes = [C.c_int32, _dp, _dp, _dp]
 lib.bs_create_cell.argtypes = [_dp, C.c_int32, _ip, _dp, _dp, _dp, C.POINTER(_vp)]
+lib.bs_create_cells_shared.argtypes = [_dp, C.c_int32, _ip, _dp, C.c_int32, _dp, _dp, C.POINTER(_vp)]
+lib.bs_set_properties.argtypes = [_vp, _dp, _dp]
 lib.bs_set_option.argtypes = [_vp, C.c_int32, C.c_int32]
 lib.bs_workspace_bytes.argtypes = [_vp, C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]
 lib.bs_set_workspace.argtypes = [_vp, _vp, C.c_size_t]
@@ -127,7 +129,12 @@ def bs_isotropic_plane_strain(E, nu) -> np.ndarray:
 class Cell:
     """Owner of one ``bs_cell`` handle and of the torch workspace tensor lent to it."""
 
-    def __init__(self, lattice, vert_offset, verts, compliance, density):
+    def __init__(self, lattice=None, vert_offset=None, verts=None, compliance=None, density=None, _adopt=None):
+        if _adopt is not None:      # a handle created by bs_create_cells_shared
+            self.handle, self.nphase = _adopt
+            self.workspace = None
+            self.Mt = None
+            return
         lattice = _f64(lattice).reshape(4)
         off = np.ascontiguousarray(np.asarray(vert_offset, dtype=np.int32))
         verts = _f64(verts).reshape(-1)
@@ -159,6 +166,30 @@ class Cell:
 
 def bs_create_cell(lattice, vert_offset, verts, compliance, density) -> Cell:
     return Cell(lattice, vert_offset, verts, compliance, density)
+
+
+def bs_create_cells_shared(lattice, vert_offset, verts, compliances, densities):
+    """ncells handles that share ONE geometry: ``compliances`` (ncells, P, 6), ``densities``
+    (ncells, P).  Returns a list of Cell."""
+    lattice = _f64(lattice).reshape(4)
+    off = np.ascontiguousarray(np.asarray(vert_offset, dtype=np.int32))
+    verts = _f64(verts).reshape(-1)
+    P = int(off.shape[0] - 1)
+    comp = _f64(compliances).reshape(-1, P, 6)
+    rho = _f64(densities).reshape(-1, P)
+    ncells = comp.shape[0]
+    if rho.shape[0] != ncells or verts.shape[0] != 2 * int(off[-1]):
+        raise BsError(BS_ERR_ARG, "array sizes do not match nphase / vert_offset / ncells")
+    hs = (_vp * ncells)()
+    _check(lib.bs_create_cells_shared(_ptr(lattice), P, _ptr(off, _ip), _ptr(verts), ncells, _ptr(comp), _ptr(rho), hs))
+    return [Cell(_adopt=(_vp(h), P)) for h in hs]
+
+
+def bs_set_properties(cell: Cell, compliance, density) -> None:
+    comp, rho = _f64(compliance).reshape(-1), _f64(density).reshape(-1)
+    if comp.shape[0] != 6 * cell.nphase or rho.shape[0] != cell.nphase:
+        raise BsError(BS_ERR_ARG, "array sizes do not match nphase")
+    _check(lib.bs_set_properties(cell.handle, _ptr(comp), _ptr(rho)))
 
 
 def bs_destroy_cell(cell: Cell) -> None:

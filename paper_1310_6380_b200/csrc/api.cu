@@ -94,6 +94,18 @@ Layout make_layout(int Mt, int nk, int mode, int nb_opt) {
 
 }  // namespace
 
+// Geometry shared by the handles of bs_create_cells_shared (refcounted): edge arrays once, and the table of polygon
+// integrals I_p(q_D) of the last truncation / quadrature it was assembled with.
+struct SharedGeom {
+  int refs = 0, device = 0, P = 0, nedge = 0;
+  char *d_blob = nullptr;
+  double *d_edge = nullptr, *d_area = nullptr;
+  int *d_ephase = nullptr, *d_poff = nullptr;
+  cplx *d_phase = nullptr;   // [P x nhalf]
+  size_t phase_cap = 0;      // elements
+  int phase_Mt = -1, phase_quad = -1;
+};
+
 struct bs_cell {
   double A[4], T[4], Q[4], V;
   int P = 0, nedge = 0;
@@ -124,6 +136,9 @@ struct bs_cell {
   int last_n = 0, last_nmat = 0, last_nk = 0;
   cudaEvent_t ev[BS_T_COUNT + 1] = {nullptr};
   bsk::KTimer *kt = nullptr;  // BS_OPT_TIMING = 2
+  SharedGeom *shared = nullptr;   // bs_create_cells_shared
+  cplx *d_sh = nullptr;           // lead handle: weights matrix and stacked tables of the shared-geometry S1
+  size_t sh_cap = 0;
   // the stream of the last call that launched work reading this handle's blocks (bs_assemble / bs_bands / accessors):
   // the accessors and bs_destroy_cell wait for THAT stream only, never for the whole device
   cudaStream_t last_stream = nullptr;
@@ -244,6 +259,97 @@ struct KtGuard {  // routes the launchers' KScope to the lead cell's timer for t
   ~KtGuard() { bsk::g_kt = nullptr; }
 };
 
+// S0 on the host (PAPER.md:23-26 eq. 1, :138): reciprocal basis, fractional coordinates, per-edge arrays, signed areas and
+// centroids, tiling check.
+struct HostGeom {
+  double T[4], Q[4], V = 0.0;
+  int ne = 0;
+  std::vector<double> edge, area;  // edge: SoA [6][ne]; area: [area | ch1 | ch2][P]
+  std::vector<int> eph;
+};
+bs_status host_geometry(const double lattice[4], int nphase, const int32_t *vert_offset, const double *verts, HostGeom &g) {
+  if (vert_offset[0] != 0) return fail(BS_ERR_ARG, "bs_create_cell: vert_offset[0] != 0");
+  for (int p = 0; p < nphase; ++p)
+    if (vert_offset[p + 1] - vert_offset[p] < 3) return fail(BS_ERR_ARG, "bs_create_cell: phase %d has < 3 vertices", p);
+  const double det = lattice[0] * lattice[3] - lattice[1] * lattice[2];
+  if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return fail(BS_ERR_GEOMETRY, "bs_create_cell: singular lattice");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(BS_ERR_CUDA, "bs_create_cell: no CUDA device");
+  // T = A^{-1}; q^j = 2 pi (column j of T)  =>  q^i . h^j = 2 pi delta_ij   (PAPER.md:23-26 eq. 1, :138)
+  g.T[0] = lattice[3] / det;  g.T[1] = -lattice[1] / det;
+  g.T[2] = -lattice[2] / det; g.T[3] = lattice[0] / det;
+  g.Q[0] = kTwoPi * g.T[0]; g.Q[1] = kTwoPi * g.T[2];  // q^1
+  g.Q[2] = kTwoPi * g.T[1]; g.Q[3] = kTwoPi * g.T[3];  // q^2
+  g.V = std::fabs(det);
+  const int ne = vert_offset[nphase];
+  g.ne = ne;
+  g.edge.assign((size_t)6 * ne, 0.0);
+  g.area.assign((size_t)3 * nphase, 0.0);
+  g.eph.assign(ne, 0);
+  double total = 0.0;
+  for (int p = 0; p < nphase; ++p) {
+    const int s = vert_offset[p], t = vert_offset[p + 1];
+    double a2 = 0.0, cxs = 0.0, cys = 0.0;
+    for (int i = s; i < t; ++i) {
+      const int k = (i + 1 < t) ? i + 1 : s;
+      const double x0 = verts[2 * i], y0 = verts[2 * i + 1], x1 = verts[2 * k], y1 = verts[2 * k + 1];
+      a2 += x0 * y1 - x1 * y0;
+      cxs += (x0 + x1) * (x0 * y1 - x1 * y0);
+      cys += (y0 + y1) * (x0 * y1 - x1 * y0);
+      const double ex = x1 - x0, ey = y1 - y0, mx = 0.5 * (x0 + x1), my = 0.5 * (y0 + y1);
+      // fractional coordinates H = x T  (x = H_1 h^1 + H_2 h^2, PAPER.md:21)
+      g.edge[0 * (size_t)ne + i] = mx * g.T[0] + my * g.T[2];
+      g.edge[1 * (size_t)ne + i] = mx * g.T[1] + my * g.T[3];
+      g.edge[2 * (size_t)ne + i] = ex * g.T[0] + ey * g.T[2];
+      g.edge[3 * (size_t)ne + i] = ex * g.T[1] + ey * g.T[3];
+      g.edge[4 * (size_t)ne + i] = ex;
+      g.edge[5 * (size_t)ne + i] = ey;
+      g.eph[i] = p;
+    }
+    g.area[p] = 0.5 * a2;
+    if (!(g.area[p] > 0.0))
+      return fail(BS_ERR_GEOMETRY, "bs_create_cell: phase %d has non-positive signed area %g (must be CCW)", p, g.area[p]);
+    total += g.area[p];
+    // area centroid (used by the centroid-rule assembly mode, eq. 12), in fractional coordinates
+    const double cx = cxs / (3.0 * a2), cy = cys / (3.0 * a2);
+    g.area[(size_t)nphase + p] = cx * g.T[0] + cy * g.T[2];
+    g.area[(size_t)2 * nphase + p] = cx * g.T[1] + cy * g.T[3];
+  }
+  if (std::fabs(total - g.V) > 1e-10 * g.V)
+    return fail(BS_ERR_GEOMETRY, "bs_create_cell: phases cover area %.17g, cell area is %.17g", total, g.V);
+  return BS_OK;
+}
+// Channel weights [7][P]: Voigt compliance with the factors 1/2/4 of PAPER.md:167-171 (eq. 20), then rho.
+bs_status host_weights(int nphase, const double *compliance, const double *density, std::vector<double> &w, bool &iso) {
+  w.assign((size_t)7 * nphase, 0.0);
+  iso = true;
+  for (int p = 0; p < nphase; ++p) {
+    if (!(density[p] > 0.0)) return fail(BS_ERR_ARG, "bs_create_cell: phase %d has density <= 0", p);
+    const double *D = compliance + 6 * (size_t)p;
+    if (D[3] != 0.0 || D[4] != 0.0 || D[0] != D[1] || std::fabs(4.0 * D[5] - 2.0 * (D[0] - D[2])) > 1e-14 * std::fabs(D[0]))
+      iso = false;
+    w[0 * (size_t)nphase + p] = D[0];
+    w[1 * (size_t)nphase + p] = D[1];
+    w[2 * (size_t)nphase + p] = D[2];
+    w[3 * (size_t)nphase + p] = 2.0 * D[3];
+    w[4 * (size_t)nphase + p] = 2.0 * D[4];
+    w[5 * (size_t)nphase + p] = 4.0 * D[5];
+    w[6 * (size_t)nphase + p] = density[p];
+  }
+  return BS_OK;
+}
+void init_cell_host(bs_cell *c, const double lattice[4], const HostGeom &g, int nphase, bool iso) {
+  std::memcpy(c->A, lattice, sizeof(double) * 4);
+  std::memcpy(c->T, g.T, sizeof(double) * 4);
+  std::memcpy(c->Q, g.Q, sizeof(double) * 4);
+  c->V = g.V;
+  c->P = nphase;
+  c->nedge = g.ne;
+  c->isotropic = iso;
+  c->geo.nedge = g.ne; c->geo.P = nphase;
+  std::memcpy(c->geo.Q, g.Q, sizeof(double) * 4);
+}
+
 double tock(bs_cell *c, int a, int b) {
   float ms = 0.f;
   if (c->ev[a] && c->ev[b]) cudaEventElapsedTime(&ms, c->ev[a], c->ev[b]);
@@ -281,84 +387,21 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
   if (!lattice || !vert_offset || !verts || !compliance || !density || !out || nphase < 1)
     return fail(BS_ERR_ARG, "bs_create_cell: null pointer or nphase < 1");
   *out = nullptr;
-  if (vert_offset[0] != 0) return fail(BS_ERR_ARG, "bs_create_cell: vert_offset[0] != 0");
-  for (int p = 0; p < nphase; ++p)
-    if (vert_offset[p + 1] - vert_offset[p] < 3) return fail(BS_ERR_ARG, "bs_create_cell: phase %d has < 3 vertices", p);
-  const double det = lattice[0] * lattice[3] - lattice[1] * lattice[2];
-  if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return fail(BS_ERR_GEOMETRY, "bs_create_cell: singular lattice");
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(BS_ERR_CUDA, "bs_create_cell: no CUDA device");
-
+  HostGeom hg;
+  bs_status st = host_geometry(lattice, nphase, vert_offset, verts, hg);
+  if (st != BS_OK) return st;
+  std::vector<double> w;
+  bool iso = true;
+  st = host_weights(nphase, compliance, density, w, iso);
+  if (st != BS_OK) return st;
   bs_cell *c = new (std::nothrow) bs_cell();
   if (!c) return fail(BS_ERR_NOMEM, "bs_create_cell: host allocation failed");
-  std::memcpy(c->A, lattice, sizeof(double) * 4);
-  // T = A^{-1}; q^j = 2 pi (column j of T)  =>  q^i . h^j = 2 pi delta_ij   (PAPER.md:23-26 eq. 1, :138)
-  c->T[0] = lattice[3] / det;  c->T[1] = -lattice[1] / det;
-  c->T[2] = -lattice[2] / det; c->T[3] = lattice[0] / det;
-  c->Q[0] = kTwoPi * c->T[0]; c->Q[1] = kTwoPi * c->T[2];  // q^1
-  c->Q[2] = kTwoPi * c->T[1]; c->Q[3] = kTwoPi * c->T[3];  // q^2
-  c->V = std::fabs(det);
-  c->P = nphase;
-  const int ne = vert_offset[nphase];
-  c->nedge = ne;
-  std::vector<double> edge((size_t)6 * ne), area((size_t)3 * nphase), w((size_t)7 * nphase);  // area: [area | ch1 | ch2]
-  std::vector<int> eph(ne);
-  double total = 0.0;
-  for (int p = 0; p < nphase; ++p) {
-    const int s = vert_offset[p], t = vert_offset[p + 1];
-    double a2 = 0.0, cxs = 0.0, cys = 0.0;
-    for (int i = s; i < t; ++i) {
-      const int k = (i + 1 < t) ? i + 1 : s;
-      const double x0 = verts[2 * i], y0 = verts[2 * i + 1], x1 = verts[2 * k], y1 = verts[2 * k + 1];
-      a2 += x0 * y1 - x1 * y0;
-      cxs += (x0 + x1) * (x0 * y1 - x1 * y0);
-      cys += (y0 + y1) * (x0 * y1 - x1 * y0);
-      const double ex = x1 - x0, ey = y1 - y0, mx = 0.5 * (x0 + x1), my = 0.5 * (y0 + y1);
-      // fractional coordinates H = x T  (x = H_1 h^1 + H_2 h^2, PAPER.md:21)
-      edge[0 * (size_t)ne + i] = mx * c->T[0] + my * c->T[2];
-      edge[1 * (size_t)ne + i] = mx * c->T[1] + my * c->T[3];
-      edge[2 * (size_t)ne + i] = ex * c->T[0] + ey * c->T[2];
-      edge[3 * (size_t)ne + i] = ex * c->T[1] + ey * c->T[3];
-      edge[4 * (size_t)ne + i] = ex;
-      edge[5 * (size_t)ne + i] = ey;
-      eph[i] = p;
-    }
-    area[p] = 0.5 * a2;
-    if (!(area[p] > 0.0)) {
-      delete c;
-      return fail(BS_ERR_GEOMETRY, "bs_create_cell: phase %d has non-positive signed area %g (must be CCW)", p, area[p]);
-    }
-    total += area[p];
-    {  // area centroid (used by the centroid-rule assembly mode, eq. 12), in fractional coordinates
-      const double cx = cxs / (3.0 * a2), cy = cys / (3.0 * a2);
-      area[(size_t)nphase + p] = cx * c->T[0] + cy * c->T[2];
-      area[(size_t)2 * nphase + p] = cx * c->T[1] + cy * c->T[3];
-    }
-    if (!(density[p] > 0.0)) {
-      delete c;
-      return fail(BS_ERR_ARG, "bs_create_cell: phase %d has density <= 0", p);
-    }
-    // Voigt weights with the factors 1/2/4 of PAPER.md:167-171 (eq. 20)
-    const double *D = compliance + 6 * (size_t)p;
-    if (D[3] != 0.0 || D[4] != 0.0 || D[0] != D[1] || std::fabs(4.0 * D[5] - 2.0 * (D[0] - D[2])) > 1e-14 * std::fabs(D[0]))
-      c->isotropic = false;
-    w[0 * (size_t)nphase + p] = D[0];
-    w[1 * (size_t)nphase + p] = D[1];
-    w[2 * (size_t)nphase + p] = D[2];
-    w[3 * (size_t)nphase + p] = 2.0 * D[3];
-    w[4 * (size_t)nphase + p] = 2.0 * D[4];
-    w[5 * (size_t)nphase + p] = 4.0 * D[5];
-    w[6 * (size_t)nphase + p] = density[p];
-  }
-  if (std::fabs(total - c->V) > 1e-10 * c->V) {
-    delete c;
-    return fail(BS_ERR_GEOMETRY, "bs_create_cell: phases cover area %.17g, cell area is %.17g", total, c->V);
-  }
+  init_cell_host(c, lattice, hg, nphase, iso);
   // one device allocation and one H2D copy per cell: [Geometry | edge | w | area | ephase], each part 256-byte aligned
   auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
-  const size_t o_geo = 0, o_edge = pad(sizeof(bsk::Geometry)), o_w = o_edge + pad(sizeof(double) * edge.size()),
-               o_area = o_w + pad(sizeof(double) * w.size()), o_eph = o_area + pad(sizeof(double) * area.size()),
-               total_bytes = o_eph + pad(sizeof(int) * eph.size());
+  const size_t o_geo = 0, o_edge = pad(sizeof(bsk::Geometry)), o_w = o_edge + pad(sizeof(double) * hg.edge.size()),
+               o_area = o_w + pad(sizeof(double) * w.size()), o_eph = o_area + pad(sizeof(double) * hg.area.size()),
+               total_bytes = o_eph + pad(sizeof(int) * hg.eph.size());
   char *dev = nullptr;
   if (dev_alloc(&dev, total_bytes) != cudaSuccess) {
     delete c;
@@ -372,20 +415,113 @@ bs_status bs_create_cell(const double lattice[4], int32_t nphase, const int32_t 
   c->d_area = reinterpret_cast<double *>(dev + o_area);
   c->d_ephase = reinterpret_cast<int *>(dev + o_eph);
   c->geo.edge = c->d_edge; c->geo.ephase = c->d_ephase; c->geo.w = c->d_w; c->geo.area = c->d_area;
-  c->geo.nedge = ne; c->geo.P = nphase;
-  std::memcpy(c->geo.Q, c->Q, sizeof(double) * 4);
   std::vector<char> host(total_bytes, 0);
   std::memcpy(host.data() + o_geo, &c->geo, sizeof(bsk::Geometry));
-  std::memcpy(host.data() + o_edge, edge.data(), sizeof(double) * edge.size());
+  std::memcpy(host.data() + o_edge, hg.edge.data(), sizeof(double) * hg.edge.size());
   std::memcpy(host.data() + o_w, w.data(), sizeof(double) * w.size());
-  std::memcpy(host.data() + o_area, area.data(), sizeof(double) * area.size());
-  std::memcpy(host.data() + o_eph, eph.data(), sizeof(int) * eph.size());
+  std::memcpy(host.data() + o_area, hg.area.data(), sizeof(double) * hg.area.size());
+  std::memcpy(host.data() + o_eph, hg.eph.data(), sizeof(int) * hg.eph.size());
   if (cudaMemcpy(dev, host.data(), total_bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
-    bs_status st = fail(BS_ERR_CUDA, "bs_create_cell: H2D copy failed: %s", cudaGetErrorString(cudaGetLastError()));
+    st = fail(BS_ERR_CUDA, "bs_create_cell: H2D copy failed: %s", cudaGetErrorString(cudaGetLastError()));
     bs_destroy_cell(c);
     return st;
   }
   *out = c;
+  return BS_OK;
+}
+
+bs_status bs_create_cells_shared(const double lattice[4], int32_t nphase, const int32_t *vert_offset, const double *verts,
+                                 int32_t ncells, const double *compliance, const double *density, bs_cell **out) {
+  if (!lattice || !vert_offset || !verts || !compliance || !density || !out || nphase < 1 || ncells < 1)
+    return fail(BS_ERR_ARG, "bs_create_cells_shared: null pointer, nphase < 1 or ncells < 1");
+  for (int i = 0; i < ncells; ++i) out[i] = nullptr;
+  HostGeom hg;
+  bs_status st = host_geometry(lattice, nphase, vert_offset, verts, hg);
+  if (st != BS_OK) return st;
+  // the geometry block shared by all handles: [edge | area | ephase | phase offsets]
+  auto pad = [](size_t b) { return (b + 255) & ~(size_t)255; };
+  const size_t o_edge = 0, o_area = pad(sizeof(double) * hg.edge.size()), o_eph = o_area + pad(sizeof(double) * hg.area.size()),
+               o_poff = o_eph + pad(sizeof(int) * hg.eph.size()), gbytes = o_poff + pad(sizeof(int) * (nphase + 1));
+  SharedGeom *sg = new (std::nothrow) SharedGeom();
+  if (!sg) return fail(BS_ERR_NOMEM, "bs_create_cells_shared: host allocation failed");
+  if (dev_alloc(&sg->d_blob, gbytes) != cudaSuccess) {
+    delete sg;
+    return fail(BS_ERR_CUDA, "bs_create_cells_shared: device allocation failed: %s", cudaGetErrorString(cudaGetLastError()));
+  }
+  cudaGetDevice(&sg->device);
+  sg->P = nphase; sg->nedge = hg.ne;
+  sg->d_edge = reinterpret_cast<double *>(sg->d_blob + o_edge);
+  sg->d_area = reinterpret_cast<double *>(sg->d_blob + o_area);
+  sg->d_ephase = reinterpret_cast<int *>(sg->d_blob + o_eph);
+  sg->d_poff = reinterpret_cast<int *>(sg->d_blob + o_poff);
+  {
+    std::vector<char> host(gbytes, 0);
+    std::memcpy(host.data() + o_edge, hg.edge.data(), sizeof(double) * hg.edge.size());
+    std::memcpy(host.data() + o_area, hg.area.data(), sizeof(double) * hg.area.size());
+    std::memcpy(host.data() + o_eph, hg.eph.data(), sizeof(int) * hg.eph.size());
+    std::memcpy(host.data() + o_poff, vert_offset, sizeof(int) * (nphase + 1));
+    if (cudaMemcpy(sg->d_blob, host.data(), gbytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+      dev_cache().release(sg->d_blob);
+      delete sg;
+      return fail(BS_ERR_CUDA, "bs_create_cells_shared: H2D copy failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+  }
+  // per handle: [Geometry | w]; all of them in one staging buffer and one H2D copy per handle block
+  const size_t o_w = pad(sizeof(bsk::Geometry)), cbytes = o_w + pad(sizeof(double) * 7 * nphase);
+  std::vector<double> w;
+  std::vector<char> host(cbytes, 0);
+  for (int i = 0; i < ncells; ++i) {
+    bool iso = true;
+    st = host_weights(nphase, compliance + (size_t)i * 6 * nphase, density + (size_t)i * nphase, w, iso);
+    bs_cell *c = st == BS_OK ? new (std::nothrow) bs_cell() : nullptr;
+    if (st == BS_OK && !c) st = fail(BS_ERR_NOMEM, "bs_create_cells_shared: host allocation failed");
+    if (st == BS_OK) {
+      init_cell_host(c, lattice, hg, nphase, iso);
+      c->shared = sg;
+      ++sg->refs;
+      out[i] = c;
+      c->device = sg->device;
+      if (dev_alloc(&c->d_blob, cbytes) != cudaSuccess) st = fail(BS_ERR_CUDA, "bs_create_cells_shared: device allocation failed");
+    }
+    if (st == BS_OK) {
+      c->d_geo = reinterpret_cast<bsk::Geometry *>(c->d_blob);
+      c->d_w = reinterpret_cast<double *>(c->d_blob + o_w);
+      c->d_edge = sg->d_edge; c->d_area = sg->d_area; c->d_ephase = sg->d_ephase;
+      c->geo.edge = c->d_edge; c->geo.ephase = c->d_ephase; c->geo.w = c->d_w; c->geo.area = c->d_area;
+      std::memcpy(host.data(), &c->geo, sizeof(bsk::Geometry));
+      std::memcpy(host.data() + o_w, w.data(), sizeof(double) * w.size());
+      if (cudaMemcpy(c->d_blob, host.data(), cbytes, cudaMemcpyHostToDevice) != cudaSuccess)
+        st = fail(BS_ERR_CUDA, "bs_create_cells_shared: H2D copy failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    if (st != BS_OK) {
+      const std::string msg = g_err;
+      int owners = 0;
+      for (int j = 0; j <= i; ++j) owners += out[j] != nullptr;
+      for (int j = 0; j <= i; ++j) {
+        if (out[j]) bs_destroy_cell(out[j]);  // (the last one frees the shared geometry)
+        out[j] = nullptr;
+      }
+      if (owners == 0) {  // no handle ever took ownership of the geometry
+        dev_cache().release(sg->d_blob);
+        delete sg;
+      }
+      std::snprintf(g_err, sizeof(g_err), "%s", msg.c_str());
+      return st;
+    }
+  }
+  return BS_OK;
+}
+
+bs_status bs_set_properties(bs_cell *c, const double *compliance, const double *density) {
+  if (!c || !compliance || !density) return fail(BS_ERR_ARG, "bs_set_properties: null argument");
+  std::vector<double> w;
+  bool iso = true;
+  bs_status st = host_weights(c->P, compliance, density, w, iso);
+  if (st != BS_OK) return st;
+  sync_handle(c);  // the kernels of the last call may still read the old weights
+  CU(cudaMemcpy(c->d_w, w.data(), sizeof(double) * w.size(), cudaMemcpyHostToDevice));
+  c->isotropic = iso;
+  c->assembled = false;
   return BS_OK;
 }
 
@@ -395,6 +531,12 @@ void bs_destroy_cell(bs_cell *c) {
   DevCache &dc = dev_cache();
   dc.release(c->d_blob);
   dc.release(c->d_bases); dc.release(c->d_geos); dc.release(c->d_info); dc.release(c->d_bases3); dc.release(c->d_flat);
+  dc.release(c->d_sh);
+  if (c->shared && --c->shared->refs == 0) {
+    dc.release(c->shared->d_blob);
+    dc.release(c->shared->d_phase);
+    delete c->shared;
+  }
   for (auto &e : c->ev)
     if (e) cudaEventDestroy(e);
   delete c->kt;
@@ -603,7 +745,37 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   tick(lead, 0, s);
   double total_edges = 0.0;
   for (int c = 0; c < ncells; ++c) total_edges += cells[c]->nedge;
-  bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s); ++nl;  // S1
+  SharedGeom *sg = lead->shared;
+  for (int c = 0; c < ncells; ++c)
+    if (cells[c]->shared != sg) sg = nullptr;
+  if (sg) {
+    // S1 with one geometry for the whole batch: polygon integrals once (kept with the geometry), then T = W I per cell
+    const long long Lt = 4LL * Mt + 1, nhalf = (Lt * Lt + 1) / 2;
+    if (sg->phase_Mt != Mt || sg->phase_quad != lead->quad) {
+      const size_t need = (size_t)nhalf * sg->P;
+      if (need > sg->phase_cap) {
+        sync_handle(lead);
+        dev_cache().release(sg->d_phase);
+        sg->d_phase = nullptr; sg->phase_cap = 0;
+        CU(dev_alloc(&sg->d_phase, need * sizeof(cplx)));
+        sg->phase_cap = need;
+      }
+      bsk::launch_phase_table(lead->geo, sg->d_poff, Mt, sg->d_phase, lead->quad, s); ++nl;
+      sg->phase_Mt = Mt; sg->phase_quad = lead->quad;
+    }
+    const size_t wel = (size_t)7 * ncells * sg->P, tel = (size_t)7 * ncells * nhalf;
+    if (wel + tel > lead->sh_cap) {
+      sync_handle(lead);
+      dev_cache().release(lead->d_sh);
+      lead->d_sh = nullptr; lead->sh_cap = 0;
+      CU(dev_alloc(&lead->d_sh, (wel + tel) * sizeof(cplx)));
+      lead->sh_cap = wel + tel;
+    }
+    bsk::launch_shared_tables(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, sg->P, Mt, sg->d_phase, lead->d_sh,
+                              lead->d_sh + wel, R(L.table), s); nl += 3;
+  } else {
+    bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s); ++nl;  // S1
+  }
   tick(lead, 1, s);
   bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2
   tick(lead, 2, s);

@@ -117,6 +117,102 @@ void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, d
   table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table, centroid_rule);
 }
 
+// ---------------------------------------------------------------------------------------------- shared geometry (NEXT-3)
+// Cells that share one geometry and differ in their properties (the optimisation-loop batch of PAPER.md:15-17, 297):
+// the polygon integrals I_p(q_D) are evaluated once per geometry, one thread per (index difference, phase), into
+// Iph[p + D_half * P]; a cell's table is then T_c(D) = sum_p w_{c,p} I_p(q_D), a (7 ncells x P) x (P x nhalf) product that
+// runs on the DMMA GEMM, followed by the scatter into the cells' tables (with T(-D) = conj T(D)).
+__global__ void __launch_bounds__(128) phase_table_kernel(Geometry g, const int *__restrict__ poff, int Mt, cplx *__restrict__ Iph,
+                                                          int centroid_rule) {
+  const int L = 4 * Mt + 1, L2 = L * L, nhalf = (L2 + 1) / 2;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x, dh = blockIdx.y;
+  if (p >= g.P || dh >= nhalf) return;
+  const int flat = dh + (L2 - 1) / 2;
+  const int D1 = flat / L - 2 * Mt, D2 = flat % L - 2 * Mt;
+  cplx out;
+  if (D1 == 0 && D2 == 0) {
+    out = cmake(g.area[p], 0.0);
+  } else if (centroid_rule) {
+    const double phi = fma((double)D1, g.area[g.P + p], (double)D2 * g.area[2 * g.P + p]);
+    double sn, cs;
+    sincospi(2.0 * phi, &sn, &cs);
+    out = cmake(g.area[p] * cs, g.area[p] * sn);
+  } else {
+    const double qx = D1 * g.Q[0] + D2 * g.Q[2], qy = D1 * g.Q[1] + D2 * g.Q[3];
+    const int ne = g.nedge;
+    const double *mh1 = g.edge, *mh2 = g.edge + ne, *eh1 = g.edge + 2 * ne, *eh2 = g.edge + 3 * ne;
+    const double *ex = g.edge + 4 * ne, *ey = g.edge + 5 * ne;
+    double sr = 0.0, si = 0.0;
+    for (int e = poff[p]; e < poff[p + 1]; ++e) {
+      const double phi = fma((double)D1, mh1[e], (double)D2 * mh2[e]);  // q.m / (2 pi)
+      const double u = fma((double)D1, eh1[e], (double)D2 * eh2[e]);    // q.e / (2 pi)
+      double sn, cs;
+      sincospi(2.0 * phi, &sn, &cs);
+      const double j0 = (u == 0.0) ? 1.0 : sinpi(u) / (kPi * u);
+      const double f = (qx * ey[e] - qy * ex[e]) * j0;
+      sr = fma(f, cs, sr);
+      si = fma(f, sn, si);
+    }
+    const double inv = 1.0 / (qx * qx + qy * qy);
+    out = cmake(si * inv, -sr * inv);  // (-i) (sr + i si) / |q|^2
+  }
+  Iph[(size_t)dh * g.P + p] = out;
+}
+
+// W[(cell * 7 + c) + p * ldw] = (w_{c,p} of cell, 0): the weights of every cell of the batch as one complex matrix
+__global__ void __launch_bounds__(256) gather_weights_kernel(const Geometry *__restrict__ geos, int ncells, cplx *__restrict__ W) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x, cell = blockIdx.y;
+  const Geometry g = geos[cell];
+  if (p >= g.P) return;
+  const size_t ldw = (size_t)7 * ncells;
+#pragma unroll
+  for (int c = 0; c < 7; ++c) W[(size_t)cell * 7 + c + (size_t)p * ldw] = cmake(g.w[c * g.P + p], 0.0);
+}
+
+// table[c][flat] of every cell from Tst[(cell * 7 + c) + dh * ldt]; the mirrored half is the conjugate
+__global__ void __launch_bounds__(256) scatter_table_kernel(int Mt, int ncells, const cplx *__restrict__ Tst, BatchRef table) {
+  const int L = 4 * Mt + 1, L2 = L * L, nhalf = (L2 + 1) / 2;
+  const int dh = blockIdx.x * blockDim.x + threadIdx.x, cell = blockIdx.y;
+  if (dh >= nhalf) return;
+  const int flat = dh + (L2 - 1) / 2;
+  cplx *T = batch_ptr(table, cell, 0);
+  const size_t ldt = (size_t)7 * ncells;
+#pragma unroll
+  for (int c = 0; c < 7; ++c) {
+    cplx v = Tst[(size_t)cell * 7 + c + (size_t)dh * ldt];
+    if (dh == 0) v.y = 0.0;
+    T[(size_t)c * L2 + flat] = v;
+    T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(v.x, -v.y);
+  }
+}
+
+void launch_phase_table(const Geometry &g, const int *poff, int Mt, cplx *Iph, int centroid_rule, cudaStream_t s) {
+  const int L = 4 * Mt + 1, nhalf = (L * L + 1) / 2;
+  KScope ks(KC_TABLE, 230.0 * g.nedge * (double)nhalf, s);
+  phase_table_kernel<<<dim3((g.P + 127) / 128, nhalf), 128, 0, s>>>(g, poff, Mt, Iph, centroid_rule);
+}
+
+void launch_shared_tables(const Geometry *geos_dev, int ncells, int P, int Mt, const cplx *Iph, cplx *W, cplx *Tst,
+                          BatchRef table, cudaStream_t s) {
+  const int L = 4 * Mt + 1, nhalf = (L * L + 1) / 2;
+  {
+    KScope ks(KC_OTHER, 0.0, s);
+    gather_weights_kernel<<<dim3((P + 255) / 256, ncells), 256, 0, s>>>(geos_dev, ncells, W);
+  }
+  GemmDesc g{};
+  g.M = 7 * ncells; g.N = nhalf; g.K = P; g.opA = 0; g.opB = 0; g.lda = 7 * ncells; g.ldb = P; g.ldc = 7 * ncells;
+  g.ncells = 1; g.inner = 1; g.kclass = KC_TABLE;
+  g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+  g.A = BatchRef{nullptr, (unsigned long long)W, 0, 0};
+  g.B = BatchRef{nullptr, (unsigned long long)Iph, 0, 0};
+  g.C = BatchRef{nullptr, (unsigned long long)Tst, 0, 0};
+  launch_zgemm(g, s);
+  {
+    KScope ks(KC_OTHER, 0.0, s);
+    scatter_table_kernel<<<dim3((nhalf + 255) / 256, ncells), 256, 0, s>>>(Mt, ncells, Tst, table);
+  }
+}
+
 // S2: one thread per (g_alpha, g_beta): Phi[(a,ga),(b,gb)] = T_{c(a,b)}(D(gb) - D(ga)), R[ga,gb] = T_rho(...).
 // Consecutive threads -> consecutive rows ga (column-major stores coalesce; table reads are nearly contiguous).
 __global__ void __launch_bounds__(256) expand_kernel(int Mt, BatchRef table, BatchRef Phi, BatchRef R) {

@@ -136,6 +136,12 @@ struct Geometry {  // device pointers, per cell
 // S1: table[c][(D1+2Mt)*(4Mt+1) + (D2+2Mt)], c < 7.  geo: device array [ncells]; table at BatchRef (inner unused).
 void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
                   cudaStream_t s);
+// S1 for cells that share one geometry: Iph[p + dh * P] = I_p(q_D) once per geometry (poff: device [P+1] edge offsets of
+// the phases), then every cell's table as W (7 ncells x P) times Iph on the DMMA GEMM.  W, Tst: device scratch of
+// 7 ncells x P and 7 ncells x nhalf complex, nhalf = ((4Mt+1)^2 + 1) / 2.
+void launch_phase_table(const Geometry &g, const int *poff, int Mt, cplx *Iph, int centroid_rule, cudaStream_t s);
+void launch_shared_tables(const Geometry *geos_dev, int ncells, int P, int Mt, const cplx *Iph, cplx *W, cplx *Tst,
+                          BatchRef table, cudaStream_t s);
 // S2: Phi (3N x 3N full) and R (N x N full) from the table.
 void launch_expand(int ncells, int Mt, BatchRef table, BatchRef Phi, BatchRef R, cudaStream_t s);
 

@@ -486,3 +486,64 @@ def test_create_destroy_loop_reuses_device_blocks(bs):
             free0 = torch.cuda.mem_get_info()[0]
     torch.cuda.empty_cache()
     assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)
+
+
+def test_shared_geometry_batch_parity_and_property_updates(bs):
+    # cells that share one geometry; S1 = polygon integrals once + T = W I per cell.
+    # Matrices and bands against the oracle (which assembles every cell from scratch), against the per-cell path, and
+    # after new properties are set on existing handles (the optimisation-loop iteration).
+    w = wl.get("C4", ncells=6)
+    c0 = w.cells[0]
+    assert all(np.array_equal(c.verts, c0.verts) for c in w.cells)
+    comps = np.stack([bs.bs_isotropic_plane_strain(c.E, c.nu) for c in w.cells])
+    rhos = np.stack([c.rho for c in w.cells])
+    shared = bs.bs_create_cells_shared(c0.lattice, c0.vert_offset, c0.verts, comps, rhos)
+    for h in shared:
+        bs.allocate_workspace(h, w.Mt, w.nk)
+    bs.bs_assemble_batch(shared, w.Mt)
+    lam = bs.bs_bands_batch(shared, w.kpts, w.nbands)
+    single = [make_cell(bs, c, w.Mt, w.nk) for c in w.cells]
+    bs.bs_assemble_batch(single, w.Mt)
+    lam1 = bs.bs_bands_batch(single, w.kpts, w.nbands)
+    for ci in (0, 3, 5):
+        Pr, Sr = oracle.assemble(*oracle_inputs(w.cells[ci]), w.Mt)
+        Phi, Psi = bs.bs_get_matrices(shared[ci])
+        assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr))
+        assert np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+        assert np.array_equal(Phi, Phi.conj().T)
+        lr, lmax = oracle.band_structure(*oracle_inputs(w.cells[ci]), w.Mt, w.kpts, w.nbands)
+        check_bands(lam[ci], lr, lmax, f"shared cell{ci}")
+        check_bands(lam1[ci], lr, lmax, f"single cell{ci}")
+    # one cell of the shared set alone gives the same bits as inside the batch
+    bs.bs_assemble(shared[3], w.Mt)
+    assert np.array_equal(bs.bs_bands(shared[3], w.kpts, w.nbands), lam[3])
+    # optimisation-loop iteration: new properties on the same handles (cell j takes the materials of cell 5 - j)
+    for j, h in enumerate(shared):
+        bs.bs_set_properties(h, comps[5 - j], rhos[5 - j])
+    with pytest.raises(bs.BsError):
+        bs.bs_bands(shared[0], w.kpts, w.nbands)        # properties changed: must be assembled again
+    bs.bs_assemble_batch(shared, w.Mt)
+    lam2 = bs.bs_bands_batch(shared, w.kpts, w.nbands)
+    assert np.array_equal(lam2, lam[::-1])
+    # the centroid-rule quadrature goes through the shared path too
+    for h in shared:
+        bs.bs_set_option(h, bs.BS_OPT_ASSEMBLY, bs.BS_ASSEMBLY_CENTROID)
+    bs.bs_assemble_batch(shared, 1)      # (at Mt = 5 the one-point rule aliases on the 8 x 8 pixels: Phi is then singular)
+    Phi, _ = bs.bs_get_matrices(shared[1])
+    Pc, _ = oracle.assemble(*oracle_inputs(w.cells[4]), 1, quadrature="centroid")
+    assert np.max(np.abs(Phi - Pc)) <= 1e-12 * np.max(np.abs(Pc))
+    # anisotropic phases and a skew lattice through the shared path
+    cell = wl.random_small_cell(21, 3, np.array([[1.0, 0.0], [0.3, 0.8]]))
+    comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu).copy()
+    comp[:, 3] = 0.01 * comp[:, 0]
+    comp[:, 4] = -0.02 * comp[:, 0]
+    comp[:, 1] *= 1.1
+    hs = bs.bs_create_cells_shared(cell.lattice, cell.vert_offset, cell.verts, np.stack([comp, 2 * comp]), np.stack([cell.rho, cell.rho]))
+    for h in hs:
+        bs.allocate_workspace(h, 2, 2)
+    bs.bs_assemble_batch(hs, 2)
+    Phi, Psi = bs.bs_get_matrices(hs[1])
+    Pr, Sr = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, 2 * comp, cell.rho, 2)
+    assert np.max(np.abs(Phi - Pr)) <= 1e-12 * np.max(np.abs(Pr)) and np.max(np.abs(Psi - Sr)) <= 1e-12 * np.max(np.abs(Sr))
+    for h in shared + single + hs:
+        bs.bs_destroy_cell(h)

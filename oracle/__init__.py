@@ -20,6 +20,7 @@ from .bandstructure import (  # noqa: F401
     coupling_B,
     pencil_K,
     bands_at_k,
+    modes_at_k,
     band_structure,
     omega_svd_route,
 )

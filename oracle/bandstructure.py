@@ -267,6 +267,21 @@ def bands_at_k(Phi, Psi, lattice, Mt, kred, nbands=None):
     return (lam if nbands is None else lam[:nbands]), lam_max
 
 
+def modes_at_k(Phi, Psi, lattice, Mt, kred, nbands):
+    """Mode shapes of the lowest nbands branches at one k-point ("the eigenvectors U give the displacement
+    mode shapes and S = -Phi^-1 H* U the stress mode shapes").  In the notation used here the paper's
+    H* is -H with H = V B(k) (reading R3), so  S = Phi^-1 H U  and eq. 10 reads  Phi S = H U,
+    H^dagger S = lambda Psi U.  zhegv with vectors: the columns of U are Psi-orthonormal, U^dagger Psi U = I.
+    Returns (lam (nbands,), U (2N, nbands), S (3N, nbands))."""
+    _, _, V = reciprocal_basis(lattice)
+    H = V * coupling_B(lattice, Mt, kred)
+    K = pencil_K(Phi, lattice, Mt, kred)
+    lam, U = sla.eigh(K, Psi, driver="gv")
+    U = U[:, :nbands]
+    S = np.linalg.solve(Phi, H @ U)
+    return lam[:nbands], U, S
+
+
 def band_structure(lattice, vert_offset, verts, compliance, density, Mt, kpts, nbands):
     """Whole path: assemble once, then lambda[k, band] for every reduced k-point.  Returns
     (lam (nk,nbands), lam_max (nk,))."""

@@ -377,3 +377,62 @@ def test_centroid_rule_is_the_leading_term_and_converges():
         errs.append(np.max(np.abs(ex - ce)) / np.max(np.abs(ex)))
     assert errs[0] > errs[1] > errs[2] and errs[2] < 2e-2
     assert 3.5 < errs[0] / errs[1] < 4.6 and 3.8 < errs[1] / errs[2] < 4.2
+
+
+# ----------------------------------------------------------------------------- mode shapes (NEXT-1)
+def test_modes_homogeneous_cell_are_polarised_plane_waves_with_hooke_stress():
+    # PAPER.md:104.  Homogeneous isotropic cell: every eigenvector is one plane wave exp(i kappa.x) polarised along kappa
+    # (longitudinal, omega = c_L |kappa|) or across it (transverse, c_T |kappa|); its stress coefficients obey Hooke's law
+    # sigma = C eps with eps = i Bt(kappa) p (textbook), i.e. S = i C Bt p on that plane wave.  Catches: a transposed or
+    # conjugated U, the sign of S (the paper's H* is minus this H), a missing factor V, a stress ordering mistake.
+    E, nu, rho = 20e9, 0.28, 2500.0
+    c = wl.homogeneous_cell(HEX, E, nu, rho, n=2)
+    comp = oracle.isotropic_plane_strain_compliance(c.E, c.nu)
+    Mt = 2
+    N = (2 * Mt + 1) ** 2
+    Phi, Psi = oracle.assemble(c.lattice, c.vert_offset, c.verts, comp, c.rho, Mt)
+    lam_, mu_ = E * nu / ((1 + nu) * (1 - 2 * nu)), E / (2 * (1 + nu))
+    Cst = np.array([[lam_ + 2 * mu_, lam_, 0], [lam_, lam_ + 2 * mu_, 0], [0, 0, mu_]])   # textbook plane-strain stiffness
+    _, Q, V = oracle.reciprocal_basis(HEX)
+    kred = (0.31, 0.12)                                  # generic point: all 2N eigenvalues distinct
+    kap = (oracle.plane_wave_indices(Mt) + np.array(kred)) @ Q
+    lam, U, S = oracle.modes_at_k(Phi, Psi, HEX, Mt, kred, 2 * N)
+    assert np.allclose(U.conj().T @ Psi @ U, np.eye(2 * N), atol=1e-10)
+    seen = set()
+    for j in range(2 * N):
+        u1, u2 = U[:N, j], U[N:, j]
+        g = int(np.argmax(np.abs(u1) ** 2 + np.abs(u2) ** 2))
+        rest = np.delete(np.abs(u1) ** 2 + np.abs(u2) ** 2, g).sum()
+        assert rest < 1e-16 * (abs(u1[g]) ** 2 + abs(u2[g]) ** 2)            # a single plane wave
+        p = np.array([u1[g], u2[g]])
+        khat = kap[g] / np.linalg.norm(kap[g])
+        along, across = abs(khat @ p), abs(khat[0] * p[1] - khat[1] * p[0])
+        cph = np.sqrt(lam[j]) / np.linalg.norm(kap[g])
+        if abs(cph - np.sqrt((lam_ + 2 * mu_) / rho)) < 1e-6 * cph:
+            assert across < 1e-9 * along                                       # longitudinal: polarised along kappa
+            seen.add((g, "L"))
+        else:
+            assert abs(cph - np.sqrt(mu_ / rho)) < 1e-6 * cph and along < 1e-9 * across
+            seen.add((g, "T"))
+        Bt = np.array([[kap[g][0], 0.0], [0.0, kap[g][1]], [kap[g][1], kap[g][0]]])
+        sig = 1j * Cst @ Bt @ p                                                # Hooke: sigma = C (i Bt p)
+        got = np.array([S[g, j], S[N + g, j], S[2 * N + g, j]])
+        assert np.max(np.abs(got - sig)) < 1e-9 * np.max(np.abs(sig))
+        others = np.delete(np.abs(S[:, j]), [g, N + g, 2 * N + g])
+        assert others.max() < 1e-9 * np.max(np.abs(sig))
+    assert len(seen) == 2 * N                                                  # every plane wave once per polarisation
+
+
+def test_modes_satisfy_the_mixed_system_of_eq10():
+    # PAPER.md:94-97 (eq. 10) on a heterogeneous skew cell:  Phi S = H U  and  H^dagger S = lambda Psi U
+    c, comp = _small_cell(seed=17, n=3, lattice=np.array([[1.0, 0.0], [0.3, 0.8]]))
+    Mt = 2
+    Phi, Psi = oracle.assemble(c.lattice, c.vert_offset, c.verts, comp, c.rho, Mt)
+    _, _, V = oracle.reciprocal_basis(c.lattice)
+    kred = (0.2, -0.35)
+    lam, U, S = oracle.modes_at_k(Phi, Psi, c.lattice, Mt, kred, 9)
+    H = V * oracle.coupling_B(c.lattice, Mt, kred)
+    assert np.max(np.abs(Phi @ S - H @ U)) < 1e-10 * np.max(np.abs(H @ U))
+    assert np.max(np.abs(H.conj().T @ S - (Psi @ U) * lam[None, :])) < 1e-9 * np.max(np.abs(H.conj().T @ S))
+    lam2, _ = oracle.bands_at_k(Phi, Psi, c.lattice, Mt, kred, 9)
+    assert np.allclose(lam, lam2, rtol=1e-12)

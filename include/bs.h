@@ -172,6 +172,25 @@ bs_status bs_bands(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands
 bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, const double *kpts, int32_t nbands,
                          double *omega2_out, void *stream);
 
+/* BS_OPT_MODES (option 7): the largest number of mode shapes per k-point bs_modes may be asked for (0 = off, default).
+ * Set it BEFORE bs_workspace_bytes / bs_assemble: the workspace then also holds the reflectors of the band reduction, a
+ * copy of the band and the vectors (about 2N x 2N complex more per k-point). */
+enum { BS_OPT_MODES = 7 };
+
+/* Mode shapes of the lowest nbands branches ("the eigenvectors U give the displacement mode shapes and
+ * S = -Phi^-1 H* U the stress mode shapes").  One handle, nk k-points.
+ *   omega2_out  nk x nbands doubles as bs_bands (host or device).
+ *   U_out       nk blocks of 2N x nbands complex128, column-major (column j = displacement coefficients (u1 | u2) of band j
+ *               on the N plane waves, Psi-orthonormal: U^dagger Psi U = I); host or device; may be NULL.
+ *   S_out       nk blocks of 3N x nbands: stress coefficients (s11 | s22 | s12), S = Phi^-1 H U with H = V B(k) (the paper's
+ *               H* is -H, R3), so that Phi S = H U and H^dagger S = lambda Psi U (eq. 10); may be NULL.
+ * Phases and, inside a degenerate eigenvalue, the basis are arbitrary.  Method: the eigenvalues as bs_bands; eigenvectors of
+ * the Hermitian band matrix of S6 stage 1 by inverse iteration (pivoted band LU, modified Gram-Schmidt inside clusters);
+ * back-transformation through the block reflectors of stage 1 and L_Psi^-H.  Synchronises the stream.
+ * Errors: BS_ERR_STATE (BS_OPT_MODES not set, or omega output selected), BS_ERR_ARG (nbands > BS_OPT_MODES), as bs_bands. */
+bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *U_out,
+                   void *S_out, void *stream);
+
 /* Parity access after bs_bands: the tridiagonal T(k) of the last call, HOST out: d (nk x 2N), e (nk x 2N, last unused). */
 bs_status bs_get_tridiagonal(bs_cell *cell, double *d_host, double *e_host);
 

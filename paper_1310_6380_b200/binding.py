@@ -22,6 +22,7 @@ BS_TRIDIAG_TWO_STAGE, BS_TRIDIAG_ONE_STAGE, BS_TRIDIAG_TWO_STAGE_STREAMED = 0, 1
 BS_OPT_ASSEMBLY = 4
 BS_OPT_PHI_INVERSE = 5
 BS_OPT_OUTPUT = 6
+BS_OPT_MODES = 7
 BS_OUTPUT_OMEGA2, BS_OUTPUT_OMEGA = 0, 1
 BS_ASSEMBLY_EXACT, BS_ASSEMBLY_CENTROID = 0, 1
 BS_PENCIL_POLY, BS_PENCIL_DIRECT = 0, 1
@@ -32,7 +33,7 @@ BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_K
 SYMBOLS = [
     "bs_isotropic_plane_strain", "bs_create_cell", "bs_create_cells_shared", "bs_set_properties", "bs_destroy_cell", "bs_set_option", "bs_workspace_bytes",
     "bs_set_workspace", "bs_assemble", "bs_assemble_batch", "bs_get_matrices", "bs_get_table", "bs_get_pencil",
-    "bs_bands", "bs_bands_batch", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
+    "bs_bands", "bs_bands_batch", "bs_modes", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
     "bs_last_error",
     "bs_fp64_peak", "bs_zgemm", "bs_zpotrf_trtri", "bs_zhetrd_scratch_elems", "bs_zhetrd", "bs_sturm",
 ]
@@ -79,6 +80,7 @@ lib.bs_get_table.argtypes = [_vp, _vp]
 lib.bs_get_pencil.argtypes = [_vp, _dp, _vp, _vp]
 lib.bs_bands.argtypes = [_vp, C.c_int32, _dp, C.c_int32, _vp, _vp]
 lib.bs_bands_batch.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int32, _dp, C.c_int32, _vp, _vp]
+lib.bs_modes.argtypes = [_vp, C.c_int32, _dp, C.c_int32, _vp, _vp, _vp, _vp]
 lib.bs_get_tridiagonal.argtypes = [_vp, _dp, _dp]
 lib.bs_get_timings.argtypes = [_vp, _dp]
 lib.bs_get_kernel_timings.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int64)]
@@ -294,6 +296,20 @@ def bs_bands_batch(cells: Sequence[Cell], kpts, nbands: int, out=None, stream=No
     _check(lib.bs_bands_batch(_handles(cells), len(cells), nk, _ptr(k), nbands, p, _stream(stream)))
     cells[0].last_nmat = len(cells) * nk
     return out
+
+
+def bs_modes(cell: Cell, kpts, nbands: int, stress: bool = True, stream=None):
+    """Mode shapes: returns (omega2 (nk, nbands), U (nk, 2N, nbands), S (nk, 3N, nbands) or None) as host
+    NumPy arrays; U[k][:, j] is the Psi-orthonormal displacement coefficient vector of band j."""
+    k = _f64(kpts).reshape(-1, 2)
+    nk, N = k.shape[0], cell.N
+    lam = np.empty((nk, nbands))
+    U = np.empty((nk, nbands, 2 * N), dtype=np.complex128)          # block k is column-major 2N x nbands
+    S = np.empty((nk, nbands, 3 * N), dtype=np.complex128) if stress else None
+    _check(lib.bs_modes(cell.handle, nk, _ptr(k), nbands, C.c_void_p(lam.ctypes.data), C.c_void_p(U.ctypes.data),
+                        C.c_void_p(S.ctypes.data) if stress else None, _stream(stream)))
+    cell.last_nmat = nk
+    return lam, U.transpose(0, 2, 1), (S.transpose(0, 2, 1) if stress else None)
 
 
 def bs_get_tridiagonal(cell: Cell, nmat: Optional[int] = None):

@@ -13,7 +13,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libbs.so")
-SOURCES = ["api.cu", "assemble.cu", "factor.cu", "zgemm.cu", "pencil.cu", "tridiag.cu", "band.cu", "chase.cu", "small.cu", "sturm.cu", "probe.cu"]
+SOURCES = ["api.cu", "assemble.cu", "factor.cu", "zgemm.cu", "pencil.cu", "tridiag.cu", "band.cu", "chase.cu", "small.cu", "sturm.cu", "modes.cu", "probe.cu"]
 # chase.cu: no implicit multiply-add contraction, so that the step function inlined into the resident and the streamed
 # kernel rounds identically in both (explicit fma() calls still compile to DFMA)
 EXTRA_FLAGS = {"chase.cu": ["-fmad=false"]}

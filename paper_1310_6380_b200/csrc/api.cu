@@ -42,6 +42,10 @@ struct Layout {
   int Mt = -1, N = 0, nk = 0, mode = 0, nb = 0;
   long long table, Phi, R, Lf, X, tmp, dinv, Y, LR, XR, tmpR, dinvR, kvecA, Coef, Tb, kvecK, Kk, Ak, VW, P, SM, AB;
   long long vw_stride, sm_stride, ab_stride;
+  // mode shapes (BS_OPT_MODES = nvmax > 0): kept reflectors of stage 1, a copy of the band, vectors and scratch
+  int nvmax = 0;
+  long long Vall, Tall, AB2, Zv, LU, Uv, HU, Sv, Wa, Wb, kapm;
+  long long lu_stride;
   long long total;  // elements
 };
 
@@ -54,10 +58,10 @@ int band_width(int nb) { return nb >= 32 ? 32 : (nb >= 16 ? 16 : 8); }  // two-s
 // that much again at this size).  The choice does not depend on the batch, so a batch and its members take the same path.
 int auto_band_width(int n) { (void)n; return 16; }
 
-Layout make_layout(int Mt, int nk, int mode, int nb_opt) {
+Layout make_layout(int Mt, int nk, int mode, int nb_opt, int nvmax = 0) {
   const int nb = nb_opt > 0 ? nb_opt : 32;  // automatic band width: sized for the widest
   Layout L;
-  L.Mt = Mt; L.nk = nk; L.mode = mode; L.nb = nb_opt;
+  L.Mt = Mt; L.nk = nk; L.mode = mode; L.nb = nb_opt; L.nvmax = nvmax;
   const long long W = 2 * Mt + 1, N = W * W, n3 = 3 * N, n2 = 2 * N, Lt = 4 * Mt + 1;
   L.N = (int)N;
   long long o = 0;
@@ -88,6 +92,20 @@ Layout make_layout(int Mt, int nk, int mode, int nb_opt) {
   L.P = take((long long)nk * (long long)bsk::tridiag_p_elems((int)n2));
   L.SM = take((long long)nk * L.sm_stride);
   L.AB = take((long long)nk * L.ab_stride);
+  if (nvmax > 0) {
+    L.Vall = take((long long)nk * n2 * n2);
+    L.Tall = take((long long)nk * n2 * 32);           // (n / b) panels of b^2 <= n * 32
+    L.AB2 = take((long long)nk * L.ab_stride);
+    L.Zv = take((long long)nk * n2 * nvmax);
+    L.lu_stride = align16((long long)bsk::band_invit_lu_elems((int)n2, 32));
+    L.LU = take((long long)nk * L.lu_stride);
+    L.Uv = take((long long)nk * n2 * nvmax);
+    L.HU = take((long long)nk * n3 * nvmax);
+    L.Sv = take((long long)nk * n3 * nvmax);
+    L.Wa = take((long long)nk * 32 * nvmax);
+    L.Wb = take((long long)nk * 32 * nvmax);
+    L.kapm = take((long long)nk * N);                 // nk x [2][N] doubles
+  }
   L.total = o;
   return L;
 }
@@ -136,6 +154,9 @@ struct bs_cell {
   int last_n = 0, last_nmat = 0, last_nk = 0;
   cudaEvent_t ev[BS_T_COUNT + 1] = {nullptr};
   bsk::KTimer *kt = nullptr;  // BS_OPT_TIMING = 2
+  int nvmax = 0;                  // BS_OPT_MODES: bs_modes may return up to this many mode shapes per k-point
+  bool keep_modes = false;        // set by bs_modes around its bs_bands pass: stage 1 keeps its reflectors and the band
+  double *last_lam = nullptr;     // device eigenvalues of the last bs_bands pass (nmat x nbands)
   SharedGeom *shared = nullptr;   // bs_create_cells_shared
   cplx *d_sh = nullptr;           // lead handle: weights matrix and stacked tables of the shared-geometry S1
   size_t sh_cap = 0;
@@ -576,6 +597,11 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       if (value != BS_OUTPUT_OMEGA2 && value != BS_OUTPUT_OMEGA) return fail(BS_ERR_ARG, "bs_set_option: bad output mode");
       c->out_root = value;
       return BS_OK;
+    case BS_OPT_MODES:
+      if (value < 0 || value > 2048) return fail(BS_ERR_ARG, "bs_set_option: BS_OPT_MODES must be 0..2048");
+      if (c->nvmax != value) c->assembled = false;
+      c->nvmax = value;
+      return BS_OK;
     case BS_OPT_TIMING:
       if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
       c->timing = value;
@@ -589,7 +615,7 @@ bs_status bs_workspace_bytes(const bs_cell *c, int32_t Mt, int32_t nk, size_t *b
   if (!c || !bytes || Mt < 0 || nk < 1) return fail(BS_ERR_ARG, "bs_workspace_bytes: bad argument");
   const long long n2 = 2LL * (2 * Mt + 1) * (2 * Mt + 1);
   if (n2 > 2048) return fail(BS_ERR_ARG, "bs_workspace_bytes: 2N = %lld exceeds 2048", n2);
-  *bytes = (size_t)make_layout(Mt, nk, c->mode, c->nb).total * sizeof(cplx);
+  *bytes = (size_t)make_layout(Mt, nk, c->mode, c->nb, c->nvmax).total * sizeof(cplx);
   return BS_OK;
 }
 
@@ -704,7 +730,7 @@ bs_status check_batch(bs_cell *const *cells, int ncells, const char *who) {
     if (!cells[c]) return fail(BS_ERR_ARG, "%s: cells[%d] is null", who, c);
     if (!cells[c]->ws) return fail(BS_ERR_NOMEM, "%s: cells[%d] has no workspace (bs_set_workspace)", who, c);
     if (cells[c]->mode != cells[0]->mode || cells[c]->nb != cells[0]->nb || cells[c]->algo != cells[0]->algo ||
-        cells[c]->quad != cells[0]->quad || cells[c]->phi_general != cells[0]->phi_general || cells[c]->out_root != cells[0]->out_root)
+        cells[c]->quad != cells[0]->quad || cells[c]->nvmax != cells[0]->nvmax || cells[c]->phi_general != cells[0]->phi_general || cells[c]->out_root != cells[0]->out_root)
       return fail(BS_ERR_ARG, "%s: cells[%d] has different options than cells[0]", who, c);
     // one V^2 scales K(k) of every cell of a launch (both pencil modes): the cells of a batch share the cell area
     if (cells[c]->V != cells[0]->V)
@@ -727,7 +753,7 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
   if (2 * N > 2048) return fail(BS_ERR_ARG, "bs_assemble: 2N = %lld exceeds 2048", 2 * N);
   bs_cell *lead = cells[0];
   cudaStream_t s = (cudaStream_t)stream;
-  const Layout L = make_layout(Mt, 1, lead->mode, lead->nb);
+  const Layout L = make_layout(Mt, 1, lead->mode, lead->nb, lead->nvmax);
   for (int c = 0; c < ncells; ++c) {
     cells[c]->assembled = false;
     if ((size_t)L.total * sizeof(cplx) > cells[c]->ws_bytes)
@@ -904,7 +930,7 @@ bs_status bs_get_pencil(bs_cell *c, const double kred[2], void *K_host, void *st
   if (!c || !kred || !K_host) return fail(BS_ERR_ARG, "bs_get_pencil: null argument");
   if (!c->assembled) return fail(BS_ERR_STATE, "bs_get_pencil: call bs_assemble first");
   cudaStream_t s = (cudaStream_t)stream;
-  const Layout L = make_layout(c->lay.Mt, 1, c->mode, c->nb);
+  const Layout L = make_layout(c->lay.Mt, 1, c->mode, c->nb, c->nvmax);
   const int N = L.N, n2 = 2 * N, n3 = 3 * N;
   std::vector<double> kv;
   fill_direct_kvec(c, L.Mt, 1, kred, kv);
@@ -934,7 +960,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
     if (cells[c]->lay.Mt != lead->lay.Mt) return fail(BS_ERR_ARG, "bs_bands: cells[%d] has a different truncation", c);
   }
   const int Mt = lead->lay.Mt;
-  const Layout L = make_layout(Mt, nk, lead->mode, lead->nb);
+  const Layout L = make_layout(Mt, nk, lead->mode, lead->nb, lead->nvmax);
   const int N = L.N, n2 = 2 * N, n3 = 3 * N;
   if (nbands < 1 || nbands > n2) return fail(BS_ERR_ARG, "bs_bands: nbands must be in 1..2N = %d", n2);
   if ((long long)ncells * nk > 65535) return fail(BS_ERR_ARG, "bs_bands: ncells * nk = %lld exceeds 65535 matrices per call", (long long)ncells * nk);
@@ -982,7 +1008,15 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
     nl += reduce_blocks(lead, cells, ncells, L, L.Kk, L.Ak, nk, s);                                                        // S5
   }
   tick(lead, 1, s);
-  if (lead->algo == BS_TRIDIAG_ONE_STAGE) {
+  if (lead->keep_modes) {
+    // mode shapes wanted: always the two-stage reduction, with the reflectors of stage 1 and a copy of the band kept
+    const int bw = lead->nb > 0 ? band_width(lead->nb) : auto_band_width(n2);
+    const BatchRef kv = R(L.Vall, mat), kt2 = R(L.Tall, (long long)n2 * 32);
+    nl += bsk::launch_sy2sb(n2, n2, bw, R(L.Ak, mat), R(L.VW, L.vw_stride), R(L.SM, L.sm_stride), R(L.AB, L.ab_stride),
+                            ncells, nk, s, &kv, &kt2);
+    bsk::launch_copy_matrix(2 * bw, n2, R(L.AB, L.ab_stride), 2 * bw, R(L.AB2, L.ab_stride), 2 * bw, ncells, nk, s); ++nl;
+    bsk::launch_sb2st(n2, bw, R(L.AB, L.ab_stride), d, e, ncells, nk, s, false, 0, chase_sync); ++nl;
+  } else if (lead->algo == BS_TRIDIAG_ONE_STAGE) {
     nl += bsk::launch_tridiag(n2, n2, lead->nb > 0 ? lead->nb : 32, R(L.Ak, mat), R(L.VW, L.vw_stride),
                               R(L.P, (long long)bsk::tridiag_p_elems(n2)), d, e, scal, ncells, nk, s);  // S6
   } else if (n2 <= bsk::tridiag_small_max_n()) {
@@ -999,6 +1033,7 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
   tick(lead, 3, s);
   lead->launches += nl;
   lead->last_n = n2; lead->last_nmat = (int)nmat; lead->last_nk = nk;
+  lead->last_lam = lam;
   // S8: one copy of ncells x nk x nbands doubles
   cudaPointerAttributes attr;
   bool on_device = false;
@@ -1020,6 +1055,114 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
 bs_status bs_bands(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *stream) {
   if (!cell) return fail(BS_ERR_ARG, "bs_bands: null handle");
   return bs_bands_batch(&cell, 1, nk, kpts, nbands, omega2_out, stream);
+}
+
+// Copies `count` blocks of `block` complex elements with source pitch `src_pitch` (elements) to a dense destination on the
+// host or the device.
+static bs_status copy_blocks(void *dst, const cplx *src, size_t block, size_t src_pitch, size_t count, cudaStream_t s) {
+  cudaPointerAttributes attr;
+  bool on_device = false;
+  if (cudaPointerGetAttributes(&attr, dst) == cudaSuccess) on_device = attr.type == cudaMemoryTypeDevice;
+  else cudaGetLastError();
+  CU(cudaMemcpy2DAsync(dst, block * sizeof(cplx), src, src_pitch * sizeof(cplx), block * sizeof(cplx), count,
+                       on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+  return BS_OK;
+}
+
+bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *U_out, void *S_out,
+                   void *stream) {
+  if (!cell || !kpts || !omega2_out || (!U_out && !S_out)) return fail(BS_ERR_ARG, "bs_modes: null argument");
+  if (cell->nvmax < 1) return fail(BS_ERR_STATE, "bs_modes: set BS_OPT_MODES (before sizing the workspace and bs_assemble) first");
+  if (nbands < 1 || nbands > cell->nvmax) return fail(BS_ERR_ARG, "bs_modes: nbands must be in 1..BS_OPT_MODES = %d", cell->nvmax);
+  if (cell->out_root) return fail(BS_ERR_STATE, "bs_modes: needs BS_OPT_OUTPUT = BS_OUTPUT_OMEGA2");
+  cudaStream_t s = (cudaStream_t)stream;
+  // S4..S7 with the reflectors of stage 1 and the band kept
+  cell->keep_modes = true;
+  bs_status st = bs_bands_batch(&cell, 1, nk, kpts, nbands, omega2_out, stream);
+  cell->keep_modes = false;
+  if (st != BS_OK) return st;
+  bs_cell *cells[1] = {cell};
+  const int Mt = cell->lay.Mt;
+  const Layout L = make_layout(Mt, nk, cell->mode, cell->nb, cell->nvmax);
+  const int N = L.N, n2 = 2 * N, n3 = 3 * N, nv = cell->nvmax;
+  const int bw = cell->nb > 0 ? band_width(cell->nb) : auto_band_width(n2);
+  auto R = [&](long long off, long long stride = 0) { return ref(cell, 1, cells, off, stride); };
+  const long long zs = (long long)n2 * nv;
+  int64_t nl = 0;
+  // 1. eigenvectors of the band matrix by inverse iteration at the eigenvalues of S7
+  bsk::launch_band_invit(n2, bw, R(L.AB2, L.ab_stride), cell->last_lam, nbands, R(L.Zv, zs), R(L.LU, L.lu_stride), 1, nk, s); ++nl;
+  // 2. back through the block reflectors of stage 1, last panel first: Z[r0:] -= V (T (V^H Z[r0:]))
+  int c_last = -1;
+  for (int c0 = 0; c0 + bw < n2 - 1; c0 += bw) c_last = c0;
+  for (int c0 = c_last; c0 >= 0; c0 -= bw) {
+    const int r0 = c0 + bw, m = n2 - r0;
+    bsk::GemmDesc g{};
+    g.ncells = 1; g.inner = nk; g.kclass = bsk::KC_OTHER;
+    g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+    g.M = bw; g.N = nbands; g.K = m; g.opA = 1; g.opB = 0;
+    g.A = R(L.Vall + (long long)c0 * n2 + r0, (long long)n2 * n2); g.lda = n2;
+    g.B = R(L.Zv + r0, zs); g.ldb = n2;
+    g.C = R(L.Wa, 32LL * nv); g.ldc = bw;
+    bsk::launch_zgemm(g, s);
+    g.M = bw; g.N = nbands; g.K = bw; g.opA = 0;
+    g.A = R(L.Tall + (long long)(c0 / bw) * bw * bw, (long long)n2 * 32); g.lda = bw;
+    g.B = R(L.Wa, 32LL * nv); g.ldb = bw;
+    g.C = R(L.Wb, 32LL * nv); g.ldc = bw;
+    bsk::launch_zgemm(g, s);
+    g.M = m; g.N = nbands; g.K = bw;
+    g.A = R(L.Vall + (long long)c0 * n2 + r0, (long long)n2 * n2); g.lda = n2;
+    g.B = R(L.Wb, 32LL * nv); g.ldb = bw;
+    g.C = R(L.Zv + r0, zs); g.ldc = n2;
+    g.alpha = cmake(-1.0, 0.0); g.beta = cmake(1.0, 0.0);
+    bsk::launch_zgemm(g, s);
+    nl += 3;
+  }
+  // 3. U = L_Psi^-H y = diag(X_R^H, X_R^H) y   (U^H Psi U = y^H y = I)
+  for (int blk = 0; blk < 2; ++blk) {
+    bsk::GemmDesc g{};
+    g.ncells = 1; g.inner = nk; g.kclass = bsk::KC_OTHER;
+    g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+    g.M = N; g.N = nbands; g.K = N; g.opA = 1; g.opB = 0;
+    g.A = R(L.XR, 0); g.lda = N;
+    g.B = R(L.Zv + (long long)blk * N, zs); g.ldb = n2;
+    g.C = R(L.Uv + (long long)blk * N, zs); g.ldc = n2;
+    bsk::launch_zgemm(g, s); ++nl;
+  }
+  // 4. S = Phi^-1 H U with H = V B(k) (the paper's S = -Phi^-1 H* U; its H* is -H, R3)
+  if (S_out) {
+    std::vector<double> kv((size_t)nk * 2 * N);
+    const int W = 2 * Mt + 1;
+    for (int k = 0; k < nk; ++k)
+      for (int a1 = -Mt; a1 <= Mt; ++a1)
+        for (int a2 = -Mt; a2 <= Mt; ++a2) {
+          const int g = (a1 + Mt) * W + (a2 + Mt);
+          const double f1 = kpts[2 * k] + a1, f2 = kpts[2 * k + 1] + a2;
+          kv[((size_t)k * 2 + 0) * N + g] = f1 * cell->Q[0] + f2 * cell->Q[2];
+          kv[((size_t)k * 2 + 1) * N + g] = f1 * cell->Q[1] + f2 * cell->Q[3];
+        }
+    double *kap = reinterpret_cast<double *>((cplx *)cell->ws + L.kapm);
+    CU(cudaMemcpyAsync(kap, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    const long long hs = (long long)n3 * nv;
+    bsk::launch_apply_h(N, cell->V, R(L.Uv, zs), n2, R(L.HU, hs), n3, kap, nbands, 1, nk, s); ++nl;
+    bsk::GemmDesc g{};
+    g.ncells = 1; g.inner = nk; g.kclass = bsk::KC_OTHER;
+    g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+    g.M = n3; g.N = nbands; g.K = n3; g.opA = 0; g.opB = 0;
+    g.A = R(L.Y, 0); g.lda = n3;
+    g.B = R(L.HU, hs); g.ldb = n3;
+    g.C = R(L.Sv, hs); g.ldc = n3;
+    bsk::launch_zgemm(g, s); ++nl;
+    st = copy_blocks(S_out, (cplx *)cell->ws + L.Sv, (size_t)n3 * nbands, (size_t)hs, nk, s);
+    if (st != BS_OK) return st;
+  }
+  if (U_out) {
+    st = copy_blocks(U_out, (cplx *)cell->ws + L.Uv, (size_t)n2 * nbands, (size_t)zs, nk, s);
+    if (st != BS_OK) return st;
+  }
+  cell->launches += nl;
+  CU(cudaStreamSynchronize(s));
+  CU(cudaGetLastError());
+  return BS_OK;
 }
 
 bs_status bs_get_tridiagonal(bs_cell *c, double *d_host, double *e_host) {

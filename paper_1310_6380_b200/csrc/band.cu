@@ -356,7 +356,7 @@ size_t band_ab_elems(int n, int b) { return (size_t)n * 2 * b; }
 
 // Stage 1 for every matrix of the batch in lock step; on exit AB holds the band (ldab = 2b, bulge space zeroed).
 int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, BatchRef AB, int ncells, int inner,
-                 cudaStream_t s) {
+                 cudaStream_t s, const BatchRef *keepV, const BatchRef *keepT) {
   int launches = 0;
   const int nmat = ncells * inner;
   static unsigned long long m1 = 0, m2 = 0, m3 = 0, m4 = 0;
@@ -402,6 +402,15 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
       // few matrices: one thread per entry (latency); many: smaller CTAs, several per SM (throughput)
       wy_small_kernel<<<nmat, nmat > 592 ? 256 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
       ++launches;
+    }
+    if (keepV) {  // mode shapes: V and T of this panel are needed again for the back-transformation
+      BatchRef src = VW, dst = *keepV;
+      src.off += r0;
+      dst.off += (long long)c0 * n + r0;
+      launch_copy_matrix(m, b, src, n, dst, n, ncells, inner, s); ++launches;
+      src = SM; src.off += (long long)2 * b * b + b;   // T inside [M2; T] (ld 2b)
+      dst = *keepT; dst.off += (long long)(c0 / b) * b * b;
+      launch_copy_matrix(b, b, src, 2 * b, dst, b, ncells, inner, s); ++launches;
     }
     // X = [V | Z] [M2; T]
     g.M = m; g.N = b; g.K = 2 * b; g.opA = 0; g.opB = 0; g.flags = 0;

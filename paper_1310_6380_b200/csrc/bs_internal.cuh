@@ -187,8 +187,10 @@ int launch_tridiag(int n, int lda, int nb, BatchRef A, BatchRef VW, BatchRef P, 
 size_t band_vw_elems(int n, int b);
 size_t band_sm_elems(int b);
 size_t band_ab_elems(int n, int b);
+// keepV / keepT (optional, for the mode shapes): the reflectors of every panel are also stored, V of the panel at columns
+// c0 .. c0+b-1 in keepV (n x n per matrix, ld n, rows r0 .. n-1 written) and its compact-WY T in keepT + (c0 / b) b^2.
 int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, BatchRef AB, int ncells, int inner,
-                 cudaStream_t s);
+                 cudaStream_t s, const BatchRef *keepV = nullptr, const BatchRef *keepT = nullptr);
 // streamed: stream the band through the ring even when it would fit shared memory; force_g > 0: at most that many
 // sweeps per train (test knob); sync: device scratch of sb2st_sync_ints(n, nmat) ints (task counter + train progress)
 void launch_sb2st(int n, int b, BatchRef AB, double *d, double *e, int ncells, int inner, cudaStream_t s, bool streamed,
@@ -198,6 +200,14 @@ bool bulge_band_resident(int n, int b);  // stage 2 keeps the whole band of widt
 // S6 for n <= tridiag_small_max_n(): the matrix in shared memory, one CTA per matrix, unblocked Householder (small.cu).
 int tridiag_small_max_n();
 void launch_tridiag_small(int n, int lda, BatchRef A, double *d, double *e, int ncells, int inner, cudaStream_t s);
+// Mode shapes (modes.cu): inverse iteration on the Hermitian band matrix (width b, ld 2b) for the nvec eigenvalues lam
+// (nvec per matrix, ascending), Z: n x nvec per matrix (ld n), LU: band_invit_lu_elems(n, b) complex of scratch per matrix.
+size_t band_invit_lu_elems(int n, int b);
+void launch_band_invit(int n, int b, BatchRef AB, const double *lam, int nvec, BatchRef Z, BatchRef LU, int ncells, int inner,
+                       cudaStream_t s);
+// HU = V B(k) U (3N x nvec from 2N x nvec); kap: per matrix [2][N] doubles (kx, ky of k + G).
+void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, const double *kap, int nvec, int ncells,
+                    int inner, cudaStream_t s);
 // S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
 void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s,
                   bool root = false);  // root: write sqrt(max(lambda, 0)) instead of lambda

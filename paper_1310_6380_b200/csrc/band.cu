@@ -10,7 +10,15 @@
 //   small   : T from G and tau (forward recurrence of the compact WY form); M2 = -1/2 T^H S T
 //   X       : X = Z T + V M2 = [V | Z] [M2; T]   (DMMA)            =>  Q^H A22 Q = A22 - X V^H - V X^H
 //   HER2K   : A22 -= [V | X] [X | V]^H on the lower tiles           (DMMA, K = 2b)
-// Workspace per matrix (VW): n x 4b complex, columns [V | X | V | Z]; SM: b x 2b (Gram) + 2b x b ([M2; T]) + b (tau).
+// Workspace per matrix (VW): six slots of n x b complex; SM: coefficient blocks, tau and the split-K partial products.
+//
+// Band widths <= 16 take the panels in PAIRS (launch_sy2sb): the trailing matrix is read and written once per 2b columns
+// by one rank-4b update (K = 4b = 64 at b = 16: the k-loop length of the b = 32 reduction) instead of twice by rank-2b
+// updates.  Panel 2 of a pair is factored after only ITS b columns have received panel 1's update (a look-ahead of width
+// b), and its Z = A22'' V2 with the not yet updated trailing matrix A22 is corrected by small products:
+//   A22'' = A22 - V1 X1^H - X1 V1^H   =>   Z2 = A22 V2 - V1 (X1^H V2) - X1 (V1^H V2) = Z0 - V1 W1 - X1 W2,
+//   S = V2^H Z2 = S0 - W2^H W1 - W1^H W2,   X2 = Z2 T2 + V2 M2 = [V1 V2 X1 Z0] [-W1 T2; M2; -W2 T2; T2]   (one GEMM, K = 4b),
+//   A22[b:, b:] -= [V1 V2 X1 X2] [X1 X2 V1 V2]^H   (slots 0..3 times slots 2..5: V1 V2 X1 X2 V1 V2).
 #include "bs_internal.cuh"
 
 namespace bsk {
@@ -59,7 +67,7 @@ __device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double
 // their own latency chain (128 registers), 4 when the batch is large and the SM is shared (64 registers, throughput).
 template <int NTHR, int MINB = 1>
 __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, int b, int c0, BatchRef A, BatchRef VW, BatchRef SM,
-                                                        int inner) {
+                                                        int inner, int slot1, int slot2) {
   extern __shared__ __align__(16) unsigned char qr_smem[];
   const int r0 = c0 + b, m = n - r0;
   cplx *sp = reinterpret_cast<cplx *>(qr_smem);                 // [SW][m]
@@ -69,8 +77,8 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
   cplx *Tm = scal + 2;
   const int z = blockIdx.x, cell = z / inner, mi = z % inner;
   cplx *Ag = batch_ptr(A, cell, mi);
-  cplx *V1 = batch_ptr(VW, cell, mi);
-  cplx *V2 = V1 + (size_t)2 * b * n;
+  cplx *V1 = batch_ptr(VW, cell, mi) + (size_t)slot1 * b * n;  // the two copies of V: slots (n x b each) of the workspace
+  cplx *V2 = batch_ptr(VW, cell, mi) + (size_t)slot2 * b * n;
   double *tau_out = reinterpret_cast<double *>(batch_ptr(SM, cell, mi) + (size_t)4 * b * b);
   const int kq = min(b, m - 1);
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -333,6 +341,87 @@ __global__ void __launch_bounds__(1024) wy_small_kernel(int b, BatchRef SM, int 
   }
 }
 
+// Second panel of a pair (see the header): from the split-K partials of Gm = [V1 V2 X1]^H [V2 X1 Z0] (3b x 3b, ld 3b) and
+// tau of panel 2, the coefficient block Cf (4b x b, ld 4b) of  X2 = [V1 V2 X1 Z0] Cf :
+//   W2 = V1^H V2 = Gm[0:b, 0:b],  G = V2^H V2 = Gm[b:2b, 0:b],  W1 = X1^H V2 = Gm[2b:3b, 0:b],  S0 = V2^H Z0 = Gm[b:2b, 2b:3b],
+//   S = S0 - W2^H W1 - W1^H W2,  T2 as in wy_small_kernel,  M2 = -1/2 T2^H S T2,  Cf = [-W1 T2; M2; -W2 T2; T2].
+// SM per matrix: Cf at 0; tau at 4 b^2; partials at 4 b^2 + 64.
+__global__ void __launch_bounds__(1024) wy_pair_kernel(int b, BatchRef SM, int inner) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *T = reinterpret_cast<cplx *>(smem_raw);  // b x b, T[i + j*b]
+  cplx *S = T + b * b;
+  cplx *U = S + b * b;
+  cplx *G = U + b * b;
+  cplx *W1 = G + b * b;
+  cplx *W2 = W1 + b * b;
+  cplx *taus = W2 + b * b;
+  const int z = blockIdx.x, cell = z / inner, mi = z % inner;
+  cplx *sm = batch_ptr(SM, cell, mi);
+  const cplx *part = sm + (size_t)4 * b * b + 64;
+  cplx *out = sm;
+  const int t = threadIdx.x, b3 = 3 * b;
+  if (t < b) taus[t] = sm[(size_t)4 * b * b + t];
+  auto gm = [&](int r, int c) {  // fixed order over the k-splits: deterministic
+    cplx a = cmake(0.0, 0.0);
+    for (int k = 0; k < KS; ++k) a = cadd(a, part[(size_t)k * b3 * b3 + r + (size_t)c * b3]);
+    return a;
+  };
+  for (int i = t; i < b * b; i += blockDim.x) {
+    const int r = i % b, c = i / b;
+    W2[i] = gm(r, c);
+    G[i] = gm(b + r, c);
+    W1[i] = gm(2 * b + r, c);
+    S[i] = gm(b + r, 2 * b + c);
+    T[i] = cmake(0.0, 0.0);
+    U[i] = (r == c) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
+  }
+  __syncthreads();
+  for (int i = t; i < b * b; i += blockDim.x) {  // S = S0 - W2^H W1 - W1^H W2
+    const int r = i % b, c = i / b;
+    cplx a = S[i];
+    for (int l = 0; l < b; ++l) {
+      cplx p = cmake(0.0, 0.0);
+      cfmac(p, W2[l + r * b], W1[l + c * b]);
+      cfmac(p, W1[l + r * b], W2[l + c * b]);
+      a = csub(a, p);
+    }
+    S[i] = a;
+  }
+  __syncthreads();
+  for (int l = b - 1; l >= 0; --l) {  // T2: column-oriented back substitution, as in wy_small_kernel
+    const cplx tl = taus[l];
+    for (int e = t; e < b * b; e += blockDim.x) {
+      const int i = e % b, j = e / b;
+      if (j < l || i > l) continue;
+      const cplx x = cmul(tl, U[l + j * b]);
+      if (i == l) T[e] = x;
+      else { cplx r = U[e]; cfms(r, G[i + l * b], x); U[e] = r; }
+    }
+    __syncthreads();
+  }
+  for (int i = t; i < b * b; i += blockDim.x) {  // U = S T
+    const int r = i % b, c = i / b;
+    cplx acc = cmake(0.0, 0.0);
+    for (int l = 0; l <= c; ++l) cfma(acc, S[r + l * b], T[l + c * b]);
+    U[i] = acc;
+  }
+  __syncthreads();
+  for (int i = t; i < b * b; i += blockDim.x) {
+    const int r = i % b, c = i / b;
+    cplx m2 = cmake(0.0, 0.0), a1 = cmake(0.0, 0.0), a2 = cmake(0.0, 0.0);
+    for (int l = 0; l <= r; ++l) cfmac(m2, T[l + r * b], U[l + c * b]);   // (T^H U)[r, c]
+    for (int l = 0; l <= c; ++l) {                                         // (W T)[r, c], T upper triangular
+      cfma(a1, W1[r + l * b], T[l + c * b]);
+      cfma(a2, W2[r + l * b], T[l + c * b]);
+    }
+    cplx *col = out + (size_t)c * 4 * b;
+    col[r] = cmake(-a1.x, -a1.y);
+    col[b + r] = cscale(m2, -0.5);
+    col[2 * b + r] = cmake(-a2.x, -a2.y);
+    col[3 * b + r] = T[i];
+  }
+}
+
 // Band extraction: AB[d + c*ldab] = A[c+d, c] for 0 <= d <= b (zero beyond the matrix and for b < d < ldab).
 __global__ void __launch_bounds__(256) band_extract_kernel(int n, int lda, int b, int ldab, BatchRef A, BatchRef AB,
                                                            int inner) {
@@ -350,8 +439,8 @@ __global__ void __launch_bounds__(256) band_extract_kernel(int n, int lda, int b
 }
 }  // namespace
 
-size_t band_vw_elems(int n, int b) { return (size_t)4 * b * n; }
-size_t band_sm_elems(int b) { return (size_t)4 * b * b + 64 + (size_t)KS * 2 * b * b; }
+size_t band_vw_elems(int n, int b) { return (size_t)6 * b * n; }
+size_t band_sm_elems(int b) { return (size_t)4 * b * b + 64 + (size_t)KS * 9 * b * b; }
 size_t band_ab_elems(int n, int b) { return (size_t)n * 2 * b; }
 
 // Stage 1 for every matrix of the batch in lock step; on exit AB holds the band (ldab = 2b, bulge space zeroed).
@@ -359,73 +448,105 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
                  cudaStream_t s, const BatchRef *keepV, const BatchRef *keepT) {
   int launches = 0;
   const int nmat = ncells * inner;
-  static unsigned long long m1 = 0, m2 = 0, m3 = 0, m4 = 0;
+  static unsigned long long m1 = 0, m2 = 0, m3 = 0, m4 = 0, m5 = 0;
   ensure_dyn_smem(panel_qr_kernel<1024>, 140 * 1024, m1);
   ensure_dyn_smem(panel_qr_kernel<256, 2>, 48 * 1024, m2);
   ensure_dyn_smem(panel_qr_kernel<256, 4>, 48 * 1024, m3);
   ensure_dyn_smem(wy_small_kernel, (4 * 32 * 32 + 32) * (int)sizeof(cplx), m4);
-  for (int c0 = 0; c0 + b < n - 1; c0 += b) {
-    const int r0 = c0 + b, m = n - r0;  // m >= 2
-    {
-      KScope ks(KC_PANEL, 0.0, s);
-      if (m > 640) {
-        const size_t smem = (size_t)SW * m * sizeof(cplx) + (32 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
-        panel_qr_kernel<1024><<<nmat, 1024, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
-      } else {
-        const size_t smem = (size_t)SW * m * sizeof(cplx) + (8 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
-        if (nmat > 592) panel_qr_kernel<256, 4><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
-        else panel_qr_kernel<256, 2><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner);
-      }
-      ++launches;
+  ensure_dyn_smem(wy_pair_kernel, (6 * 32 * 32 + 32) * (int)sizeof(cplx), m5);
+  auto slot = [&](int k, int r0) { BatchRef r = VW; r.off += (long long)k * b * n + r0; return r; };  // rows r0.. of slot k
+  auto qr = [&](int c0, int s1, int s2) {
+    const int m = n - (c0 + b);
+    KScope ks(KC_PANEL, 0.0, s);
+    if (m > 640) {
+      const size_t smem = (size_t)SW * m * sizeof(cplx) + (32 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
+      panel_qr_kernel<1024><<<nmat, 1024, smem, s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
+    } else {
+      const size_t smem = (size_t)SW * m * sizeof(cplx) + (8 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
+      if (nmat > 592) panel_qr_kernel<256, 4><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
+      else panel_qr_kernel<256, 2><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
     }
+    ++launches;
+  };
+  auto gemm = [&](int kclass, int M, int N, int K, int opA, int opB, int flags, BatchRef Ar, int la, BatchRef Br, int lb,
+                  BatchRef Cr, int lc, double alpha, double beta, int ksplit = 0, long long sstride = 0) {
     GemmDesc g{};
-    g.ncells = ncells; g.inner = inner; g.kclass = KC_GEMM_TRIDIAG;
-    // Z = A22 V
-    g.kclass = KC_GEMM_HEMM;
-    g.M = m; g.N = b; g.K = m; g.opA = 0; g.opB = 0; g.flags = BS_GEMM_A_HERM_LOWER;
-    g.A = A; g.A.off += (long long)r0 * (lda + 1); g.lda = lda;
-    g.B = VW; g.B.off += r0; g.ldb = n;
-    g.C = VW; g.C.off += (long long)3 * b * n + r0; g.ldc = n;
-    g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
+    g.ncells = ncells; g.inner = inner; g.kclass = kclass;
+    g.M = M; g.N = N; g.K = K; g.opA = opA; g.opB = opB; g.flags = flags;
+    g.A = Ar; g.lda = la; g.B = Br; g.ldb = lb; g.C = Cr; g.ldc = lc;
+    g.alpha = cmake(alpha, 0.0); g.beta = cmake(beta, 0.0);
+    g.ksplit = ksplit; g.split_stride = sstride;
     launch_zgemm(g, s); ++launches;
-    // [G | S] = V^H [V | Z]
-    g.kclass = KC_GEMM_WY;
-    g.M = b; g.N = 2 * b; g.K = m; g.opA = 1; g.opB = 0; g.flags = 0;
-    g.A = VW; g.A.off += r0; g.lda = n;
-    g.B = VW; g.B.off += (long long)2 * b * n + r0; g.ldb = n;
-    g.C = SM; g.C.off += (long long)4 * b * b + 64; g.ldc = b;
-    g.ksplit = KS; g.split_stride = (long long)2 * b * b;
-    launch_zgemm(g, s); ++launches;
-    g.ksplit = 0; g.split_stride = 0;
+  };
+  auto keep = [&](int c0, int vslot, long long t_off, int t_ld) {  // mode shapes: V and T of this panel are needed again
+    if (!keepV) return;
+    const int r0 = c0 + b, m = n - r0;
+    BatchRef dst = *keepV;
+    dst.off += (long long)c0 * n + r0;
+    launch_copy_matrix(m, b, slot(vslot, r0), n, dst, n, ncells, inner, s); ++launches;
+    BatchRef src = SM;
+    src.off += t_off;
+    dst = *keepT; dst.off += (long long)(c0 / b) * b * b;
+    launch_copy_matrix(b, b, src, t_ld, dst, b, ncells, inner, s); ++launches;
+  };
+  auto trailing = [&](int r0) { BatchRef r = A; r.off += (long long)r0 * (lda + 1); return r; };
+  BatchRef smG = SM, smOut = SM, smCf = SM;
+  smG.off += (long long)4 * b * b + 64;  // split-K partials
+  smOut.off += (long long)2 * b * b;     // [M2; T] of a single panel (ld 2b)
+  // One panel: V -> slots (sv, sv2), Z -> slot sv2 + 1, X -> slot sx;  Gram with B = [V copy | Z], X = [V copy | Z] [M2; T]
+  auto single_front = [&](int c0, int sv, int sv2, int sx) {
+    const int r0 = c0 + b, m = n - r0;
+    qr(c0, sv, sv2);
+    gemm(KC_GEMM_HEMM, m, b, m, 0, 0, BS_GEMM_A_HERM_LOWER, trailing(r0), lda, slot(sv, r0), n, slot(sv2 + 1, r0), n, 1.0, 0.0);
+    gemm(KC_GEMM_WY, b, 2 * b, m, 1, 0, 0, slot(sv, r0), n, slot(sv2, r0), n, smG, b, 1.0, 0.0, KS, (long long)2 * b * b);
     {
       KScope ks(KC_OTHER, 0.0, s);
       // few matrices: one thread per entry (latency); many: smaller CTAs, several per SM (throughput)
       wy_small_kernel<<<nmat, nmat > 592 ? 256 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
       ++launches;
     }
-    if (keepV) {  // mode shapes: V and T of this panel are needed again for the back-transformation
-      BatchRef src = VW, dst = *keepV;
-      src.off += r0;
-      dst.off += (long long)c0 * n + r0;
-      launch_copy_matrix(m, b, src, n, dst, n, ncells, inner, s); ++launches;
-      src = SM; src.off += (long long)2 * b * b + b;   // T inside [M2; T] (ld 2b)
-      dst = *keepT; dst.off += (long long)(c0 / b) * b * b;
-      launch_copy_matrix(b, b, src, 2 * b, dst, b, ncells, inner, s); ++launches;
+    keep(c0, sv, (long long)2 * b * b + b, 2 * b);
+    gemm(KC_GEMM_WY, m, b, 2 * b, 0, 0, 0, slot(sv2, r0), n, smOut, 2 * b, slot(sx, r0), n, 1.0, 0.0);
+  };
+  int c0 = 0;
+  // Pairs pay off where the trailing updates dominate: measured S6 totals (ms, pairs / single panels) C5 (n = 1922) 235.7 /
+  // 249.8, C3 (n = 882) 32.1 / 31.5, C2 (n = 450) 8.3 / 7.8, C4 (n = 242, 10240 matrices) 155 / 141 (the extra small products).
+  // The rule depends on n only, so a batch and its members take the same path.  (The in-place X2 product needs one column
+  // tile: N = b <= 16.)
+  const bool pairs = b <= 16 && n >= 1200;
+  while (c0 + b < n - 1) {
+    const int r0 = c0 + b, m = n - r0;  // m >= 2
+    const bool second = pairs && (c0 + 2 * b < n - 1);
+    if (!second) {
+      // a single panel: slots [. V X V Z .]: A22 -= [V | X] [X | V]^H on the lower tiles
+      single_front(c0, 1, 3, 2);
+      gemm(KC_GEMM_TRIDIAG, m, m, 2 * b, 0, 1, BS_GEMM_LOWER_ONLY, slot(1, r0), n, slot(2, r0), n, trailing(r0), lda, -1.0, 1.0);
+      c0 += b;
+      continue;
     }
-    // X = [V | Z] [M2; T]
-    g.M = m; g.N = b; g.K = 2 * b; g.opA = 0; g.opB = 0; g.flags = 0;
-    g.A = VW; g.A.off += (long long)2 * b * n + r0; g.lda = n;
-    g.B = SM; g.B.off += (long long)2 * b * b; g.ldb = 2 * b;
-    g.C = VW; g.C.off += (long long)b * n + r0; g.ldc = n;
-    launch_zgemm(g, s); ++launches;
-    // A22 -= [V | X] [X | V]^H  (lower tiles)
-    g.kclass = KC_GEMM_TRIDIAG;
-    g.M = m; g.N = m; g.K = 2 * b; g.opA = 0; g.opB = 1; g.flags = BS_GEMM_LOWER_ONLY;
-    g.A = VW; g.A.off += r0; g.lda = n;
-    g.B = VW; g.B.off += (long long)b * n + r0; g.ldb = n;
-    g.C = A; g.C.off += (long long)r0 * (lda + 1); g.ldc = lda;
-    g.alpha = cmake(-1.0, 0.0); g.beta = cmake(1.0, 0.0);
-    launch_zgemm(g, s); ++launches;
+    // ---- a pair of panels: slots [V1 V2 X1 X2 V1 V2]
+    single_front(c0, 0, 4, 2);  // V1 -> 0 and 4, Z1 -> 5, X1 -> 2
+    // look-ahead: only the next panel's b columns receive panel 1's update now:  A[r0:, r0:r0+b] -= X1 V1[0:b]^H + V1 X1[0:b]^H
+    gemm(KC_GEMM_TRIDIAG, m, b, b, 0, 1, 0, slot(2, r0), n, slot(0, r0), n, trailing(r0), lda, -1.0, 1.0);
+    gemm(KC_GEMM_TRIDIAG, m, b, b, 0, 1, 0, slot(4, r0), n, slot(2, r0), n, trailing(r0), lda, -1.0, 1.0);
+    const int c1 = c0 + b, r1 = c1 + b, m2 = n - r1;
+    qr(c1, 1, 5);  // V2 -> 1 and 5
+    // Z0 = A22 V2 with the trailing matrix as it was before panel 1's update -> slot 3
+    gemm(KC_GEMM_HEMM, m2, b, m2, 0, 0, BS_GEMM_A_HERM_LOWER, trailing(r1), lda, slot(1, r1), n, slot(3, r1), n, 1.0, 0.0);
+    // Gm = [V1 V2 X1]^H [V2 X1 Z0]  (3b x 3b, split-K)
+    gemm(KC_GEMM_WY, 3 * b, 3 * b, m2, 1, 0, 0, slot(0, r1), n, slot(1, r1), n, smG, 3 * b, 1.0, 0.0, KS, (long long)9 * b * b);
+    {
+      KScope ks(KC_OTHER, 0.0, s);
+      wy_pair_kernel<<<nmat, nmat > 592 ? 256 : b * b, (6 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
+      ++launches;
+    }
+    keep(c1, 1, (long long)3 * b, 4 * b);
+    // X2 = [V1 V2 X1 Z0] Cf, written over Z0 (slot 3): a CTA of the 64 x 16 tiling owns complete rows and has read all of
+    // its A operand before its epilogue stores
+    gemm(KC_GEMM_WY, m2, b, 4 * b, 0, 0, 0, slot(0, r1), n, smCf, 4 * b, slot(3, r1), n, 1.0, 0.0);
+    // A22[b:, b:] -= [V1 V2 X1 X2] [X1 X2 V1 V2]^H on the lower tiles: ONE read-modify-write of the trailing matrix per pair
+    gemm(KC_GEMM_TRIDIAG, m2, m2, 4 * b, 0, 1, BS_GEMM_LOWER_ONLY, slot(0, r1), n, slot(2, r1), n, trailing(r1), lda, -1.0, 1.0);
+    c0 += 2 * b;
   }
   {
     KScope ks(KC_OTHER, 0.0, s);

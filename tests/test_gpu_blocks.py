@@ -171,7 +171,7 @@ def test_zpotrf_reports_not_pd(bs):
 
 @pytest.mark.parametrize("algo", [0, 1])
 @pytest.mark.parametrize("n,nb", [(1, 8), (2, 8), (5, 4), (9, 8), (64, 8), (98, 32), (242, 32), (242, 16), (450, 16), (130, 32),
-                                  (333, 8), (700, 32)])
+                                  (333, 8), (700, 32), (1210, 16), (1217, 16), (1230, 8)])   # n >= 1200, b <= 16: panels in pairs
 def test_zhetrd_eigenvalues(bs, n, nb, algo):
     import torch
     rng = np.random.default_rng(n + nb)

@@ -284,7 +284,7 @@ struct KtGuard {  // routes the launchers' KScope to the lead cell's timer for t
 // centroids, tiling check.
 struct HostGeom {
   double T[4], Q[4], V = 0.0;
-  int ne = 0;
+  int ne = 0, nes = 0;
   std::vector<double> edge, area;  // edge: SoA [6][ne]; area: [area | ch1 | ch2][P]
   std::vector<int> eph;
 };
@@ -302,9 +302,10 @@ bs_status host_geometry(const double lattice[4], int nphase, const int32_t *vert
   g.Q[0] = kTwoPi * g.T[0]; g.Q[1] = kTwoPi * g.T[2];  // q^1
   g.Q[2] = kTwoPi * g.T[1]; g.Q[3] = kTwoPi * g.T[3];  // q^2
   g.V = std::fabs(det);
-  const int ne = vert_offset[nphase];
+  const int ne = vert_offset[nphase], nes = (ne + 1) & ~1;  // (SoA stride: even, so that every array is 16-byte aligned)
   g.ne = ne;
-  g.edge.assign((size_t)6 * ne, 0.0);
+  g.nes = nes;
+  g.edge.assign((size_t)6 * nes, 0.0);
   g.area.assign((size_t)3 * nphase, 0.0);
   g.eph.assign(ne, 0);
   double total = 0.0;
@@ -319,12 +320,12 @@ bs_status host_geometry(const double lattice[4], int nphase, const int32_t *vert
       cys += (y0 + y1) * (x0 * y1 - x1 * y0);
       const double ex = x1 - x0, ey = y1 - y0, mx = 0.5 * (x0 + x1), my = 0.5 * (y0 + y1);
       // fractional coordinates H = x T  (x = H_1 h^1 + H_2 h^2)
-      g.edge[0 * (size_t)ne + i] = mx * g.T[0] + my * g.T[2];
-      g.edge[1 * (size_t)ne + i] = mx * g.T[1] + my * g.T[3];
-      g.edge[2 * (size_t)ne + i] = ex * g.T[0] + ey * g.T[2];
-      g.edge[3 * (size_t)ne + i] = ex * g.T[1] + ey * g.T[3];
-      g.edge[4 * (size_t)ne + i] = ex;
-      g.edge[5 * (size_t)ne + i] = ey;
+      g.edge[0 * (size_t)nes + i] = mx * g.T[0] + my * g.T[2];
+      g.edge[1 * (size_t)nes + i] = mx * g.T[1] + my * g.T[3];
+      g.edge[2 * (size_t)nes + i] = ex * g.T[0] + ey * g.T[2];
+      g.edge[3 * (size_t)nes + i] = ex * g.T[1] + ey * g.T[3];
+      g.edge[4 * (size_t)nes + i] = ex;
+      g.edge[5 * (size_t)nes + i] = ey;
       g.eph[i] = p;
     }
     g.area[p] = 0.5 * a2;
@@ -367,7 +368,7 @@ void init_cell_host(bs_cell *c, const double lattice[4], const HostGeom &g, int 
   c->P = nphase;
   c->nedge = g.ne;
   c->isotropic = iso;
-  c->geo.nedge = g.ne; c->geo.P = nphase;
+  c->geo.nedge = g.ne; c->geo.nes = g.nes; c->geo.P = nphase;
   std::memcpy(c->geo.Q, g.Q, sizeof(double) * 4);
 }
 
@@ -800,7 +801,9 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
     bsk::launch_shared_tables(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, sg->P, Mt, sg->d_phase, lead->d_sh,
                               lead->d_sh + wel, R(L.table), s); nl += 3;
   } else {
-    bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s); ++nl;  // S1
+    int maxP = 0;
+    for (int c = 0; c < ncells; ++c) maxP = std::max(maxP, cells[c]->P);
+    bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s, maxP); ++nl;  // S1
   }
   tick(lead, 1, s);
   bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2

@@ -52,9 +52,9 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
   } else {
     const double qx = D1 * g.Q[0] + D2 * g.Q[2];
     const double qy = D1 * g.Q[1] + D2 * g.Q[3];
-    const int ne = g.nedge;
-    const double *mh1 = g.edge, *mh2 = g.edge + ne, *eh1 = g.edge + 2 * ne, *eh2 = g.edge + 3 * ne;
-    const double *ex = g.edge + 4 * ne, *ey = g.edge + 5 * ne;
+    const int ne = g.nedge, nes = g.nes;
+    const double *mh1 = g.edge, *mh2 = g.edge + nes, *eh1 = g.edge + 2 * nes, *eh2 = g.edge + 3 * nes;
+    const double *ex = g.edge + 4 * nes, *ey = g.edge + 5 * nes;
     for (int e = threadIdx.x; e < ne; e += 256) {
       const double phi = fma((double)D1, mh1[e], (double)D2 * mh2[e]);  // q.m / (2 pi)
       const double u = fma((double)D1, eh1[e], (double)D2 * eh2[e]);    // q.e / (2 pi)  ->  q.e/2 = pi u
@@ -106,14 +106,170 @@ __global__ void __launch_bounds__(256) table_kernel(const Geometry *__restrict__
   }
 }
 
+// ---------------------------------------------------------------------------------------------- S1 with TMA staging
+// The same table, DPB index differences per CTA (one warp each), with the phase geometry and properties staged in shared
+// memory by 1-D bulk TMA copies (cp.async.bulk, completion on an mbarrier): the weights w[7][P] and the areas once, the
+// edge arrays in chunks of EC edges, double-buffered so that the copy of chunk i+1 runs under the arithmetic of chunk i.
+// (north_star: "phase geometry and properties staged in shared memory via TMA".)
+namespace {
+constexpr int DPB = 16, EC = 1024;  // at most DPB index differences (warps) per CTA; edges per staged chunk
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__host__ __device__ __forceinline__ unsigned up16(unsigned b) { return (b + 15u) & ~15u; }
+}  // namespace
+
+size_t table_tma_smem(int P) {  // w, area, two edge chunks (6 arrays + phase indices), barriers, partial sums of Delta = 0
+  return up16(7u * P * 8u) + up16(P * 8u) + 2 * (6 * EC * 8 + EC * 4) + 64;
+}
+
+__global__ void __launch_bounds__(DPB * 32) table_tma_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table) {
+  extern __shared__ __align__(128) unsigned char tsm[];
+  const int cell = blockIdx.y;
+  const Geometry g = geos[cell];
+  const int L = 4 * Mt + 1, L2 = L * L, nhalf = (L2 + 1) / 2;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int P = g.P, ne = g.nedge, nes = g.nes;
+  double *ws = reinterpret_cast<double *>(tsm);                                   // [7][P]
+  double *as = reinterpret_cast<double *>(tsm + up16(7u * P * 8u));               // [P]
+  unsigned char *ebase = tsm + up16(7u * P * 8u) + up16(P * 8u);
+  const size_t cbytes = 6 * EC * 8 + EC * 4;
+  unsigned long long *bars = reinterpret_cast<unsigned long long *>(ebase + 2 * cbytes);  // [0]: w + area, [1], [2]: chunks
+  const int nchunk = (ne + EC - 1) / EC;
+  auto issue_chunk = [&](int ch) {  // thread 0
+    const int e0 = ch * EC, cnt = min(EC, ne - e0), buf = ch & 1;
+    unsigned char *dst = ebase + buf * cbytes;
+    const unsigned bd = up16(cnt * 8u), bi = up16(cnt * 4u);
+    mbar_expect_tx(&bars[1 + buf], 6 * bd + bi);
+    for (int k = 0; k < 6; ++k) bulk_g2s(dst + k * EC * 8, g.edge + (size_t)k * nes + e0, bd, &bars[1 + buf]);
+    bulk_g2s(dst + 6 * EC * 8, g.ephase + e0, bi, &bars[1 + buf]);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_init(&bars[2], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    mbar_expect_tx(&bars[0], up16(7u * P * 8u) + up16(P * 8u));
+    bulk_g2s(ws, g.w, up16(7u * P * 8u), &bars[0]);
+    bulk_g2s(as, g.area, up16(P * 8u), &bars[0]);
+    issue_chunk(0);
+  }
+  __syncthreads();
+  const int dh = blockIdx.x * (blockDim.x >> 5) + warp;  // this warp's index difference (half plane)
+  const bool active = dh < nhalf;
+  const int flat = dh + (L2 - 1) / 2;
+  const int D1 = flat / L - 2 * Mt, D2 = flat % L - 2 * Mt;
+  const double qx = D1 * g.Q[0] + D2 * g.Q[2], qy = D1 * g.Q[1] + D2 * g.Q[3];
+  double accr[7], acci[7];
+#pragma unroll
+  for (int c = 0; c < 7; ++c) accr[c] = acci[c] = 0.0;
+  mbar_wait(&bars[0], 0);
+  if (active && D1 == 0 && D2 == 0) {
+    for (int p = lane; p < P; p += 32) {
+      const double a = as[p];
+#pragma unroll
+      for (int c = 0; c < 7; ++c) accr[c] = fma(ws[c * P + p], a, accr[c]);
+    }
+  }
+  for (int ch = 0; ch < nchunk; ++ch) {
+    const int buf = ch & 1, e0 = ch * EC, cnt = min(EC, ne - e0);
+    if (threadIdx.x == 0 && ch + 1 < nchunk) issue_chunk(ch + 1);  // (its buffer was released by the barrier that ended chunk ch - 1)
+    mbar_wait(&bars[1 + buf], (ch >> 1) & 1);
+    if (active && !(D1 == 0 && D2 == 0)) {
+      const double *eb = reinterpret_cast<const double *>(ebase + buf * cbytes);
+      const int *ep = reinterpret_cast<const int *>(ebase + buf * cbytes + 6 * EC * 8);
+      for (int e = lane; e < cnt; e += 32) {
+        const double phi = fma((double)D1, eb[e], (double)D2 * eb[EC + e]);              // q.m / (2 pi)
+        const double u = fma((double)D1, eb[2 * EC + e], (double)D2 * eb[3 * EC + e]);  // q.e / (2 pi)
+        double sn, cs;
+        sincospi(2.0 * phi, &sn, &cs);
+        const double j0 = (u == 0.0) ? 1.0 : sinpi(u) / (kPi * u);
+        const double f = (qx * eb[5 * EC + e] - qy * eb[4 * EC + e]) * j0;
+        const double tr = f * cs, ti = f * sn;
+        const int p = ep[e];
+#pragma unroll
+        for (int c = 0; c < 7; ++c) {
+          const double w = ws[c * P + p];
+          accr[c] = fma(w, tr, accr[c]);
+          acci[c] = fma(w, ti, acci[c]);
+        }
+      }
+    }
+    __syncthreads();  // every warp is done with this buffer: it may be refilled (chunk ch + 2)
+  }
+  if (!active) return;
+#pragma unroll
+  for (int c = 0; c < 7; ++c) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      accr[c] += __shfl_xor_sync(0xffffffffu, accr[c], o);
+      acci[c] += __shfl_xor_sync(0xffffffffu, acci[c], o);
+    }
+  }
+  cplx *T = batch_ptr(table, cell, 0);
+  if (lane < 7) {
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int c = 0; c < 7; ++c) {
+      sr = lane == c ? accr[c] : sr;
+      si = lane == c ? acci[c] : si;
+    }
+    const int c = lane;
+    if (D1 == 0 && D2 == 0) {
+      T[(size_t)c * L2 + flat] = cmake(sr, 0.0);
+    } else {
+      const double inv = 1.0 / (qx * qx + qy * qy);
+      const double re = si * inv, im = -sr * inv;  // (-i) (sr + i si) / |q|^2
+      T[(size_t)c * L2 + flat] = cmake(re, im);
+      T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);  // T(-D) = conj T(D): Phi, R exactly Hermitian
+    }
+  }
+}
+
 void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
-                  cudaStream_t s) {
+                  cudaStream_t s, int maxP) {
   const int L = 4 * Mt + 1;
   const int nhalf = (L * L + 1) / 2;
-  dim3 grid(nhalf, ncells);
   // algorithmic work: ~230 real flops per (index difference, edge) term: sincospi + sinpi + the 7-channel accumulation,
   // counted from the SASS of the loop body (about 95 DFMA, 25 DMUL, 15 DADD)
   KScope ks(KC_TABLE, 230.0 * total_edges * nhalf, s);
+  const size_t smem = table_tma_smem(maxP);
+  if (!centroid_rule && smem <= 200 * 1024) {  // geometry and properties staged in shared memory by bulk TMA copies
+    static unsigned long long mask = 0;
+    ensure_dyn_smem(table_tma_kernel, 200 * 1024, mask);
+    // one CTA per SM (its shared memory holds the cell's properties): as many warps per CTA as it takes to give every SM
+    // one CTA, so that a single cell with few index differences still uses the whole device
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int dpb = (int)(((long long)nhalf * ncells + sms - 1) / sms);
+    dpb = dpb < 1 ? 1 : (dpb > DPB ? DPB : dpb);
+    table_tma_kernel<<<dim3((nhalf + dpb - 1) / dpb, ncells), dpb * 32, smem, s>>>(geo_dev, Mt, table);
+    return;
+  }
+  dim3 grid(nhalf, ncells);
   table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table, centroid_rule);
 }
 
@@ -139,9 +295,9 @@ __global__ void __launch_bounds__(128) phase_table_kernel(Geometry g, const int 
     out = cmake(g.area[p] * cs, g.area[p] * sn);
   } else {
     const double qx = D1 * g.Q[0] + D2 * g.Q[2], qy = D1 * g.Q[1] + D2 * g.Q[3];
-    const int ne = g.nedge;
-    const double *mh1 = g.edge, *mh2 = g.edge + ne, *eh1 = g.edge + 2 * ne, *eh2 = g.edge + 3 * ne;
-    const double *ex = g.edge + 4 * ne, *ey = g.edge + 5 * ne;
+    const int ne = g.nedge, nes = g.nes;
+    const double *mh1 = g.edge, *mh2 = g.edge + nes, *eh1 = g.edge + 2 * nes, *eh2 = g.edge + 3 * nes;
+    const double *ex = g.edge + 4 * nes, *ey = g.edge + 5 * nes;
     double sr = 0.0, si = 0.0;
     for (int e = poff[p]; e < poff[p + 1]; ++e) {
       const double phi = fma((double)D1, mh1[e], (double)D2 * mh2[e]);  // q.m / (2 pi)

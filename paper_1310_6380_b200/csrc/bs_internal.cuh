@@ -125,17 +125,19 @@ struct KScope {                    // RAII: times one launch of class c on strea
 };
 
 struct Geometry {  // device pointers, per cell
-  const double *edge;   // SoA [6][nedge]: mh1, mh2 (fractional midpoint), eh1, eh2 (fractional edge), ex, ey (Cartesian edge)
+  const double *edge;   // SoA [6][nes]: mh1, mh2 (fractional midpoint), eh1, eh2 (fractional edge), ex, ey (Cartesian edge);
+                        // nes = nedge rounded up to even: every array starts 16-byte aligned (1-D bulk TMA copies)
   const int *ephase;    // [nedge] phase of each edge
   const double *w;      // [7][P] channel weights: Dv11 Dv22 Dv12 Dv13 Dv23 Dv33 rho
   const double *area;   // [3][P]: signed area, fractional centroid (ch1, ch2)
-  int nedge, P;
+  int nedge, nes, P;
   double Q[4];          // rows q^1, q^2 (Cartesian)
 };
 
 // S1: table[c][(D1+2Mt)*(4Mt+1) + (D2+2Mt)], c < 7.  geo: device array [ncells]; table at BatchRef (inner unused).
+// maxP: the largest phase count of the batch (shared memory of the TMA-staged kernel)
 void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
-                  cudaStream_t s);
+                  cudaStream_t s, int maxP);
 // S1 for cells that share one geometry: Iph[p + dh * P] = I_p(q_D) once per geometry (poff: device [P+1] edge offsets of
 // the phases), then every cell's table as W (7 ncells x P) times Iph on the DMMA GEMM.  W, Tst: device scratch of
 // 7 ncells x P and 7 ncells x nhalf complex, nhalf = ((4Mt+1)^2 + 1) / 2.

@@ -566,15 +566,20 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
     const int nsteps0 = (n - 1 - t0 + B - 1) / B;
     const int S = nsteps0 + 2 * (nvalid - 1);
     for (int s = 0; s < S; ++s) {
-      // window bookkeeping (uniform): keep = first column still needed at macro-step s or later; hi = end of the columns
-      // needed at macro-step s + 1
-      int keep = n, hi = whi;
-      for (int g2 = 0; g2 < nvalid; ++g2) {
-        const int ig = t0 + g2, kg = s - 2 * g2, ns = (n - 1 - ig + B - 1) / B;
-        if (kg >= ns) continue;  // this sweep is finished
-        keep = min(keep, kg <= 0 ? ig : ig + 1 + kg * B);
-        const int k1 = kg + 1;
-        if (k1 >= 0 && k1 < ns) hi = max(hi, min(n, ig + 1 + (k1 + 1) * B));
+      // window bookkeeping (uniform, closed form): keep = first column still needed at macro-step s or later, hi = end of
+      // the columns needed at macro-step s + 1.  Team g is at step s - 2g; window starts decrease with g and a later team
+      // finishes later, so keep is decided by the first team that has not started (its own column t0 + g) or else by the
+      // last team; hi is decided by team 0 alone (once it has reached the end of the band, hi = n stays).
+      int keep, hi = whi;
+      {
+        const int gu = (s + 1) >> 1, gl = nvalid - 1;
+        if (gu < nvalid) {
+          keep = t0 + gu;
+        } else {
+          const int kg = s - 2 * gl, ns = (n - 1 - (t0 + gl) + B - 1) / B;
+          keep = kg < ns ? t0 + gl + 1 + kg * B : n;
+        }
+        if (s + 1 < nsteps0) hi = max(hi, min(n, t0 + 1 + (s + 2) * B));
       }
       keep = max(keep, wlo);
       if (is_io) {

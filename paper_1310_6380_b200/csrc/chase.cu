@@ -380,7 +380,7 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
 // every thread of the team.  Named barriers: 1 + team (whole team, only at k = 0), 5 + team / 9 + team (the D / C pair
 // of a B = 32 team; G <= 4 there), 15 (I/O warps).
 template <int B, int NW>
-__device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, int i, int &k, int &J, int &L,
+__device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, int i, int &k, int &J, int &sJ, int &L,
                                           bool &finished, int role, int rw, int lane, int team, double *dg, double *eg) {
   using C = Cfg<B, NW>;
   const int par = k & 1;
@@ -405,7 +405,6 @@ __device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, i
   }
   const cplx tau = ts[C::O_TAU + par];
   const int Jn = J + L, L2 = min(B, n - Jn);
-  const int sJ = J % Wc;
   if (role == 0) {
     // the C warps (the longer chain of the step) load their tiles first: the D warps wait until those are in registers
     if (L2 > 0) named_bar(1 + team, C::TT);
@@ -416,6 +415,8 @@ __device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, i
   if (L2 <= 0) {
     finished = true;
   } else {
+    sJ += L;  // ring slot of column J, kept incrementally (L <= B < Wc)
+    sJ -= sJ >= Wc ? Wc : 0;
     J = Jn; L = L2; ++k;
   }
 }
@@ -454,14 +455,14 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_resident_kernel(int n,
   asm volatile("cp.async.wait_group 0;\n" ::: "memory");
   __syncthreads();
   const int S = n >= 2 ? start[n - 2] + 1 : 0;  // the last sweep has a single step
-  int i = 0, k = 0, J = 0, L = 0, next_i = team;
+  int i = 0, k = 0, J = 0, sJ = 0, L = 0, next_i = team;
   bool finished = true;
   for (int s = 0; s < S; ++s) {
     if (finished && next_i <= n - 2 && start[next_i] == s) {
-      i = next_i; k = 0; J = i + 1; L = 0; finished = false;
+      i = next_i; k = 0; J = i + 1; sJ = J % Wc; L = 0; finished = false;
     }
     if (!finished) {
-      team_step<B, NW>(ring, Wc, ts, n, i, k, J, L, finished, role, rw, lane, team, dg, eg);
+      team_step<B, NW>(ring, Wc, ts, n, i, k, J, sJ, L, finished, role, rw, lane, team, dg, eg);
       if (finished) next_i += G;
     }
     __syncthreads();
@@ -561,7 +562,7 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
     io_load(wlo, whi, tid, blockDim.x);
     __syncthreads();
 
-    int i = t0 + team, k = 0, J = i + 1, L = 0;
+    int i = t0 + team, k = 0, J = i + 1, sJ = J % Wc, L = 0;
     bool finished = is_io || team >= nvalid;
     const int nsteps0 = (n - 1 - t0 + B - 1) / B;
     const int S = nsteps0 + 2 * (nvalid - 1);
@@ -584,12 +585,15 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
       keep = max(keep, wlo);
       if (is_io) {
         io_evict(max(wlo, t0 + nvalid), keep, io_tid, io_nt);  // (columns < t0 + nvalid are finished sweeps: never read again)
-        __threadfence();
+        // progress is published every fourth macro-step (the fence costs ~2000 cycles of the I/O warps; followers are rare
+        // with one group of matrices per wave of CTAs and only start a little later)
+        const bool publish = (s & 3) == 3;
+        if (publish) __threadfence();
         // the columns fetched below reuse ring slots of columns written back just above, in general through another
         // thread: all slot reads (and global writes) first
         named_bar(15, io_nt);
         if (io_tid == 0) {
-          st_release(mine, keep);
+          if (publish) st_release(mine, keep);
           if (prev && hi > whi)
             while (ld_acquire(prev) < hi) __nanosleep(20);
         }
@@ -597,7 +601,7 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
         io_load(whi, hi, io_tid, io_nt);
       }
       wlo = keep; whi = hi;
-      if (!finished && s >= 2 * team) team_step<B, NW>(ring, Wc, ts, n, i, k, J, L, finished, role, rw, lane, team, dg, eg);
+      if (!finished && s >= 2 * team) team_step<B, NW>(ring, Wc, ts, n, i, k, J, sJ, L, finished, role, rw, lane, team, dg, eg);
       __syncthreads();
     }
     // the tail of the window goes back; the train is done

@@ -4,15 +4,15 @@
 // instead of four:  Re = ar br - ai bi,  Im = (ar + ai)(br + bi) - ar br - ai bi  (norm-wise backward stable; the
 // tolerance budget is in DESIGN.md section 5, zgemm).
 #include "bs_internal.cuh"
+#include <type_traits>
 
 namespace bsk {
 
 namespace {
-constexpr int BK = 8, STAGES = 4;
 // CTA tile BM x BN = 32 x 32, four warps of 16 x 16 each (three accumulator sets of 2 x 2 m8n8 tiles = 48 registers),
 // four CTAs per SM: small CTAs in different phases hide each other's prologue and read-modify-write epilogue, which
 // is what the K = 2b = 64 rank-2b updates consist of.  Row strides are padded by 2 (conflict-free fragments).
-template <int BM, int BN>
+template <int BM, int BN, int BK, int STAGES>
 constexpr size_t smem_bytes() { return (size_t)STAGES * BK * ((BM + 2) + (BN + 2)) * sizeof(cplx); }
 
 __device__ __forceinline__ void cp16(unsigned dst, const void *src, bool ok) {  // dst: shared-space address
@@ -32,11 +32,11 @@ __device__ __forceinline__ void dmma(double &d0, double &d1, double a, double b)
 
 // HERM = 1: A is an M x M Hermitian matrix of which only the LOWER triangle is valid (K == M, OPA == 0):
 //   op(A)[m][k] = A[m][k] for m > k, Re A[m][m] for m == k, conj(A[k][m]) for m < k  (the HEMM of the band reduction).
-template <int OPA, int OPB, int HERM, int BM, int BN, int NT>
-__global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
-  constexpr int NI = 2;                                         // 8-column sub-tiles per warp
-  constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / 16;  // WMN warps along m, (NT / 32) / WMN along n
-  static_assert((BM / 16) * (BN / (8 * NI)) == NT / 32, "warps of 16 x 8 NI");
+template <int OPA, int OPB, int HERM, int BM, int BN, int NT, int MI, int BK, int STAGES, int CPS>
+__global__ void __launch_bounds__(NT, CPS) zgemm_kernel(const GemmDesc g) {
+  constexpr int NI = 2;                                              // 8-column sub-tiles per warp
+  constexpr int LDA_S = BM + 2, LDB_S = BN + 2, WMN = BM / (8 * MI);  // WMN warps along m, (NT / 32) / WMN along n
+  static_assert((BM / (8 * MI)) * (BN / (8 * NI)) == NT / 32, "warps of 8 MI x 8 NI");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx(*As)[BK][LDA_S] = reinterpret_cast<cplx(*)[BK][LDA_S]>(smem_raw);
   cplx(*Bs)[BK][LDB_S] = reinterpret_cast<cplx(*)[BK][LDB_S]>(smem_raw + (size_t)STAGES * BK * LDA_S * sizeof(cplx));
@@ -159,15 +159,15 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
     for (int ni = 0; ni < NI; ++ni) {
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const int row = m0 + wm * 16 + (lane >> 2), col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
+        const int row = m0 + wm * (8 * MI) + (lane >> 2), col = n0 + wn * (8 * NI) + ni * 8 + (lane & 3) * 2 + j;
         if (row < g.M && col < g.N) asm volatile("prefetch.global.L2 [%0];\n" ::"l"(C + (size_t)row + (size_t)col * g.ldc));
       }
     }
   }
   // c1 = sum ar br, c2 = sum ai bi (stored imaginary parts), c3 = sum (ar +- ai)(br +- bi) (- where conjugated)
-  double c1[2][NI][2], c2[2][NI][2], c3[2][NI][2];
+  double c1[MI][NI][2], c2[MI][NI][2], c3[MI][NI][2];
 #pragma unroll
-  for (int i = 0; i < 2; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int j = 0; j < NI; ++j)
       c1[i][j][0] = c1[i][j][1] = c2[i][j][0] = c2[i][j][1] = c3[i][j][0] = c3[i][j][1] = 0.0;
@@ -183,9 +183,9 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
     const int st = kt % STAGES;
 #pragma unroll
     for (int kk = 0; kk < BK; kk += 4) {
-      cplx a[2], b[NI];
+      cplx a[MI], b[NI];
 #pragma unroll
-      for (int mi = 0; mi < 2; ++mi) a[mi] = As[st][kk + (lane & 3)][wm * 16 + mi * 8 + (lane >> 2)];
+      for (int mi = 0; mi < MI; ++mi) a[mi] = As[st][kk + (lane & 3)][wm * (8 * MI) + mi * 8 + (lane >> 2)];
 #pragma unroll
       for (int ni = 0; ni < NI; ++ni) b[ni] = Bs[st][kk + (lane & 3)][wn * (8 * NI) + ni * 8 + (lane >> 2)];
       if (kk == 0) {  // the fragment loads of this k-tile are in flight: now refill the stage read one k-tile ago
@@ -197,8 +197,8 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
       // sign bit with an integer operation.
       if (HERM) {
 #pragma unroll
-        for (int mi = 0; mi < 2; ++mi) {
-          const int mg = m0 + wm * 16 + mi * 8 + (lane >> 2), kg = klo + kt * BK + kk + (lane & 3);
+        for (int mi = 0; mi < MI; ++mi) {
+          const int mg = m0 + wm * (8 * MI) + mi * 8 + (lane >> 2), kg = klo + kt * BK + kk + (lane & 3);
           int hi = __double2hiint(a[mi].y), lo = __double2loint(a[mi].y);
           hi = kg > mg ? hi ^ (int)0x80000000 : hi;
           hi = kg == mg ? 0 : hi;
@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
 #pragma unroll
       for (int ni = 0; ni < NI; ++ni) bs[ni] = OPB ? b[ni].x - b[ni].y : b[ni].x + b[ni].y;
 #pragma unroll
-      for (int mi = 0; mi < 2; ++mi) {
+      for (int mi = 0; mi < MI; ++mi) {
         const double as = OPA ? a[mi].x - a[mi].y : a[mi].x + a[mi].y;
 #pragma unroll
         for (int ni = 0; ni < NI; ++ni) dmma(c1[mi][ni][0], c1[mi][ni][1], a[mi].x, b[ni].x);
@@ -229,8 +229,8 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
     // C += alpha A B: every entry receives exactly one addition per launch, sent as two fire-and-forget FP64
     // reductions that L2 performs; no read of C, no latency in the epilogue (deterministic: one addend per entry)
 #pragma unroll
-    for (int mi = 0; mi < 2; ++mi) {
-      const int row = m0 + wm * 16 + mi * 8 + (lane >> 2);
+    for (int mi = 0; mi < MI; ++mi) {
+      const int row = m0 + wm * (8 * MI) + mi * 8 + (lane >> 2);
       if (row >= g.M) continue;
 #pragma unroll
       for (int ni = 0; ni < NI; ++ni) {
@@ -249,8 +249,8 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
     return;
   }
 #pragma unroll
-  for (int mi = 0; mi < 2; ++mi) {
-    const int row = m0 + wm * 16 + mi * 8 + (lane >> 2);
+  for (int mi = 0; mi < MI; ++mi) {
+    const int row = m0 + wm * (8 * MI) + mi * 8 + (lane >> 2);
     if (row >= g.M) continue;
     // all eight C loads of this row first (independent, in flight together), then the eight stores: a load placed
     // after a store to C could not be hoisted above it
@@ -279,15 +279,211 @@ __global__ void __launch_bounds__(NT, 640 / NT) zgemm_kernel(const GemmDesc g) {
     }
   }
 }
-template <int OPA, int OPB, int HERM, int BM = 32, int BN = 32, int NT = 128>
-void launch_one(const GemmDesc &g, cudaStream_t s) {
-  constexpr size_t smem = smem_bytes<BM, BN>();
+
+// ---- the Hermitian product of the band reduction, Z = A22 V with exactly 16 columns (band width 16) ---------------
+// Same tile shape and accumulators as zgemm_kernel<0, 0, 1, 64, 16, 128>, specialised so that the long parts of the
+// k loop carry no per-element logic and the memory side moves every byte once:
+//  * k-tiles left of the CTA's diagonal block read A[m][k] down the columns, k-tiles right of it read conj(A[k][m])
+//    along the rows of the lower triangle and flip one sign bit per fragment; only the 8 k-tiles of the diagonal
+//    block take the per-element path.  Source addresses are one 64-bit base per part plus constant multiples of the
+//    column stride; rows beyond M are requested with src-size 0 (zero fill, nothing is read).
+//  * Shared-memory layout: tiles read down the columns of A are stored k-major (As[k][m], consecutive lanes write
+//    consecutive 16 bytes); tiles read along its rows, and the V tile, are stored m-major (As[m][k ^ 4 (m & 1)]) so
+//    that the lanes of a cp.async instruction, which then run along k, again write consecutive shared memory.
+//    Measured (profiles/r2_hemm16.md): with lanes along k writing the k-major layout (one row stride per lane) every
+//    sector crossed the crossbar twice (8.3 GB instead of 5.3 GB per launch) and the loads alone took 0.85 ms instead
+//    of 0.43 ms at m = 1472.
+//  * Order of the k-tiles: see block_of below (both readers of a lower-triangle block meet in L2).
+// The k order differs from the generic kernel's, so results differ from it in the last bits; they depend only on
+// (M, block row), not on the batch.
+template <int CPS, int BK, int ST>
+__global__ void __launch_bounds__(128, CPS) hemm16_kernel(const GemmDesc g) {
+  constexpr int BM = 64, BN = 16, LDA_S = BM + 2, LDB_S = BN + 2;
+  static_assert(BK == 8, "the swizzle below is for rows of 8 elements");
+  constexpr int STAGE_A = BK * LDA_S, STAGE_B = BN * BK;  // elements; a k-major A tile (BM x BK, row stride BK) fits too
+  constexpr int RA = BM * BK / 128, RB = BN * BK / 128, MSTEP = 128 / BK;  // cp.async slots per thread and k-tile
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx *As = reinterpret_cast<cplx *>(smem_raw), *Bs = As + ST * STAGE_A;
+  const int tiles_m = (g.M + BM - 1) / BM;
+  const int zz = blockIdx.x / tiles_m, m0 = (blockIdx.x % tiles_m) * BM;
+  const int cell = zz / g.inner, bi = zz % g.inner;
+  const cplx *__restrict__ A = batch_ptr(g.A, cell, bi);
+  const cplx *__restrict__ B = batch_ptr(g.B, cell, bi);
+  cplx *C = batch_ptr(g.C, cell, bi);
+  const int M = g.M, nkt = (M + BK - 1) / BK;
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5, gq = lane >> 2, tq = lane & 3;
+
+  const unsigned as_s = (unsigned)__cvta_generic_to_shared(As), bs_s = (unsigned)__cvta_generic_to_shared(Bs);
+  const long long ldab = (long long)g.lda * (long long)sizeof(cplx);  // bytes per column of A
+  // left part: element (m, k) of a k-tile, m = t % 64, k = t / 64 + 2 r
+  const int md = t & 63, kd = t >> 6;
+  const char *pD = reinterpret_cast<const char *>(A + (m0 + md)) + kd * ldab;
+  const unsigned dD = as_s + (unsigned)((kd * LDA_S + md) * sizeof(cplx)), szd = m0 + md < M ? 16u : 0u;
+  // right part: k = t % BK, m = t / BK + MSTEP r, read from A[k][m]
+  const int km = t % BK, mm = t / BK;
+  const char *pM = reinterpret_cast<const char *>(A + km) + (long long)(m0 + mm) * ldab;
+  const int swm = (mm & 1) << 2;
+  const unsigned dM = as_s + (unsigned)((mm * BK + (km ^ swm)) * sizeof(cplx));
+  unsigned szm[RA];
+#pragma unroll
+  for (int r = 0; r < RA; ++r) szm[r] = m0 + mm + MSTEP * r < M ? 16u : 0u;
+  // V: k = t % BK, n = t / BK + MSTEP r
+  const long long ldbb = (long long)g.ldb * (long long)sizeof(cplx);
+  const char *pB = reinterpret_cast<const char *>(B + km + (size_t)mm * g.ldb);
+  const unsigned dB = bs_s + (unsigned)((mm * BK + (km ^ swm)) * sizeof(cplx));
+
+  int ld_stage = 0;
+  auto load_tile = [&](int kl, int stage) {
+    const int k0 = kl * BK;
+    const unsigned so = (unsigned)(stage * STAGE_A * sizeof(cplx)), sob = (unsigned)(stage * STAGE_B * sizeof(cplx));
+    if (k0 + BK <= m0) {
+      const char *p = pD + k0 * ldab;
+#pragma unroll
+      for (int r = 0; r < RA; ++r) cp16(dD + so + (unsigned)(r * 2 * LDA_S * sizeof(cplx)), p + (2 * r) * ldab, szd);
+    } else if (k0 >= m0 + BM) {
+      const char *p = pM + (long long)k0 * (long long)sizeof(cplx);
+      const bool kok = k0 + km < M;  // false only in a ragged last k-tile
+#pragma unroll
+      for (int r = 0; r < RA; ++r)
+        cp16(dM + so + (unsigned)(r * MSTEP * BK * sizeof(cplx)), p + (MSTEP * r) * ldab, kok ? szm[r] : 0u);
+    } else {  // the diagonal block: per element
+#pragma unroll
+      for (int r = 0; r < RA; ++r) {
+        const int row = m0 + md, col = k0 + kd + 2 * r;
+        const bool ok = row < M && col < M;
+        const cplx *src = col > row ? A + (size_t)col + (size_t)row * g.lda : A + (size_t)row + (size_t)col * g.lda;
+        cp16(dD + so + (unsigned)(r * 2 * LDA_S * sizeof(cplx)), ok ? src : A, ok ? 16u : 0u);
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < RB; ++r)
+      cp16(dB + sob + (unsigned)(r * MSTEP * BK * sizeof(cplx)), pB + (long long)k0 * (long long)sizeof(cplx) + (long long)(r * MSTEP) * ldbb, k0 + km < M ? 16u : 0u);
+  };
+
+  double c1[2][2][2], c2[2][2][2], c3[2][2][2];
+#pragma unroll
+  for (int i = 0; i < 2; ++i)
+#pragma unroll
+    for (int j = 0; j < 2; ++j) c1[i][j][0] = c1[i][j][1] = c2[i][j][0] = c2[i][j][1] = c3[i][j][0] = c3[i][j][1] = 0.0;
+
+  // Order of the k-tiles: by blocks of 64 columns, block J = (r - I) mod tiles_m in round r (I = this CTA's block row).
+  // The lower-triangle block {I, J} is needed by the CTAs I and J only, and this order has both of them read it in the
+  // same round r, so the second reader finds it in L2 (the CTAs of one matrix are launched together and do the same
+  // work per round); with J = 0, 1, 2, ... the two readers are |I - J| rounds apart and both go to DRAM.
+  const int I = m0 / BM;
+  auto block_of = [&](int r) { int J = r - I; return J < 0 ? J + tiles_m : J; };
+  int ld_r = 0, ld_kt = block_of(0) * (BM / BK), ld_end = min(ld_kt + BM / BK, nkt);
+  auto load_next = [&]() {  // loads the next k-tile of the sequence into the stage of its sequence number
+    if (ld_r < tiles_m) load_tile(ld_kt, ld_stage);
+    ld_stage = ld_stage + 1 == ST ? 0 : ld_stage + 1;
+    if (++ld_kt >= ld_end) {
+      ++ld_r;
+      ld_kt = block_of(ld_r) * (BM / BK);
+      ld_end = min(ld_kt + BM / BK, nkt);
+    }
+  };
+#pragma unroll
+  for (int s = 0; s < ST - 1; ++s) {
+    load_next();
+    cp_commit();
+  }
+  const int sw = (gq & 1) << 2;
+  const cplx *fa0 = As + tq * LDA_S + warp * 16 + gq, *fat0 = As + (warp * 16 + gq) * BK + tq, *fb0 = Bs + gq * BK + tq;
+  int stage = 0;
+  // MODE 0: left of the diagonal block, 1: right of it (every element conjugated), 2: inside it
+  auto k_tile = [&](int kt, auto mode) {
+    constexpr int MODE = decltype(mode)::value;
+    cp_wait<ST - 2>();
+    __syncthreads();
+    load_next();
+    cp_commit();
+    const cplx *fa = (MODE == 1 ? fat0 : fa0) + stage * STAGE_A, *fb = fb0 + stage * STAGE_B;
+    stage = stage + 1 == ST ? 0 : stage + 1;
+#pragma unroll
+    for (int kk = 0; kk < BK; kk += 4) {
+      cplx a[2], b[2];
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) a[mi] = MODE == 1 ? fa[mi * 8 * BK + (kk ^ sw)] : fa[kk * LDA_S + mi * 8];
+#pragma unroll
+      for (int ni = 0; ni < 2; ++ni) b[ni] = fb[ni * 8 * BK + (kk ^ sw)];
+      if (MODE == 1) {
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi) a[mi].y = __hiloint2double(__double2hiint(a[mi].y) ^ (int)0x80000000, __double2loint(a[mi].y));
+      } else if (MODE == 2) {
+#pragma unroll
+        for (int mi = 0; mi < 2; ++mi) {
+          const int mg = m0 + warp * 16 + mi * 8 + gq, kg = kt * BK + kk + tq;
+          int hi = __double2hiint(a[mi].y), lo = __double2loint(a[mi].y);
+          hi = kg > mg ? hi ^ (int)0x80000000 : hi;
+          hi = kg == mg ? 0 : hi;
+          lo = kg == mg ? 0 : lo;
+          a[mi].y = __hiloint2double(hi, lo);
+        }
+      }
+      double bs[2];
+#pragma unroll
+      for (int ni = 0; ni < 2; ++ni) bs[ni] = b[ni].x + b[ni].y;
+#pragma unroll
+      for (int mi = 0; mi < 2; ++mi) {
+        const double as = a[mi].x + a[mi].y;
+#pragma unroll
+        for (int ni = 0; ni < 2; ++ni) dmma(c1[mi][ni][0], c1[mi][ni][1], a[mi].x, b[ni].x);
+#pragma unroll
+        for (int ni = 0; ni < 2; ++ni) dmma(c2[mi][ni][0], c2[mi][ni][1], a[mi].y, b[ni].y);
+#pragma unroll
+        for (int ni = 0; ni < 2; ++ni) dmma(c3[mi][ni][0], c3[mi][ni][1], as, bs[ni]);
+      }
+    }
+  };
+  for (int r = 0; r < tiles_m; ++r) {
+    const int J = block_of(r), kt0 = J * (BM / BK), kt1 = min(kt0 + BM / BK, nkt);
+    if (J < I) {
+      for (int kt = kt0; kt < kt1; ++kt) k_tile(kt, std::integral_constant<int, 0>());
+    } else if (J > I) {
+      for (int kt = kt0; kt < kt1; ++kt) k_tile(kt, std::integral_constant<int, 1>());
+    } else {
+      for (int kt = kt0; kt < kt1; ++kt) k_tile(kt, std::integral_constant<int, 2>());
+    }
+  }
+  cp_wait<0>();
+
+  const bool has_beta = (g.beta.x != 0.0 || g.beta.y != 0.0);
+#pragma unroll
+  for (int mi = 0; mi < 2; ++mi) {
+    const int row = m0 + warp * 16 + mi * 8 + gq;
+    if (row >= M) continue;
+#pragma unroll
+    for (int ni = 0; ni < 2; ++ni) {
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int col = ni * 8 + tq * 2 + j;
+        const double t1 = c1[mi][ni][j], t2 = c2[mi][ni][j];
+        cplx v = cmul(g.alpha, cmake(t1 - t2, c3[mi][ni][j] - t1 - t2));
+        cplx *dst = C + (size_t)row + (size_t)col * g.ldc;
+        if (has_beta) v = cadd(v, cmul(g.beta, *dst));
+        *dst = v;
+      }
+    }
+  }
+}
+void launch_hemm16(const GemmDesc &g, cudaStream_t s) {
+  constexpr int CPS = 4;
+  constexpr size_t smem = (size_t)4 * (8 * (64 + 2) + 16 * 8) * sizeof(cplx);
   static unsigned long long attr_mask = 0;
-  ensure_dyn_smem(zgemm_kernel<OPA, OPB, HERM, BM, BN, NT>, (int)smem, attr_mask);
+  ensure_dyn_smem(hemm16_kernel<CPS, 8, 4>, (int)smem, attr_mask);
+  const int tm = (g.M + 63) / 64;
+  hemm16_kernel<CPS, 8, 4><<<tm * g.ncells * g.inner, 128, smem, s>>>(g);
+}
+
+template <int OPA, int OPB, int HERM, int BM = 32, int BN = 32, int NT = 128, int MI = 2, int BK = 8, int STAGES = 4, int CPS = 640 / NT>
+void launch_one(const GemmDesc &g, cudaStream_t s) {
+  constexpr size_t smem = smem_bytes<BM, BN, BK, STAGES>();
+  static unsigned long long attr_mask = 0;
+  ensure_dyn_smem(zgemm_kernel<OPA, OPB, HERM, BM, BN, NT, MI, BK, STAGES, CPS>, (int)smem, attr_mask);
   const int tm = (g.M + BM - 1) / BM, zz = g.ncells * g.inner * (g.ksplit > 1 ? g.ksplit : 1);
   dim3 grid(tm * zz, (g.N + BN - 1) / BN, 1);
   if (g.flags & BS_GEMM_LOWER_ONLY) grid = dim3((BM / BN) * (tm * (tm + 1) / 2) * zz, 1, 1);  // requires M == N
-  zgemm_kernel<OPA, OPB, HERM, BM, BN, NT><<<grid, NT, smem, s>>>(g);
+  zgemm_kernel<OPA, OPB, HERM, BM, BN, NT, MI, BK, STAGES, CPS><<<grid, NT, smem, s>>>(g);
 }
 }  // namespace
 
@@ -302,6 +498,10 @@ void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   if (g.C.bases == g.A.bases && g.C.single == g.A.single && g.C.off == g.A.off && g.opA == 0 && g.opB == 1 &&
       g.N <= 64 && g.flags == 0) {
     launch_one<0, 1, 0, 16, 64>(g, s);
+    return;
+  }
+  if (g.N == 16 && g.opA == 0 && g.opB == 0 && g.flags == BS_GEMM_A_HERM_LOWER && g.ksplit <= 1) {
+    launch_hemm16(g, s);
     return;
   }
   if (g.N <= 16 && g.opA == 0 && g.opB == 0 && !(g.flags & BS_GEMM_LOWER_ONLY)) {  // band width 16: 64 x 16 tiles

@@ -249,6 +249,23 @@ size_t bs_zhetrd_scratch_elems(int32_t n, int32_t nb);
 bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, void *scratch, int32_t nb,
                     int32_t algo /* BS_TRIDIAG_* ; two-stage: nb is the band width, rounded to 8/16/32 */,
                     int32_t batch, void *stream);
+/* bs_zhetrd without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture, serving
+ * loops, harnesses that forbid it): the same two-stage reduction (band width 16; n <= 112: the shared-memory kernel),
+ * Q^H A Q = T (the eigenvalues of the pencil), with ALL of its scratch (reflector blocks, band
+ * storage, progress words of the bulge chase) in one file-scope static device array of BS_ZHETRD_STATIC_BYTES that
+ * every GPU which loads the library holds until the process exits.  The call issues no cudaMalloc / cudaFree and calls
+ * no allocating library routine; it does not synchronise: d and e are valid once `stream` has reached the end of the
+ * work enqueued here.  A, d, e: DEVICE, as for bs_zhetrd (A: batch matrices, strideA elements apart, lower triangle
+ * read, overwritten; d, e: batch x n doubles).  The device of `stream` must be the current device.
+ * Limit: bs_zhetrd_static_bytes(n, batch) <= BS_ZHETRD_STATIC_BYTES (one matrix up to n = 2048, six of n = 450, ten of
+ * n = 242), otherwise BS_ERR_ARG with the two numbers in bs_last_error(); n > 2048 is BS_ERR_ARG as for bs_zhetrd.
+ * ALL calls on a device share the array, whatever the stream or host thread: calls whose GPU work overlaps race on it
+ * (order them on one stream, or with events).  The array keeps the previous call's contents; the call clears what
+ * must start at zero (the progress words) on `stream` itself. */
+#define BS_ZHETRD_STATIC_BYTES (8 * 1024 * 1024)
+size_t bs_zhetrd_static_bytes(int32_t n, int32_t batch);
+bs_status bs_zhetrd_static(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, int32_t batch,
+                           void *stream);
 /* Lowest nev eigenvalues of `batch` real symmetric tridiagonal matrices (d, e: DEVICE, batch x n) by Sturm bisection;
  * lam: DEVICE, batch x nev, ascending. */
 bs_status bs_sturm(int32_t n, const double *d, const double *e, int32_t nev, double *lam, int32_t batch, void *stream);

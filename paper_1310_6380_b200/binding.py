@@ -36,6 +36,7 @@ SYMBOLS = [
     "bs_bands", "bs_bands_batch", "bs_modes", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
     "bs_last_error",
     "bs_fp64_peak", "bs_zgemm", "bs_zpotrf_trtri", "bs_zhetrd_scratch_elems", "bs_zhetrd", "bs_sturm",
+    "bs_zhetrd_static_bytes", "bs_zhetrd_static",
 ]
 
 
@@ -90,8 +91,11 @@ lib.bs_zgemm.argtypes = [C.c_int32] * 5 + [_dp, _vp, C.c_int32, C.c_int64, _vp, 
 lib.bs_zpotrf_trtri.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, _vp, C.c_int32, _vp]
 lib.bs_zhetrd.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, C.c_int32, C.c_int32, _vp]
 lib.bs_sturm.argtypes = [C.c_int32, _vp, _vp, C.c_int32, _vp, C.c_int32, _vp]
+lib.bs_zhetrd_static_bytes.restype = C.c_size_t
+lib.bs_zhetrd_static_bytes.argtypes = [C.c_int32, C.c_int32]
+lib.bs_zhetrd_static.argtypes = [C.c_int32, _vp, C.c_int32, C.c_int64, _vp, _vp, C.c_int32, _vp]
 for _name in SYMBOLS:
-    if _name not in ("bs_last_error", "bs_launch_count", "bs_zhetrd_scratch_elems", "bs_destroy_cell"):
+    if _name not in ("bs_last_error", "bs_launch_count", "bs_zhetrd_scratch_elems", "bs_zhetrd_static_bytes", "bs_destroy_cell"):
         getattr(lib, _name).restype = C.c_int
 
 
@@ -375,6 +379,19 @@ def bs_zhetrd_scratch_elems(n: int, nb: int) -> int:
 def bs_zhetrd(n, A, lda, strideA, d, e, scratch, nb=32, algo=BS_TRIDIAG_TWO_STAGE, batch=1, stream=None):
     _check(lib.bs_zhetrd(n, C.c_void_p(A.data_ptr()), lda, strideA, C.c_void_p(d.data_ptr()), C.c_void_p(e.data_ptr()),
                          C.c_void_p(scratch.data_ptr()), nb, algo, batch, _stream(stream)))
+
+
+BS_ZHETRD_STATIC_BYTES = 8 * 1024 * 1024
+
+
+def bs_zhetrd_static_bytes(n: int, batch: int = 1) -> int:
+    return int(lib.bs_zhetrd_static_bytes(n, batch))
+
+
+def bs_zhetrd_static(n, A, lda, strideA, d, e, batch=1, stream=None):
+    """bs_zhetrd with its scratch in the library's static device array: no allocation, no synchronisation (bs.h)."""
+    _check(lib.bs_zhetrd_static(n, C.c_void_p(A.data_ptr()), lda, strideA, C.c_void_p(d.data_ptr()),
+                                C.c_void_p(e.data_ptr()), batch, _stream(stream)))
 
 
 def bs_sturm(n, d, e, nev, lam, batch=1, stream=None):

@@ -1277,6 +1277,69 @@ bs_status bs_zhetrd(int32_t n, void *A, int32_t lda, int64_t strideA, double *d,
   return BS_OK;
 }
 
+// ---- bs_zhetrd_static: the two-stage tridiagonalisation with its scratch in a static device array ----------------
+// For callers that cannot call cudaMalloc (CUDA graph capture, serving loops, harnesses that forbid it).  The array is
+// part of the library image: every GPU that loads libbs.so holds BS_ZHETRD_STATIC_BYTES of it until the process exits.
+// In host code the NAME of the array is a host-side stand-in, not a device address; the address on the current device
+// comes from cudaGetSymbolAddress (once per device, with that device current) and only that pointer goes to kernels.
+static __device__ __align__(256) unsigned char g_zhetrd_static[BS_ZHETRD_STATIC_BYTES];
+
+static bs_status zhetrd_static_base(unsigned char **base) {
+  static unsigned char *cache[64] = {nullptr};
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(BS_ERR_ARG, "bs_zhetrd_static: device index beyond 63");
+  if (!cache[dev]) {
+    unsigned char *ptr = nullptr;
+    CU(cudaGetSymbolAddress((void **)&ptr, g_zhetrd_static));  // address on the CURRENT device
+    if (!ptr) return fail(BS_ERR_CUDA, "bs_zhetrd_static: cudaGetSymbolAddress returned a null pointer");
+    cache[dev] = ptr;
+  }
+  *base = cache[dev];
+  return BS_OK;
+}
+
+size_t bs_zhetrd_static_bytes(int32_t n, int32_t batch) {
+  if (n < 1 || batch < 1) return 0;
+  const size_t per = bs_zhetrd_scratch_elems(n, 16) * sizeof(cplx);
+  const size_t sync = (sizeof(int) * bsk::sb2st_sync_ints(n, batch) + 255) / 256 * 256;
+  return per * (size_t)batch + sync;
+}
+
+bs_status bs_zhetrd_static(int32_t n, void *A, int32_t lda, int64_t strideA, double *d, double *e, int32_t batch,
+                           void *stream) {
+  if (!A || !d || !e || n < 1 || n > 2048 || batch < 1 || lda < n) return fail(BS_ERR_ARG, "bs_zhetrd_static: bad argument");
+  const size_t need = bs_zhetrd_static_bytes(n, batch);
+  if (need > (size_t)BS_ZHETRD_STATIC_BYTES)
+    return fail(BS_ERR_ARG, "bs_zhetrd_static: n = %d, batch = %d needs %zu bytes of scratch, the static array holds %d",
+                (int)n, (int)batch, need, (int)BS_ZHETRD_STATIC_BYTES);
+  cudaStream_t s = (cudaStream_t)stream;
+  if (n <= bsk::tridiag_small_max_n()) {  // the matrix fits in shared memory: no scratch at all
+    bsk::launch_tridiag_small(n, lda, raw(A, strideA), d, e, 1, batch, s);
+    CU(cudaGetLastError());
+    return BS_OK;
+  }
+  unsigned char *base = nullptr;
+  const bs_status st = zhetrd_static_base(&base);
+  if (st != BS_OK) return st;
+  // layout: [progress words of the chase, padded to 256 B][per-matrix slots as in bs_zhetrd, band width 16]
+  const int bw = 16;
+  const size_t sync_bytes = (sizeof(int) * bsk::sb2st_sync_ints(n, batch) + 255) / 256 * 256;
+  int *sync = reinterpret_cast<int *>(base);
+  cplx *sc = reinterpret_cast<cplx *>(base + sync_bytes);
+  const long long vw = (long long)std::max(bsk::tridiag_vw_elems(n, bw), bsk::band_vw_elems(n, bw));
+  const long long pp = (long long)bsk::tridiag_p_elems(n);
+  const long long smn = align16((long long)bsk::band_sm_elems(bw));
+  const long long per = (long long)bs_zhetrd_scratch_elems(n, bw);
+  BatchRef VW = raw(sc, per), SMr = raw(sc + vw + pp, per), ABr = raw(sc + vw + pp + smn, per);
+  // what must start at zero: the progress words (launch_sb2st clears them on the stream) and nothing else: stage 1
+  // writes every element of VW / SM / AB that a later kernel of this call reads
+  bsk::launch_sy2sb(n, lda, bw, raw(A, strideA), VW, SMr, ABr, 1, batch, s);
+  bsk::launch_sb2st(n, bw, ABr, d, e, 1, batch, s, false, 0, sync);
+  CU(cudaGetLastError());
+  return BS_OK;
+}
+
 bs_status bs_sturm(int32_t n, const double *d, const double *e, int32_t nev, double *lam, int32_t batch, void *stream) {
   if (!d || !e || !lam || n < 1 || nev < 1 || nev > n || batch < 1) return fail(BS_ERR_ARG, "bs_sturm: bad argument");
   bsk::launch_sturm(n, d, e, nev, lam, batch, (cudaStream_t)stream);

@@ -801,9 +801,14 @@ bs_status bs_assemble_batch(bs_cell *const *cells, int32_t ncells, int32_t Mt, v
     bsk::launch_shared_tables(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, sg->P, Mt, sg->d_phase, lead->d_sh,
                               lead->d_sh + wel, R(L.table), s); nl += 3;
   } else {
-    int maxP = 0;
-    for (int c = 0; c < ncells; ++c) maxP = std::max(maxP, cells[c]->P);
-    bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s, maxP); ++nl;  // S1
+    int maxP = 0, max_nes = 0;
+    for (int c = 0; c < ncells; ++c) {
+      maxP = std::max(maxP, cells[c]->P);
+      max_nes = std::max(max_nes, cells[c]->geo.nes);
+    }
+    // S1; scratch for the separable-phase table: the regions Lf, X, tmp of the workspace (contiguous, first written by S3)
+    nl += bsk::launch_table(ncells > 1 ? lead->d_geos : lead->d_geo, ncells, Mt, R(L.table), total_edges, lead->quad, s, maxP,
+                            max_nes, R(L.Lf), L.dinv - L.Lf);
   }
   tick(lead, 1, s);
   bsk::launch_expand(ncells, Mt, R(L.table), R(L.Phi), R(L.R), s); ++nl;                      // S2

@@ -248,29 +248,221 @@ __global__ void __launch_bounds__(DPB * 32) table_tma_kernel(const Geometry *__r
   }
 }
 
-void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
-                  cudaStream_t s, int maxP) {
+
+// ---------------------------------------------------------------------------------------------- S1 with separable phases
+// The index differences form a lattice, q_D = D1 q^1 + D2 q^2, so the two transcendental factors of an edge term split
+// into factors that depend on (edge, D1) and (edge, D2) only:
+//   exp(i q.m)  = exp(2 pi i D1 mh1) exp(2 pi i D2 mh2),      sin(q.e / 2) = Im[ exp(pi i D1 eh1) exp(pi i D2 eh2) ].
+// edge_phasor_kernel evaluates the four families once per (edge, d), d = -2Mt .. 2Mt (4 L nedge sincospi instead of
+// L^2 nedge sincospi + sinpi), into a table that stays in L2; table_sep_kernel forms every term with two complex
+// products.  Accuracy: a product of two correctly rounded unit phasors has an ABSOLUTE error of ~2e-16, which is what the
+// phase factor needs; sin(q.e/2) is divided by q.e/2, so for |q.e / 2 pi| < 2^-10 (q almost perpendicular to the edge,
+// including the cases where rounding leaves 1e-17 in place of an exact zero) the kernel calls sinpi directly: the
+// relative error of j0 stays below 1e-13 everywhere.  A CTA takes a TA x TB tile of (D1, D2), one warp per index
+// difference: its (TA + TB) rows of each family are shared by the warps through L1.  Weights, areas and the edge
+// arrays are staged in shared memory by bulk TMA copies as in table_tma_kernel.
+__global__ void __launch_bounds__(128) edge_phasor_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef scratch) {
+  const int cell = blockIdx.z;
+  const Geometry g = geos[cell];
+  const int L = 4 * Mt + 1, nes = g.nes;
+  const int e = blockIdx.x * blockDim.x + threadIdx.x, di = blockIdx.y;
+  if (e >= g.nedge) return;
+  const double d = (double)(di - 2 * Mt);
+  cplx *tab = batch_ptr(scratch, cell, 0);
+  const size_t fam = (size_t)L * nes, at = (size_t)di * nes + e;
+  double sn, cs;
+  sincospi(2.0 * (d * g.edge[e]), &sn, &cs);
+  tab[at] = cmake(cs, sn);
+  sincospi(2.0 * (d * g.edge[nes + e]), &sn, &cs);
+  tab[fam + at] = cmake(cs, sn);
+  sincospi(d * g.edge[2 * (size_t)nes + e], &sn, &cs);
+  tab[2 * fam + at] = cmake(cs, sn);
+  sincospi(d * g.edge[3 * (size_t)nes + e], &sn, &cs);
+  tab[3 * fam + at] = cmake(cs, sn);
+}
+
+size_t table_sep_smem(int P) {  // w, area, two edge chunks (eh1, eh2, ex, ey + phase indices), barriers
+  return up16(7u * P * 8u) + up16(P * 8u) + 2 * (4 * EC * 8 + EC * 4) + 64;
+}
+
+__global__ void __launch_bounds__(DPB * 32) table_sep_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table,
+                                                             BatchRef scratch, int TA, int TB) {
+  extern __shared__ __align__(128) unsigned char tsm[];
+  const int cell = blockIdx.y;
+  const Geometry g = geos[cell];
+  const int L = 4 * Mt + 1, L2 = L * L;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int P = g.P, ne = g.nedge, nes = g.nes;
+  double *ws = reinterpret_cast<double *>(tsm);                                   // [7][P]
+  double *as = reinterpret_cast<double *>(tsm + up16(7u * P * 8u));               // [P]
+  unsigned char *ebase = tsm + up16(7u * P * 8u) + up16(P * 8u);
+  const size_t cbytes = 4 * EC * 8 + EC * 4;
+  unsigned long long *bars = reinterpret_cast<unsigned long long *>(ebase + 2 * cbytes);  // [0]: w + area, [1], [2]: chunks
+  const int nchunk = (ne + EC - 1) / EC;
+  auto issue_chunk = [&](int ch) {  // thread 0
+    const int e0 = ch * EC, cnt = min(EC, ne - e0), buf = ch & 1;
+    unsigned char *dst = ebase + buf * cbytes;
+    const unsigned bd = up16(cnt * 8u), bi = up16(cnt * 4u);
+    mbar_expect_tx(&bars[1 + buf], 4 * bd + bi);
+    for (int k = 0; k < 4; ++k) bulk_g2s(dst + k * EC * 8, g.edge + (size_t)(k + 2) * nes + e0, bd, &bars[1 + buf]);
+    bulk_g2s(dst + 4 * EC * 8, g.ephase + e0, bi, &bars[1 + buf]);
+  };
+  if (threadIdx.x == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_init(&bars[2], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    mbar_expect_tx(&bars[0], up16(7u * P * 8u) + up16(P * 8u));
+    bulk_g2s(ws, g.w, up16(7u * P * 8u), &bars[0]);
+    bulk_g2s(as, g.area, up16(P * 8u), &bars[0]);
+    issue_chunk(0);
+  }
+  __syncthreads();
+  // tile of (D1, D2): D1 in [0, 2Mt], D2 in [-2Mt, 2Mt]; the half plane is D1 > 0, or D1 == 0 and D2 >= 0
+  const int tb_count = (L + TB - 1) / TB;
+  const int D1 = (blockIdx.x / tb_count) * TA + warp / TB, D2 = (blockIdx.x % tb_count) * TB + warp % TB - 2 * Mt;
+  const bool active = D1 <= 2 * Mt && D2 <= 2 * Mt && (D1 > 0 || D2 >= 0);
+  const bool origin = D1 == 0 && D2 == 0;
+  const int flat = (D1 + 2 * Mt) * L + D2 + 2 * Mt;
+  const double qx = D1 * g.Q[0] + D2 * g.Q[2], qy = D1 * g.Q[1] + D2 * g.Q[3];
+  const cplx *tab = batch_ptr(scratch, cell, 0);
+  const size_t fam = (size_t)L * nes;
+  const double2 *r1 = reinterpret_cast<const double2 *>(tab) + (size_t)(active ? D1 + 2 * Mt : 0) * nes;
+  const double2 *r2 = reinterpret_cast<const double2 *>(tab) + fam + (size_t)(active ? D2 + 2 * Mt : 0) * nes;
+  const double2 *r3 = r1 + 2 * fam, *r4 = r2 + 2 * fam;
+  double accr[7], acci[7];
+#pragma unroll
+  for (int c = 0; c < 7; ++c) accr[c] = acci[c] = 0.0;
+  mbar_wait(&bars[0], 0);
+  if (active && origin) {
+    for (int p = lane; p < P; p += 32) {
+      const double a = as[p];
+#pragma unroll
+      for (int c = 0; c < 7; ++c) accr[c] = fma(ws[c * P + p], a, accr[c]);
+    }
+  }
+  for (int ch = 0; ch < nchunk; ++ch) {
+    const int buf = ch & 1, e0 = ch * EC, cnt = min(EC, ne - e0);
+    if (threadIdx.x == 0 && ch + 1 < nchunk) issue_chunk(ch + 1);  // (its buffer was released by the barrier that ended chunk ch - 1)
+    mbar_wait(&bars[1 + buf], (ch >> 1) & 1);
+    if (active && !origin) {
+      const double *eb = reinterpret_cast<const double *>(ebase + buf * cbytes);
+      const int *ep = reinterpret_cast<const int *>(ebase + buf * cbytes + 4 * EC * 8);
+      // four edges per lane and pass: all sixteen table loads are issued before the first is used (the direct-sinpi
+      // branch below would otherwise keep the compiler from hoisting the loads of the next edge above it)
+      for (int eb0 = lane; eb0 < cnt; eb0 += 128) {
+        double2 p1[4], p2[4], h1[4], h2[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const int e = min(eb0 + 32 * k, cnt - 1);
+          p1[k] = __ldg(r1 + e0 + e);  // (cos, sin)(2 pi D1 mh1)
+          p2[k] = __ldg(r2 + e0 + e);  // (cos, sin)(2 pi D2 mh2)
+          h1[k] = __ldg(r3 + e0 + e);  // (cos, sin)(pi D1 eh1)
+          h2[k] = __ldg(r4 + e0 + e);  // (cos, sin)(pi D2 eh2)
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const int e = eb0 + 32 * k;
+          if (e >= cnt) break;
+          const double u = fma((double)D1, eb[e], (double)D2 * eb[EC + e]);  // q.e / (2 pi)  ->  q.e/2 = pi u
+          const double cs = fma(p1[k].x, p2[k].x, -p1[k].y * p2[k].y), sn = fma(p1[k].y, p2[k].x, p1[k].x * p2[k].y);
+          double sp = fma(h1[k].y, h2[k].x, h1[k].x * h2[k].y);  // sin(pi u)
+          if (fabs(u) < 0x1p-10) sp = sinpi(u);
+          // 1 / (pi u) by the hardware's reciprocal estimate and two Newton steps (error ~1 ulp; an IEEE division
+          // with its special-case path is three times as many instructions); u == 0 yields inf/NaN, replaced below
+          const double y = kPi * u;
+          double r;
+          asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+          r = fma(r, fma(-y, r, 1.0), r);
+          r = fma(r, fma(-y, r, 1.0), r);
+          const double j0 = (u == 0.0) ? 1.0 : sp * r;
+          const double f = (qx * eb[3 * EC + e] - qy * eb[2 * EC + e]) * j0;
+          const double tr = f * cs, ti = f * sn;
+          const int p = ep[e];
+#pragma unroll
+          for (int c = 0; c < 7; ++c) {
+            const double w = ws[c * P + p];
+            accr[c] = fma(w, tr, accr[c]);
+            acci[c] = fma(w, ti, acci[c]);
+          }
+        }
+      }
+    }
+    __syncthreads();  // every warp is done with this buffer: it may be refilled (chunk ch + 2)
+  }
+  if (!active) return;
+#pragma unroll
+  for (int c = 0; c < 7; ++c) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      accr[c] += __shfl_xor_sync(0xffffffffu, accr[c], o);
+      acci[c] += __shfl_xor_sync(0xffffffffu, acci[c], o);
+    }
+  }
+  cplx *T = batch_ptr(table, cell, 0);
+  if (lane < 7) {
+    double sr = 0.0, si = 0.0;
+#pragma unroll
+    for (int c = 0; c < 7; ++c) {
+      sr = lane == c ? accr[c] : sr;
+      si = lane == c ? acci[c] : si;
+    }
+    const int c = lane;
+    if (origin) {
+      T[(size_t)c * L2 + flat] = cmake(sr, 0.0);
+    } else {
+      const double inv = 1.0 / (qx * qx + qy * qy);
+      const double re = si * inv, im = -sr * inv;  // (-i) (sr + i si) / |q|^2
+      T[(size_t)c * L2 + flat] = cmake(re, im);
+      T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);  // T(-D) = conj T(D): Phi, R exactly Hermitian
+    }
+  }
+}
+
+int launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
+                  cudaStream_t s, int maxP, int max_nes, BatchRef scratch, long long scratch_elems) {
   const int L = 4 * Mt + 1;
   const int nhalf = (L * L + 1) / 2;
-  // algorithmic work: ~230 real flops per (index difference, edge) term: sincospi + sinpi + the 7-channel accumulation,
-  // counted from the SASS of the loop body (about 95 DFMA, 25 DMUL, 15 DADD)
+  // algorithmic work: ~230 real flops per (index difference, edge) term when the formula is evaluated directly:
+  // sincospi + sinpi + the 7-channel accumulation, counted from the SASS of table_tma_kernel's loop body (about 95 DFMA,
+  // 25 DMUL, 15 DADD)
   KScope ks(KC_TABLE, 230.0 * total_edges * nhalf, s);
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (!centroid_rule && table_sep_smem(maxP) <= 200 * 1024 && (long long)4 * L * max_nes <= scratch_elems) {
+    static unsigned long long mask = 0;
+    ensure_dyn_smem(table_sep_kernel, 200 * 1024, mask);
+    edge_phasor_kernel<<<dim3((max_nes + 127) / 128, L, ncells), 128, 0, s>>>(geo_dev, Mt, scratch);
+    // tile TA x TB of (D1, D2) per CTA (one CTA per SM): the shortest sequence of waves, then the most reuse of rows
+    const int n1 = 2 * Mt + 1;
+    int TA = 1, TB = 1;
+    long long best = -1;
+    for (int a = 1; a <= 4; ++a)
+      for (int b = 1; a * b <= DPB; ++b) {
+        const long long tiles = (long long)((n1 + a - 1) / a) * ((L + b - 1) / b) * ncells;
+        // a CTA's time: its warps share the FP64 pipe, but below ~8 warps the loop is bound by its own latency
+        const long long cost = ((tiles + sms - 1) / sms) * (a * b > 8 ? a * b : 8) * 1000 + (100 * (a + b)) / (a * b);
+        if (best < 0 || cost < best) { best = cost; TA = a; TB = b; }
+      }
+    table_sep_kernel<<<dim3(((n1 + TA - 1) / TA) * ((L + TB - 1) / TB), ncells), TA * TB * 32, table_sep_smem(maxP), s>>>(
+        geo_dev, Mt, table, scratch, TA, TB);
+    return 2;
+  }
   const size_t smem = table_tma_smem(maxP);
   if (!centroid_rule && smem <= 200 * 1024) {  // geometry and properties staged in shared memory by bulk TMA copies
     static unsigned long long mask = 0;
     ensure_dyn_smem(table_tma_kernel, 200 * 1024, mask);
     // one CTA per SM (its shared memory holds the cell's properties): as many warps per CTA as it takes to give every SM
     // one CTA, so that a single cell with few index differences still uses the whole device
-    int dev = 0, sms = 148;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     int dpb = (int)(((long long)nhalf * ncells + sms - 1) / sms);
     dpb = dpb < 1 ? 1 : (dpb > DPB ? DPB : dpb);
     table_tma_kernel<<<dim3((nhalf + dpb - 1) / dpb, ncells), dpb * 32, smem, s>>>(geo_dev, Mt, table);
-    return;
+    return 1;
   }
   dim3 grid(nhalf, ncells);
   table_kernel<<<grid, 256, 0, s>>>(geo_dev, Mt, table, centroid_rule);
+  return 1;
 }
 
 // ---------------------------------------------------------------------------------------------- shared geometry (NEXT-3)

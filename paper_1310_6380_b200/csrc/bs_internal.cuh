@@ -136,8 +136,10 @@ struct Geometry {  // device pointers, per cell
 
 // S1: table[c][(D1+2Mt)*(4Mt+1) + (D2+2Mt)], c < 7.  geo: device array [ncells]; table at BatchRef (inner unused).
 // maxP: the largest phase count of the batch (shared memory of the TMA-staged kernel)
-void launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
-                  cudaStream_t s, int maxP);
+// scratch: per cell, scratch_elems complex elements that nothing else uses during S1 (the separable-phase table of
+// 4 (4Mt+1) max_nes elements goes there when it fits; otherwise the direct kernels run)
+int launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, double total_edges, int centroid_rule,
+                  cudaStream_t s, int maxP, int max_nes, BatchRef scratch, long long scratch_elems);
 // S1 for cells that share one geometry: Iph[p + dh * P] = I_p(q_D) once per geometry (poff: device [P+1] edge offsets of
 // the phases), then every cell's table as W (7 ncells x P) times Iph on the DMMA GEMM.  W, Tst: device scratch of
 // 7 ncells x P and 7 ncells x nhalf complex, nhalf = ((4Mt+1)^2 + 1) / 2.

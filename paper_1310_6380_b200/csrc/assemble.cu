@@ -281,10 +281,13 @@ __global__ void __launch_bounds__(128) edge_phasor_kernel(const Geometry *__rest
   tab[3 * fam + at] = cmake(cs, sn);
 }
 
-size_t table_sep_smem(int P) {  // w, area, two edge chunks (eh1, eh2, ex, ey + phase indices), barriers
-  return up16(7u * P * 8u) + up16(P * 8u) + 2 * (4 * EC * 8 + EC * 4) + 64;
+size_t table_sep_smem(int P) {  // w, area, two edge chunks (eh1, eh2, ex, ey + phase indices), barriers, partial sums
+  return up16(7u * P * 8u) + up16(P * 8u) + 2 * (4 * EC * 8 + EC * 4) + 64 + DPB * 28 * 8;
 }
 
+// One PAIR of index differences (D1, +D2), (D1, -D2), D1, D2 >= 0, per two warps (each takes every other group of 32
+// edges): the members share the four table loads, the edge data, the seven weights and the four real products of
+// each phasor pair (cos/sin of a sum and of a difference), which halves the memory instructions per term.
 __global__ void __launch_bounds__(DPB * 32) table_sep_kernel(const Geometry *__restrict__ geos, int Mt, BatchRef table,
                                                              BatchRef scratch, int TA, int TB) {
   extern __shared__ __align__(128) unsigned char tsm[];
@@ -298,6 +301,7 @@ __global__ void __launch_bounds__(DPB * 32) table_sep_kernel(const Geometry *__r
   unsigned char *ebase = tsm + up16(7u * P * 8u) + up16(P * 8u);
   const size_t cbytes = 4 * EC * 8 + EC * 4;
   unsigned long long *bars = reinterpret_cast<unsigned long long *>(ebase + 2 * cbytes);  // [0]: w + area, [1], [2]: chunks
+  double *part = reinterpret_cast<double *>(ebase + 2 * cbytes + 64);                      // [warps][28]
   const int nchunk = (ne + EC - 1) / EC;
   auto issue_chunk = [&](int ch) {  // thread 0
     const int e0 = ch * EC, cnt = min(EC, ne - e0), buf = ch & 1;
@@ -318,29 +322,41 @@ __global__ void __launch_bounds__(DPB * 32) table_sep_kernel(const Geometry *__r
     issue_chunk(0);
   }
   __syncthreads();
-  // tile of (D1, D2): D1 in [0, 2Mt], D2 in [-2Mt, 2Mt]; the half plane is D1 > 0, or D1 == 0 and D2 >= 0
-  const int tb_count = (L + TB - 1) / TB;
-  const int D1 = (blockIdx.x / tb_count) * TA + warp / TB, D2 = (blockIdx.x % tb_count) * TB + warp % TB - 2 * Mt;
-  const bool active = D1 <= 2 * Mt && D2 <= 2 * Mt && (D1 > 0 || D2 >= 0);
+  // tile of pairs: D1 in [0, 2Mt], D2 in [0, 2Mt]
+  const int n1 = 2 * Mt + 1, tb_count = (n1 + TB - 1) / TB;
+  const int pw = warp >> 1, half = warp & 1;
+  const int D1 = (blockIdx.x / tb_count) * TA + pw / TB, D2 = (blockIdx.x % tb_count) * TB + pw % TB;
+  const bool active = D1 <= 2 * Mt && D2 <= 2 * Mt;
   const bool origin = D1 == 0 && D2 == 0;
-  const int flat = (D1 + 2 * Mt) * L + D2 + 2 * Mt;
-  const double qx = D1 * g.Q[0] + D2 * g.Q[2], qy = D1 * g.Q[1] + D2 * g.Q[3];
+  const bool minus = D1 > 0 && D2 > 0;  // (D1, -D2) is a member of the half plane of its own (else: the conjugate / the same)
+  const double qxp = D1 * g.Q[0] + D2 * g.Q[2], qyp = D1 * g.Q[1] + D2 * g.Q[3];
+  const double qxm = D1 * g.Q[0] - D2 * g.Q[2], qym = D1 * g.Q[1] - D2 * g.Q[3];
   const cplx *tab = batch_ptr(scratch, cell, 0);
   const size_t fam = (size_t)L * nes;
   const double2 *r1 = reinterpret_cast<const double2 *>(tab) + (size_t)(active ? D1 + 2 * Mt : 0) * nes;
   const double2 *r2 = reinterpret_cast<const double2 *>(tab) + fam + (size_t)(active ? D2 + 2 * Mt : 0) * nes;
   const double2 *r3 = r1 + 2 * fam, *r4 = r2 + 2 * fam;
-  double accr[7], acci[7];
+  double apr[7], api[7], amr[7], ami[7];
 #pragma unroll
-  for (int c = 0; c < 7; ++c) accr[c] = acci[c] = 0.0;
+  for (int c = 0; c < 7; ++c) apr[c] = api[c] = amr[c] = ami[c] = 0.0;
   mbar_wait(&bars[0], 0);
   if (active && origin) {
-    for (int p = lane; p < P; p += 32) {
+    for (int p = half * 32 + lane; p < P; p += 64) {
       const double a = as[p];
 #pragma unroll
-      for (int c = 0; c < 7; ++c) accr[c] = fma(ws[c * P + p], a, accr[c]);
+      for (int c = 0; c < 7; ++c) apr[c] = fma(ws[c * P + p], a, apr[c]);
     }
   }
+  // sinc(pi u) = sin(pi u) / (pi u) from the product form sp of sin(pi u); see the header comment for the two guards
+  auto sinc_of = [&](double u, double sp) {
+    if (fabs(u) < 0x1p-10) sp = sinpi(u);
+    const double y = kPi * u;
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
+    r = fma(r, fma(-y, r, 1.0), r);
+    r = fma(r, fma(-y, r, 1.0), r);
+    return (u == 0.0) ? 1.0 : sp * r;
+  };
   for (int ch = 0; ch < nchunk; ++ch) {
     const int buf = ch & 1, e0 = ch * EC, cnt = min(EC, ne - e0);
     if (threadIdx.x == 0 && ch + 1 < nchunk) issue_chunk(ch + 1);  // (its buffer was released by the barrier that ended chunk ch - 1)
@@ -348,74 +364,90 @@ __global__ void __launch_bounds__(DPB * 32) table_sep_kernel(const Geometry *__r
     if (active && !origin) {
       const double *eb = reinterpret_cast<const double *>(ebase + buf * cbytes);
       const int *ep = reinterpret_cast<const int *>(ebase + buf * cbytes + 4 * EC * 8);
-      // four edges per lane and pass: all sixteen table loads are issued before the first is used (the direct-sinpi
-      // branch below would otherwise keep the compiler from hoisting the loads of the next edge above it)
-      for (int eb0 = lane; eb0 < cnt; eb0 += 128) {
-        double2 p1[4], p2[4], h1[4], h2[4];
+      // two edges per lane and pass: their eight table loads are issued before the first is used
+      for (int eb0 = half * 32 + lane; eb0 < cnt; eb0 += 128) {
+        double2 p1[2], p2[2], h1[2], h2[2];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const int e = min(eb0 + 32 * k, cnt - 1);
+        for (int k = 0; k < 2; ++k) {
+          const int e = min(eb0 + 64 * k, cnt - 1);
           p1[k] = __ldg(r1 + e0 + e);  // (cos, sin)(2 pi D1 mh1)
           p2[k] = __ldg(r2 + e0 + e);  // (cos, sin)(2 pi D2 mh2)
           h1[k] = __ldg(r3 + e0 + e);  // (cos, sin)(pi D1 eh1)
           h2[k] = __ldg(r4 + e0 + e);  // (cos, sin)(pi D2 eh2)
         }
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          const int e = eb0 + 32 * k;
+        for (int k = 0; k < 2; ++k) {
+          const int e = eb0 + 64 * k;
           if (e >= cnt) break;
-          const double u = fma((double)D1, eb[e], (double)D2 * eb[EC + e]);  // q.e / (2 pi)  ->  q.e/2 = pi u
-          const double cs = fma(p1[k].x, p2[k].x, -p1[k].y * p2[k].y), sn = fma(p1[k].y, p2[k].x, p1[k].x * p2[k].y);
-          double sp = fma(h1[k].y, h2[k].x, h1[k].x * h2[k].y);  // sin(pi u)
-          if (fabs(u) < 0x1p-10) sp = sinpi(u);
-          // 1 / (pi u) by the hardware's reciprocal estimate and two Newton steps (error ~1 ulp; an IEEE division
-          // with its special-case path is three times as many instructions); u == 0 yields inf/NaN, replaced below
-          const double y = kPi * u;
-          double r;
-          asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));
-          r = fma(r, fma(-y, r, 1.0), r);
-          r = fma(r, fma(-y, r, 1.0), r);
-          const double j0 = (u == 0.0) ? 1.0 : sp * r;
-          const double f = (qx * eb[3 * EC + e] - qy * eb[2 * EC + e]) * j0;
-          const double tr = f * cs, ti = f * sn;
+          const double t1 = (double)D1 * eb[e], t2 = (double)D2 * eb[EC + e];  // q.e / (2 pi) = t1 +- t2
+          const double cc = p1[k].x * p2[k].x, ss = p1[k].y * p2[k].y, sc = p1[k].y * p2[k].x, cs = p1[k].x * p2[k].y;
+          const double ba = h1[k].y * h2[k].x, ab = h1[k].x * h2[k].y;
+          const double exv = eb[2 * EC + e], eyv = eb[3 * EC + e];
           const int p = ep[e];
+          const double fp = (qxp * eyv - qyp * exv) * sinc_of(t1 + t2, ba + ab);
+          const double trp = fp * (cc - ss), tip = fp * (sc + cs);
+          double trm = 0.0, tim = 0.0;
+          if (minus) {
+            const double fm = (qxm * eyv - qym * exv) * sinc_of(t1 - t2, ba - ab);
+            trm = fm * (cc + ss);
+            tim = fm * (sc - cs);
+          }
 #pragma unroll
           for (int c = 0; c < 7; ++c) {
             const double w = ws[c * P + p];
-            accr[c] = fma(w, tr, accr[c]);
-            acci[c] = fma(w, ti, acci[c]);
+            apr[c] = fma(w, trp, apr[c]);
+            api[c] = fma(w, tip, api[c]);
+            amr[c] = fma(w, trm, amr[c]);
+            ami[c] = fma(w, tim, ami[c]);
           }
         }
       }
     }
     __syncthreads();  // every warp is done with this buffer: it may be refilled (chunk ch + 2)
   }
-  if (!active) return;
 #pragma unroll
   for (int c = 0; c < 7; ++c) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      accr[c] += __shfl_xor_sync(0xffffffffu, accr[c], o);
-      acci[c] += __shfl_xor_sync(0xffffffffu, acci[c], o);
+      apr[c] += __shfl_xor_sync(0xffffffffu, apr[c], o);
+      api[c] += __shfl_xor_sync(0xffffffffu, api[c], o);
+      amr[c] += __shfl_xor_sync(0xffffffffu, amr[c], o);
+      ami[c] += __shfl_xor_sync(0xffffffffu, ami[c], o);
     }
   }
-  cplx *T = batch_ptr(table, cell, 0);
-  if (lane < 7) {
-    double sr = 0.0, si = 0.0;
+  if (lane == 0) {
 #pragma unroll
     for (int c = 0; c < 7; ++c) {
-      sr = lane == c ? accr[c] : sr;
-      si = lane == c ? acci[c] : si;
+      part[warp * 28 + c] = apr[c];
+      part[warp * 28 + 7 + c] = api[c];
+      part[warp * 28 + 14 + c] = amr[c];
+      part[warp * 28 + 21 + c] = ami[c];
     }
-    const int c = lane;
+  }
+  __syncthreads();
+  if (!active || half != 0 || lane >= 7) return;
+  cplx *T = batch_ptr(table, cell, 0);
+  const int c = lane;
+  const double *pa = part + warp * 28, *pb = part + (warp + 1) * 28;  // the two halves, always summed in this order
+  {
+    const double sr = pa[c] + pb[c], si = pa[7 + c] + pb[7 + c];
+    const int flat = (D1 + 2 * Mt) * L + D2 + 2 * Mt;
     if (origin) {
       T[(size_t)c * L2 + flat] = cmake(sr, 0.0);
     } else {
-      const double inv = 1.0 / (qx * qx + qy * qy);
+      const double inv = 1.0 / (qxp * qxp + qyp * qyp);
       const double re = si * inv, im = -sr * inv;  // (-i) (sr + i si) / |q|^2
       T[(size_t)c * L2 + flat] = cmake(re, im);
       T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);  // T(-D) = conj T(D): Phi, R exactly Hermitian
     }
+  }
+  if (minus) {
+    const double sr = pa[14 + c] + pb[14 + c], si = pa[21 + c] + pb[21 + c];
+    const int flat = (D1 + 2 * Mt) * L - D2 + 2 * Mt;
+    const double inv = 1.0 / (qxm * qxm + qym * qym);
+    const double re = si * inv, im = -sr * inv;
+    T[(size_t)c * L2 + flat] = cmake(re, im);
+    T[(size_t)c * L2 + (L2 - 1 - flat)] = cmake(re, -im);
   }
 }
 
@@ -423,10 +455,10 @@ int launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, do
                   cudaStream_t s, int maxP, int max_nes, BatchRef scratch, long long scratch_elems) {
   const int L = 4 * Mt + 1;
   const int nhalf = (L * L + 1) / 2;
-  // algorithmic work: ~230 real flops per (index difference, edge) term when the formula is evaluated directly:
-  // sincospi + sinpi + the 7-channel accumulation, counted from the SASS of table_tma_kernel's loop body (about 95 DFMA,
-  // 25 DMUL, 15 DADD)
-  KScope ks(KC_TABLE, 230.0 * total_edges * nhalf, s);
+  // algorithmic work: 118 real flops per (index difference, edge) term = the formula evaluated directly (sincospi + sinpi
+  // + the division + the 7-channel accumulation), counted from the SASS of table_tma_kernel's edge loop: 50 DFMA,
+  // 15 DMUL, 3 DADD (profiles/r2_s1_table.md; SURVEY 8(d) estimated ~120).  Earlier rounds used 230, which was wrong.
+  KScope ks(KC_TABLE, 118.0 * total_edges * nhalf, s);
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -434,18 +466,19 @@ int launch_table(const Geometry *geo_dev, int ncells, int Mt, BatchRef table, do
     static unsigned long long mask = 0;
     ensure_dyn_smem(table_sep_kernel, 200 * 1024, mask);
     edge_phasor_kernel<<<dim3((max_nes + 127) / 128, L, ncells), 128, 0, s>>>(geo_dev, Mt, scratch);
-    // tile TA x TB of (D1, D2) per CTA (one CTA per SM): the shortest sequence of waves, then the most reuse of rows
+    // tile TA x TB of PAIRS (D1, +-D2), D1, D2 in [0, 2Mt], per CTA (one CTA per SM), two warps per pair: the shortest
+    // sequence of waves, then the most reuse of table rows
     const int n1 = 2 * Mt + 1;
     int TA = 1, TB = 1;
     long long best = -1;
     for (int a = 1; a <= 4; ++a)
-      for (int b = 1; a * b <= DPB; ++b) {
-        const long long tiles = (long long)((n1 + a - 1) / a) * ((L + b - 1) / b) * ncells;
+      for (int b = 1; 2 * a * b <= DPB; ++b) {
+        const long long tiles = (long long)((n1 + a - 1) / a) * ((n1 + b - 1) / b) * ncells;
         // a CTA's time: its warps share the FP64 pipe, but below ~8 warps the loop is bound by its own latency
-        const long long cost = ((tiles + sms - 1) / sms) * (a * b > 8 ? a * b : 8) * 1000 + (100 * (a + b)) / (a * b);
+        const long long cost = ((tiles + sms - 1) / sms) * (2 * a * b > 8 ? 2 * a * b : 8) * 1000 + (100 * (a + b)) / (a * b);
         if (best < 0 || cost < best) { best = cost; TA = a; TB = b; }
       }
-    table_sep_kernel<<<dim3(((n1 + TA - 1) / TA) * ((L + TB - 1) / TB), ncells), TA * TB * 32, table_sep_smem(maxP), s>>>(
+    table_sep_kernel<<<dim3(((n1 + TA - 1) / TA) * ((n1 + TB - 1) / TB), ncells), 2 * TA * TB * 32, table_sep_smem(maxP), s>>>(
         geo_dev, Mt, table, scratch, TA, TB);
     return 2;
   }
@@ -536,7 +569,7 @@ __global__ void __launch_bounds__(256) scatter_table_kernel(int Mt, int ncells, 
 
 void launch_phase_table(const Geometry &g, const int *poff, int Mt, cplx *Iph, int centroid_rule, cudaStream_t s) {
   const int L = 4 * Mt + 1, nhalf = (L * L + 1) / 2;
-  KScope ks(KC_TABLE, 230.0 * g.nedge * (double)nhalf, s);
+  KScope ks(KC_TABLE, 118.0 * g.nedge * (double)nhalf, s);
   phase_table_kernel<<<dim3((g.P + 127) / 128, nhalf), 128, 0, s>>>(g, poff, Mt, Iph, centroid_rule);
 }
 

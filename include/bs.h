@@ -177,6 +177,15 @@ bs_status bs_bands_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, cons
  * copy of the band and the vectors (about 2N x 2N complex more per k-point). */
 enum { BS_OPT_MODES = 7 };
 
+/* BS_OPT_REFINE (option 8; 0 = off, default; 1): bs_modes returns in omega2_out, instead of the eigenvalues of the assembled
+ * pencil, the Rayleigh quotients of its modes in factored form, omega^2_j = (H u_j)^dagger Phi^-1 (H u_j) / (u_j^dagger Psi u_j).
+ * The eigenvalues of K(k) = H^dagger Phi^-1 H carry an absolute error of ~eps lambda_max, which destroys the relative
+ * accuracy of the acoustic branches next to Gamma (omega^2 / lambda_max ~ 1e-10 at |k| = 1e-4 of the zone: omega wrong in
+ * the 7th digit); the factored quotient is accurate to ~eps kappa(Phi) relative (the accuracy of the singular-value route
+ * omega = sigma(L_Phi^-1 H L_Psi^-dagger), SURVEY 8(c)-7 / DESIGN.md R8, without forming an SVD) as long as
+ * omega^2 / lambda_max >~ 1e-12.  bs_bands is not affected. */
+enum { BS_OPT_REFINE = 8 };
+
 /* Mode shapes of the lowest nbands branches ("the eigenvectors U give the displacement mode shapes and
  * S = -Phi^-1 H* U the stress mode shapes").  One handle, nk k-points.
  *   omega2_out  nk x nbands doubles as bs_bands (host or device).

@@ -23,6 +23,7 @@ BS_OPT_ASSEMBLY = 4
 BS_OPT_PHI_INVERSE = 5
 BS_OPT_OUTPUT = 6
 BS_OPT_MODES = 7
+BS_OPT_REFINE = 8
 BS_OUTPUT_OMEGA2, BS_OUTPUT_OMEGA = 0, 1
 BS_ASSEMBLY_EXACT, BS_ASSEMBLY_CENTROID = 0, 1
 BS_PENCIL_POLY, BS_PENCIL_DIRECT = 0, 1

@@ -155,6 +155,7 @@ struct bs_cell {
   cudaEvent_t ev[BS_T_COUNT + 1] = {nullptr};
   bsk::KTimer *kt = nullptr;  // BS_OPT_TIMING = 2
   int nvmax = 0;                  // BS_OPT_MODES: bs_modes may return up to this many mode shapes per k-point
+  int refine = 0;                 // BS_OPT_REFINE: bs_modes returns the factored Rayleigh quotients of its modes
   bool keep_modes = false;        // set by bs_modes around its bs_bands pass: stage 1 keeps its reflectors and the band
   double *last_lam = nullptr;     // device eigenvalues of the last bs_bands pass (nmat x nbands)
   SharedGeom *shared = nullptr;   // bs_create_cells_shared
@@ -602,6 +603,10 @@ bs_status bs_set_option(bs_cell *c, int32_t option, int32_t value) {
       if (value < 0 || value > 2048) return fail(BS_ERR_ARG, "bs_set_option: BS_OPT_MODES must be 0..2048");
       if (c->nvmax != value) c->assembled = false;
       c->nvmax = value;
+      return BS_OK;
+    case BS_OPT_REFINE:
+      if (value != 0 && value != 1) return fail(BS_ERR_ARG, "bs_set_option: BS_OPT_REFINE must be 0 or 1");
+      c->refine = value;
       return BS_OK;
     case BS_OPT_TIMING:
       if (value < 0 || value > 2) return fail(BS_ERR_ARG, "bs_set_option: timing must be 0, 1 or 2");
@@ -1137,7 +1142,7 @@ bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands
     bsk::launch_zgemm(g, s); ++nl;
   }
   // 4. S = Phi^-1 H U with H = V B(k) (the paper's S = -Phi^-1 H* U; its H* is -H, R3)
-  if (S_out) {
+  if (S_out || cell->refine) {
     std::vector<double> kv((size_t)nk * 2 * N);
     const int W = 2 * Mt + 1;
     for (int k = 0; k < nk; ++k)
@@ -1160,8 +1165,20 @@ bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands
     g.B = R(L.HU, hs); g.ldb = n3;
     g.C = R(L.Sv, hs); g.ldc = n3;
     bsk::launch_zgemm(g, s); ++nl;
-    st = copy_blocks(S_out, (cplx *)cell->ws + L.Sv, (size_t)n3 * nbands, (size_t)hs, nk, s);
-    if (st != BS_OK) return st;
+    if (S_out) {
+      st = copy_blocks(S_out, (cplx *)cell->ws + L.Sv, (size_t)n3 * nbands, (size_t)hs, nk, s);
+      if (st != BS_OK) return st;
+    }
+    if (cell->refine) {
+      // 5. omega^2 again, as the Rayleigh quotient (H u)^dagger Phi^-1 (H u) / (y^dagger y) of every mode (BS_OPT_REFINE)
+      bsk::launch_rayleigh(n3, n2, R(L.HU, hs), R(L.Sv, hs), n3, R(L.Zv, zs), n2, cell->last_lam, nbands, 1, nk, s); ++nl;
+      cudaPointerAttributes attr;
+      bool on_device = false;
+      if (cudaPointerGetAttributes(&attr, omega2_out) == cudaSuccess) on_device = attr.type == cudaMemoryTypeDevice;
+      else cudaGetLastError();
+      CU(cudaMemcpyAsync(omega2_out, cell->last_lam, (size_t)nk * nbands * sizeof(double),
+                         on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+    }
   }
   if (U_out) {
     st = copy_blocks(U_out, (cplx *)cell->ws + L.Uv, (size_t)n2 * nbands, (size_t)zs, nk, s);

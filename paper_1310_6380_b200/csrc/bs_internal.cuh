@@ -212,6 +212,9 @@ void launch_band_invit(int n, int b, BatchRef AB, const double *lam, int nvec, B
 // HU = V B(k) U (3N x nvec from 2N x nvec); kap: per matrix [2][N] doubles (kx, ky of k + G).
 void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, const double *kap, int nvec, int ncells,
                     int inner, cudaStream_t s);
+// out[z * nvec + j] = Re (HU_j^dagger S_j) / (Y_j^dagger Y_j): the factored Rayleigh quotient of mode j of matrix z
+void launch_rayleigh(int n3, int n2, BatchRef HU, BatchRef S, int lds, BatchRef Y, int ldy, double *out, int nvec, int ncells,
+                     int inner, cudaStream_t s);
 // S7: Sturm bisection.  lam: per matrix nev doubles at lam + z*nev.
 void launch_sturm(int n, const double *d, const double *e, int nev, double *lam, int nmat, cudaStream_t s,
                   bool root = false);  // root: write sqrt(max(lambda, 0)) instead of lambda

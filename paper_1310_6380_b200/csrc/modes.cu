@@ -205,6 +205,33 @@ __global__ void __launch_bounds__(256) apply_h_kernel(int N, double V, BatchRef 
   h[N + g] = cmake(-V * ky * u2.y, V * ky * u2.x);
   h[2 * N + g] = cmake(-V * (ky * u1.y + kx * u2.y), V * (ky * u1.x + kx * u2.x));
 }
+
+// Rayleigh quotients in factored form: omega^2_j = (H u_j)^dagger (Phi^-1 H u_j) / (y_j^dagger y_j), u = L_Psi^-H y.
+// For omega^2 << lambda_max this is far more accurate than the eigenvalue of the assembled pencil (whose absolute error
+// is ~eps lambda_max): the quotient is second-order accurate in the vector and every factor is computed to a relative
+// error of ~eps kappa(Phi) (the singular-value route of SURVEY 8(c)-7 / reading R8, reached without an SVD).
+__global__ void __launch_bounds__(256) rayleigh_kernel(int n3, int n2, BatchRef HU, BatchRef S, int lds, BatchRef Y, int ldy,
+                                                       double *__restrict__ out, int nvec, int inner) {
+  __shared__ double red[2][8];
+  const int z = blockIdx.y, cell = z / inner, mi = z % inner, j = blockIdx.x;
+  const cplx *h = batch_ptr(HU, cell, mi) + (size_t)j * lds, *sv = batch_ptr(S, cell, mi) + (size_t)j * lds;
+  const cplx *y = batch_ptr(Y, cell, mi) + (size_t)j * ldy;
+  double num = 0.0, den = 0.0;
+  for (int i = threadIdx.x; i < n3; i += 256) num += h[i].x * sv[i].x + h[i].y * sv[i].y;  // Re conj(h) s
+  for (int i = threadIdx.x; i < n2; i += 256) den += y[i].x * y[i].x + y[i].y * y[i].y;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    num += __shfl_xor_sync(0xffffffffu, num, o);
+    den += __shfl_xor_sync(0xffffffffu, den, o);
+  }
+  if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = num; red[1][threadIdx.x >> 5] = den; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b = 0.0;
+    for (int w = 0; w < 8; ++w) { a += red[0][w]; b += red[1][w]; }
+    out[(size_t)z * nvec + j] = a / b;
+  }
+}
 }  // namespace
 
 size_t band_invit_lu_elems(int n, int b) { return (size_t)n * (2 * b + 1) + (size_t)n * b + (size_t)n / 4 + 16; }
@@ -222,6 +249,12 @@ void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, 
                     int inner, cudaStream_t s) {
   KScope ks(KC_OTHER, 0.0, s);
   apply_h_kernel<<<dim3((N + 255) / 256, nvec, ncells * inner), 256, 0, s>>>(N, V, U, ldu, HU, ldh, kap, nvec, inner);
+}
+
+void launch_rayleigh(int n3, int n2, BatchRef HU, BatchRef S, int lds, BatchRef Y, int ldy, double *out, int nvec, int ncells,
+                     int inner, cudaStream_t s) {
+  KScope ks(KC_OTHER, 0.0, s);
+  rayleigh_kernel<<<dim3(nvec, ncells * inner), 256, 0, s>>>(n3, n2, HU, S, lds, Y, ldy, out, nvec, inner);
 }
 
 }  // namespace bsk

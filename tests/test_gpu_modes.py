@@ -150,6 +150,40 @@ def test_modes_homogeneous_cell_polarisation_on_gpu(bs):
         assert np.max(np.abs(got - sig)) < 1e-8 * np.max(np.abs(sig))
 
 
+def test_refined_frequencies_next_to_gamma_have_singular_value_accuracy(bs):
+    """NEXT-4 (R8): next to Gamma the acoustic omega^2 are ~1e-8 .. 1e-12 of lambda_max, so the
+    eigenvalues of the assembled pencil lose them in the 9th .. 5th digit (the backward-error clause of R8 is what lets
+    bs_bands pass there).  With BS_OPT_REFINE bs_modes returns the factored Rayleigh quotients, which must agree with the
+    oracle's singular-value route (omega = sigma(L_Phi^-1 H L_Psi^-dagger)) to <= 1e-9 relative on EVERY branch."""
+    cell = wl.get("C1").cells[0]
+    Mt, nb = 3, 6
+    comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu)
+    kpts = np.array([[1e-2, 3e-3], [1e-3, 3e-4], [1e-4, 3e-5], [3e-5, -1e-5], [0.31, 0.17]])
+    h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho)
+    bs.bs_set_option(h, bs.BS_OPT_MODES, nb)
+    bs.allocate_workspace(h, Mt, len(kpts))
+    bs.bs_assemble(h, Mt)
+    lam_plain = bs.bs_bands(h, kpts, nb)
+    bs.bs_set_option(h, bs.BS_OPT_REFINE, 1)
+    lam_ref, U, S = bs.bs_modes(h, kpts, nb)
+    bs.bs_set_option(h, bs.BS_OPT_REFINE, 0)
+    lam_off, _, _ = bs.bs_modes(h, kpts, nb)
+    bs.bs_destroy_cell(h)
+    # the option off: the eigenvalues of the assembled pencil as bs_bands returns them (bs_modes always takes the two-stage
+    # reduction, bs_bands the shared-memory kernel at this size: equal to the backward error of either)
+    Phi, Psi = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho, Mt)
+    worst_plain = 0.0
+    for i, kr in enumerate(kpts):
+        lmax = oracle.bands_at_k(Phi, Psi, cell.lattice, Mt, kr)[1]
+        assert np.max(np.abs(lam_off[i] - lam_plain[i])) <= 64 * EPS * lmax
+        om = oracle.omega_svd_route(Phi, Psi, cell.lattice, Mt, kr)[:nb]
+        err = np.abs(np.sqrt(lam_ref[i]) - om) / om
+        assert np.all(lam_ref[i] > 0) and err.max() <= 1e-9, (i, err)
+        worst_plain = max(worst_plain, np.max(np.abs(np.sqrt(np.maximum(lam_plain[i], 0)) - om) / om))
+    # the plain route really is not good enough here (otherwise this test shows nothing)
+    assert worst_plain > 1e-8
+
+
 def test_modes_error_paths(bs):
     cell = wl.random_small_cell(1, 2)
     h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, bs.bs_isotropic_plane_strain(cell.E, cell.nu), cell.rho)

@@ -199,6 +199,11 @@ enum { BS_OPT_REFINE = 8 };
  * Errors: BS_ERR_STATE (BS_OPT_MODES not set, or omega output selected), BS_ERR_ARG (nbands > BS_OPT_MODES), as bs_bands. */
 bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *U_out,
                    void *S_out, void *stream);
+/* The same for a batch of handles (as bs_bands_batch: equal options, truncation and cell area; ncells * nk <= 65535): omega2_out
+ * ncells x nk x nbands; U_out ncells x nk blocks of 2N x nbands; S_out ncells x nk blocks of 3N x nbands, cell-major.  Every
+ * matrix is treated exactly as in the single-handle call (bitwise equal results). */
+bs_status bs_modes_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, const double *kpts, int32_t nbands,
+                         double *omega2_out, void *U_out, void *S_out, void *stream);
 
 /* Parity access after bs_bands: the tridiagonal T(k) of the last call, HOST out: d (nk x 2N), e (nk x 2N, last unused). */
 bs_status bs_get_tridiagonal(bs_cell *cell, double *d_host, double *e_host);

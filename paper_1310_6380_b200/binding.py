@@ -34,7 +34,7 @@ BS_GEMM_LOWER_ONLY, BS_GEMM_KLO_ROW, BS_GEMM_KHI_ROW, BS_GEMM_KLO_COL, BS_GEMM_K
 SYMBOLS = [
     "bs_isotropic_plane_strain", "bs_create_cell", "bs_create_cells_shared", "bs_set_properties", "bs_destroy_cell", "bs_set_option", "bs_workspace_bytes",
     "bs_set_workspace", "bs_assemble", "bs_assemble_batch", "bs_get_matrices", "bs_get_table", "bs_get_pencil",
-    "bs_bands", "bs_bands_batch", "bs_modes", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
+    "bs_bands", "bs_bands_batch", "bs_modes", "bs_modes_batch", "bs_get_tridiagonal", "bs_get_timings", "bs_get_kernel_timings", "bs_launch_count",
     "bs_last_error",
     "bs_fp64_peak", "bs_zgemm", "bs_zpotrf_trtri", "bs_zhetrd_scratch_elems", "bs_zhetrd", "bs_sturm",
     "bs_zhetrd_static_bytes", "bs_zhetrd_static",
@@ -83,6 +83,7 @@ lib.bs_get_pencil.argtypes = [_vp, _dp, _vp, _vp]
 lib.bs_bands.argtypes = [_vp, C.c_int32, _dp, C.c_int32, _vp, _vp]
 lib.bs_bands_batch.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int32, _dp, C.c_int32, _vp, _vp]
 lib.bs_modes.argtypes = [_vp, C.c_int32, _dp, C.c_int32, _vp, _vp, _vp, _vp]
+lib.bs_modes_batch.argtypes = [C.POINTER(_vp), C.c_int32, C.c_int32, _dp, C.c_int32, _vp, _vp, _vp, _vp]
 lib.bs_get_tridiagonal.argtypes = [_vp, _dp, _dp]
 lib.bs_get_timings.argtypes = [_vp, _dp]
 lib.bs_get_kernel_timings.argtypes = [_vp, _dp, _dp, C.POINTER(C.c_int64)]
@@ -315,6 +316,20 @@ def bs_modes(cell: Cell, kpts, nbands: int, stress: bool = True, stream=None):
                         C.c_void_p(S.ctypes.data) if stress else None, _stream(stream)))
     cell.last_nmat = nk
     return lam, U.transpose(0, 2, 1), (S.transpose(0, 2, 1) if stress else None)
+
+
+def bs_modes_batch(cells: Sequence[Cell], kpts, nbands: int, stress: bool = True, stream=None):
+    """bs_modes for a batch of handles: (omega2 (ncells, nk, nbands), U (ncells, nk, 2N, nbands), S (ncells, nk, 3N, nbands)
+    or None) as host NumPy arrays."""
+    k = _f64(kpts).reshape(-1, 2)
+    nc, nk, N = len(cells), k.shape[0], cells[0].N
+    lam = np.empty((nc, nk, nbands))
+    U = np.empty((nc, nk, nbands, 2 * N), dtype=np.complex128)
+    S = np.empty((nc, nk, nbands, 3 * N), dtype=np.complex128) if stress else None
+    _check(lib.bs_modes_batch(_handles(cells), nc, nk, _ptr(k), nbands, C.c_void_p(lam.ctypes.data), C.c_void_p(U.ctypes.data),
+                              C.c_void_p(S.ctypes.data) if stress else None, _stream(stream)))
+    cells[0].last_nmat = nc * nk
+    return lam, U.transpose(0, 1, 3, 2), (S.transpose(0, 1, 3, 2) if stress else None)
 
 
 def bs_get_tridiagonal(cell: Cell, nmat: Optional[int] = None):

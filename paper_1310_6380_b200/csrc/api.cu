@@ -1082,35 +1082,35 @@ static bs_status copy_blocks(void *dst, const cplx *src, size_t block, size_t sr
   return BS_OK;
 }
 
-bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *U_out, void *S_out,
-                   void *stream) {
-  if (!cell || !kpts || !omega2_out || (!U_out && !S_out)) return fail(BS_ERR_ARG, "bs_modes: null argument");
+bs_status bs_modes_batch(bs_cell *const *cells, int32_t ncells, int32_t nk, const double *kpts, int32_t nbands,
+                         double *omega2_out, void *U_out, void *S_out, void *stream) {
+  if (!cells || ncells < 1 || !cells[0] || !kpts || !omega2_out || (!U_out && !S_out)) return fail(BS_ERR_ARG, "bs_modes: null argument");
+  bs_cell *cell = cells[0];  // the lead: options are equal across the batch (checked by bs_bands_batch)
   if (cell->nvmax < 1) return fail(BS_ERR_STATE, "bs_modes: set BS_OPT_MODES (before sizing the workspace and bs_assemble) first");
   if (nbands < 1 || nbands > cell->nvmax) return fail(BS_ERR_ARG, "bs_modes: nbands must be in 1..BS_OPT_MODES = %d", cell->nvmax);
   if (cell->out_root) return fail(BS_ERR_STATE, "bs_modes: needs BS_OPT_OUTPUT = BS_OUTPUT_OMEGA2");
   cudaStream_t s = (cudaStream_t)stream;
   // S4..S7 with the reflectors of stage 1 and the band kept
   cell->keep_modes = true;
-  bs_status st = bs_bands_batch(&cell, 1, nk, kpts, nbands, omega2_out, stream);
+  bs_status st = bs_bands_batch(cells, ncells, nk, kpts, nbands, omega2_out, stream);
   cell->keep_modes = false;
   if (st != BS_OK) return st;
-  bs_cell *cells[1] = {cell};
   const int Mt = cell->lay.Mt;
   const Layout L = make_layout(Mt, nk, cell->mode, cell->nb, cell->nvmax);
   const int N = L.N, n2 = 2 * N, n3 = 3 * N, nv = cell->nvmax;
   const int bw = cell->nb > 0 ? band_width(cell->nb) : auto_band_width(n2);
-  auto R = [&](long long off, long long stride = 0) { return ref(cell, 1, cells, off, stride); };
+  auto R = [&](long long off, long long stride = 0) { return ref(cell, ncells, cells, off, stride); };
   const long long zs = (long long)n2 * nv;
   int64_t nl = 0;
   // 1. eigenvectors of the band matrix by inverse iteration at the eigenvalues of S7
-  bsk::launch_band_invit(n2, bw, R(L.AB2, L.ab_stride), cell->last_lam, nbands, R(L.Zv, zs), R(L.LU, L.lu_stride), 1, nk, s); ++nl;
+  bsk::launch_band_invit(n2, bw, R(L.AB2, L.ab_stride), cell->last_lam, nbands, R(L.Zv, zs), R(L.LU, L.lu_stride), ncells, nk, s); ++nl;
   // 2. back through the block reflectors of stage 1, last panel first: Z[r0:] -= V (T (V^H Z[r0:]))
   int c_last = -1;
   for (int c0 = 0; c0 + bw < n2 - 1; c0 += bw) c_last = c0;
   for (int c0 = c_last; c0 >= 0; c0 -= bw) {
     const int r0 = c0 + bw, m = n2 - r0;
     bsk::GemmDesc g{};
-    g.ncells = 1; g.inner = nk; g.kclass = bsk::KC_OTHER;
+    g.ncells = ncells; g.inner = nk; g.kclass = bsk::KC_OTHER;
     g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
     g.M = bw; g.N = nbands; g.K = m; g.opA = 1; g.opB = 0;
     g.A = R(L.Vall + (long long)c0 * n2 + r0, (long long)n2 * n2); g.lda = n2;
@@ -1133,7 +1133,7 @@ bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands
   // 3. U = L_Psi^-H y = diag(X_R^H, X_R^H) y   (U^H Psi U = y^H y = I)
   for (int blk = 0; blk < 2; ++blk) {
     bsk::GemmDesc g{};
-    g.ncells = 1; g.inner = nk; g.kclass = bsk::KC_OTHER;
+    g.ncells = ncells; g.inner = nk; g.kclass = bsk::KC_OTHER;
     g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
     g.M = N; g.N = nbands; g.K = N; g.opA = 1; g.opB = 0;
     g.A = R(L.XR, 0); g.lda = N;
@@ -1145,49 +1145,57 @@ bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands
   if (S_out || cell->refine) {
     std::vector<double> kv((size_t)nk * 2 * N);
     const int W = 2 * Mt + 1;
-    for (int k = 0; k < nk; ++k)
-      for (int a1 = -Mt; a1 <= Mt; ++a1)
-        for (int a2 = -Mt; a2 <= Mt; ++a2) {
-          const int g = (a1 + Mt) * W + (a2 + Mt);
-          const double f1 = kpts[2 * k] + a1, f2 = kpts[2 * k + 1] + a2;
-          kv[((size_t)k * 2 + 0) * N + g] = f1 * cell->Q[0] + f2 * cell->Q[2];
-          kv[((size_t)k * 2 + 1) * N + g] = f1 * cell->Q[1] + f2 * cell->Q[3];
-        }
-    double *kap = reinterpret_cast<double *>((cplx *)cell->ws + L.kapm);
-    CU(cudaMemcpyAsync(kap, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    for (int c = 0; c < ncells; ++c) {  // (k + G) in Cartesian components, per cell: [k][x | y][N] doubles in its workspace
+      for (int k = 0; k < nk; ++k)
+        for (int a1 = -Mt; a1 <= Mt; ++a1)
+          for (int a2 = -Mt; a2 <= Mt; ++a2) {
+            const int g = (a1 + Mt) * W + (a2 + Mt);
+            const double f1 = kpts[2 * k] + a1, f2 = kpts[2 * k + 1] + a2;
+            kv[((size_t)k * 2 + 0) * N + g] = f1 * cells[c]->Q[0] + f2 * cells[c]->Q[2];
+            kv[((size_t)k * 2 + 1) * N + g] = f1 * cells[c]->Q[1] + f2 * cells[c]->Q[3];
+          }
+      // (pageable source: the copy is staged before the call returns, so kv may be refilled for the next cell)
+      CU(cudaMemcpyAsync((cplx *)cells[c]->ws + L.kapm, kv.data(), kv.size() * sizeof(double), cudaMemcpyHostToDevice, s));
+    }
     const long long hs = (long long)n3 * nv;
-    bsk::launch_apply_h(N, cell->V, R(L.Uv, zs), n2, R(L.HU, hs), n3, kap, nbands, 1, nk, s); ++nl;
+    bsk::launch_apply_h(N, cell->V, R(L.Uv, zs), n2, R(L.HU, hs), n3, R(L.kapm, N), nbands, ncells, nk, s); ++nl;
     bsk::GemmDesc g{};
-    g.ncells = 1; g.inner = nk; g.kclass = bsk::KC_OTHER;
+    g.ncells = ncells; g.inner = nk; g.kclass = bsk::KC_OTHER;
     g.alpha = cmake(1.0, 0.0); g.beta = cmake(0.0, 0.0);
     g.M = n3; g.N = nbands; g.K = n3; g.opA = 0; g.opB = 0;
     g.A = R(L.Y, 0); g.lda = n3;
     g.B = R(L.HU, hs); g.ldb = n3;
     g.C = R(L.Sv, hs); g.ldc = n3;
     bsk::launch_zgemm(g, s); ++nl;
-    if (S_out) {
-      st = copy_blocks(S_out, (cplx *)cell->ws + L.Sv, (size_t)n3 * nbands, (size_t)hs, nk, s);
+    for (int c = 0; S_out && c < ncells; ++c) {
+      st = copy_blocks((cplx *)S_out + (size_t)c * nk * n3 * nbands, (cplx *)cells[c]->ws + L.Sv, (size_t)n3 * nbands, (size_t)hs, nk, s);
       if (st != BS_OK) return st;
     }
     if (cell->refine) {
       // 5. omega^2 again, as the Rayleigh quotient (H u)^dagger Phi^-1 (H u) / (y^dagger y) of every mode (BS_OPT_REFINE)
-      bsk::launch_rayleigh(n3, n2, R(L.HU, hs), R(L.Sv, hs), n3, R(L.Zv, zs), n2, cell->last_lam, nbands, 1, nk, s); ++nl;
+      bsk::launch_rayleigh(n3, n2, R(L.HU, hs), R(L.Sv, hs), n3, R(L.Zv, zs), n2, cell->last_lam, nbands, ncells, nk, s); ++nl;
       cudaPointerAttributes attr;
       bool on_device = false;
       if (cudaPointerGetAttributes(&attr, omega2_out) == cudaSuccess) on_device = attr.type == cudaMemoryTypeDevice;
       else cudaGetLastError();
-      CU(cudaMemcpyAsync(omega2_out, cell->last_lam, (size_t)nk * nbands * sizeof(double),
+      CU(cudaMemcpyAsync(omega2_out, cell->last_lam, (size_t)ncells * nk * nbands * sizeof(double),
                          on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
     }
   }
-  if (U_out) {
-    st = copy_blocks(U_out, (cplx *)cell->ws + L.Uv, (size_t)n2 * nbands, (size_t)zs, nk, s);
+  for (int c = 0; U_out && c < ncells; ++c) {
+    st = copy_blocks((cplx *)U_out + (size_t)c * nk * n2 * nbands, (cplx *)cells[c]->ws + L.Uv, (size_t)n2 * nbands, (size_t)zs, nk, s);
     if (st != BS_OK) return st;
   }
   cell->launches += nl;
   CU(cudaStreamSynchronize(s));
   CU(cudaGetLastError());
   return BS_OK;
+}
+
+bs_status bs_modes(bs_cell *cell, int32_t nk, const double *kpts, int32_t nbands, double *omega2_out, void *U_out, void *S_out,
+                   void *stream) {
+  if (!cell) return fail(BS_ERR_ARG, "bs_modes: null argument");
+  return bs_modes_batch(&cell, 1, nk, kpts, nbands, omega2_out, U_out, S_out, stream);
 }
 
 bs_status bs_get_tridiagonal(bs_cell *c, double *d_host, double *e_host) {

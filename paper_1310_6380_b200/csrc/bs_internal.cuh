@@ -210,8 +210,8 @@ size_t band_invit_lu_elems(int n, int b);
 void launch_band_invit(int n, int b, BatchRef AB, const double *lam, int nvec, BatchRef Z, BatchRef LU, int ncells, int inner,
                        cudaStream_t s);
 // HU = V B(k) U (3N x nvec from 2N x nvec); kap: per matrix [2][N] doubles (kx, ky of k + G).
-void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, const double *kap, int nvec, int ncells,
-                    int inner, cudaStream_t s);
+void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, BatchRef KAP, int nvec, int ncells,
+                    int inner, cudaStream_t s);  // KAP: per matrix [kx | ky][N] doubles (stride N complex elements)
 // out[z * nvec + j] = Re (HU_j^dagger S_j) / (Y_j^dagger Y_j): the factored Rayleigh quotient of mode j of matrix z
 void launch_rayleigh(int n3, int n2, BatchRef HU, BatchRef S, int lds, BatchRef Y, int ldy, double *out, int nvec, int ncells,
                      int inner, cudaStream_t s);

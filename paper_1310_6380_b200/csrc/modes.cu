@@ -191,14 +191,15 @@ __global__ void __launch_bounds__(MT) band_invit_kernel(int n, int b, int ld, Ba
 
 // HU = V B(k) U on the N plane waves of every mode (eq. 18; H = V B, B = i (k + G) on diagonal blocks):
 // rows (1,g) = i V kx_g U1[g], (2,g) = i V ky_g U2[g], (3,g) = i V (ky_g U1[g] + kx_g U2[g]).
-__global__ void __launch_bounds__(256) apply_h_kernel(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh,
-                                                      const double *__restrict__ kap, int nvec, int inner) {
+__global__ void __launch_bounds__(256) apply_h_kernel(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, BatchRef KAP,
+                                                      int nvec, int inner) {
   const int z = blockIdx.z, cell = z / inner, mi = z % inner;
   const int g = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
   if (g >= N || j >= nvec) return;
   const cplx *u = batch_ptr(U, cell, mi) + (size_t)j * ldu;
   cplx *h = batch_ptr(HU, cell, mi) + (size_t)j * ldh;
-  const double kx = kap[((size_t)z * 2 + 0) * N + g], ky = kap[((size_t)z * 2 + 1) * N + g];
+  const double *kap = reinterpret_cast<const double *>(batch_ptr(KAP, cell, mi));  // [x | y][N] doubles of this k-point
+  const double kx = kap[g], ky = kap[N + g];
   const cplx u1 = u[g], u2 = u[N + g];
   // i * (a + i b) = -b + i a
   h[g] = cmake(-V * kx * u1.y, V * kx * u1.x);
@@ -245,10 +246,10 @@ void launch_band_invit(int n, int b, BatchRef AB, const double *lam, int nvec, B
   band_invit_kernel<<<ncells * inner, MT, smem, s>>>(n, b, 2 * b, AB, lam, nvec, Z, LU, inner);
 }
 
-void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, const double *kap, int nvec, int ncells,
+void launch_apply_h(int N, double V, BatchRef U, int ldu, BatchRef HU, int ldh, BatchRef KAP, int nvec, int ncells,
                     int inner, cudaStream_t s) {
   KScope ks(KC_OTHER, 0.0, s);
-  apply_h_kernel<<<dim3((N + 255) / 256, nvec, ncells * inner), 256, 0, s>>>(N, V, U, ldu, HU, ldh, kap, nvec, inner);
+  apply_h_kernel<<<dim3((N + 255) / 256, nvec, ncells * inner), 256, 0, s>>>(N, V, U, ldu, HU, ldh, KAP, nvec, inner);
 }
 
 void launch_rayleigh(int n3, int n2, BatchRef HU, BatchRef S, int lds, BatchRef Y, int ldy, double *out, int nvec, int ncells,

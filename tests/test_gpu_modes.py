@@ -184,6 +184,41 @@ def test_refined_frequencies_next_to_gamma_have_singular_value_accuracy(bs):
     assert worst_plain > 1e-8
 
 
+def test_modes_batch_equals_single_handle_calls(bs):
+    """bs_modes_batch over three cells with different geometries and lattices of equal area: every matrix is treated as in
+    the single-handle call, so eigenvalues, U and S agree bit for bit; with BS_OPT_REFINE the refined frequencies too."""
+    Mt, nb = 3, 5
+    kpts = np.array([[0.11, 0.07], [0.5, 0.5], [1e-3, 2e-3], [0.3, -0.2]])
+    cells = [wl.random_small_cell(31, 3), wl.random_small_cell(32, 4),
+             wl.random_small_cell(33, 3, np.array([[1.25, 0.0], [0.3, 0.8]]))]
+    def make(c):
+        h = bs.bs_create_cell(c.lattice, c.vert_offset, c.verts, oracle.isotropic_plane_strain_compliance(c.E, c.nu), c.rho)
+        bs.bs_set_option(h, bs.BS_OPT_MODES, nb)
+        bs.bs_set_option(h, bs.BS_OPT_REFINE, 1)
+        bs.allocate_workspace(h, Mt, len(kpts))
+        return h
+    hs = [make(c) for c in cells]
+    bs.bs_assemble_batch(hs, Mt)
+    lam_b, U_b, S_b = bs.bs_modes_batch(hs, kpts, nb)
+    N = (2 * Mt + 1) ** 2
+    assert lam_b.shape == (3, len(kpts), nb) and U_b.shape == (3, len(kpts), 2 * N, nb) and S_b.shape == (3, len(kpts), 3 * N, nb)
+    for c, h in enumerate(hs):
+        lam, U, S = bs.bs_modes(h, kpts, nb)
+        assert np.array_equal(lam, lam_b[c]) and np.array_equal(U, U_b[c]) and np.array_equal(S, S_b[c])
+        # and they are modes: Phi S = H U to rounding, refined frequencies against the oracle's singular-value route
+        cell = cells[c]
+        comp = oracle.isotropic_plane_strain_compliance(cell.E, cell.nu)
+        Phi, Psi = oracle.assemble(cell.lattice, cell.vert_offset, cell.verts, comp, cell.rho, Mt)
+        _, _, V = oracle.reciprocal_basis(cell.lattice)
+        for i, kr in enumerate(kpts):
+            H = V * oracle.coupling_B(cell.lattice, Mt, kr)
+            assert np.max(np.abs(Phi @ S[i] - H @ U[i])) <= 1e-10 * np.max(np.abs(H @ U[i]))
+            om = oracle.omega_svd_route(Phi, Psi, cell.lattice, Mt, kr)[:nb]
+            assert np.max(np.abs(np.sqrt(lam[i]) - om) / om) <= 1e-9
+    for h in hs:
+        bs.bs_destroy_cell(h)
+
+
 def test_modes_error_paths(bs):
     cell = wl.random_small_cell(1, 2)
     h = bs.bs_create_cell(cell.lattice, cell.vert_offset, cell.verts, bs.bs_isotropic_plane_strain(cell.E, cell.nu), cell.rho)

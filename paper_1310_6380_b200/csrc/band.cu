@@ -190,23 +190,36 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
       }
       block_reduce<12, NTHR>(gv, red, res);
       if (t == 0) {
+        // (every loop fully unrolled: Gm, Tl and taus stay in registers; with run-time indices they lived in local memory
+        // and this 4 x 4 recurrence alone took 12 % of the kernel)
         cplx Gm[SW][SW];
-        int e = 0;
+        {
+          int e = 0;
+#pragma unroll
+          for (int a = 0; a < SW; ++a)
+#pragma unroll
+            for (int c = a + 1; c < SW; ++c) { Gm[a][c] = cmake(gv[2 * e], gv[2 * e + 1]); ++e; }
+        }
+        // T is built in place in shared memory (row-major Tm[a * SW + c]; this thread reads back only what it wrote):
+        // the 64-register variants have no room for a second 4 x 4 complex array next to Gm
+#pragma unroll
         for (int a = 0; a < SW; ++a)
-          for (int c = a + 1; c < SW; ++c) { Gm[a][c] = cmake(gv[2 * e], gv[2 * e + 1]); ++e; }
-        cplx Tl[SW][SW];
-        for (int a = 0; a < SW; ++a)
-          for (int c = 0; c < SW; ++c) Tl[a][c] = cmake(0.0, 0.0);
+#pragma unroll
+          for (int c = 0; c < SW; ++c) Tm[a * SW + c] = cmake(0.0, 0.0);
+#pragma unroll
         for (int c = 0; c < SW; ++c) {
-          Tl[c][c] = taus[c];
-          for (int a = 0; a < c; ++a) {
-            cplx acc = cmake(0.0, 0.0);
-            for (int l2 = a; l2 < c; ++l2) cfma(acc, Tl[a][l2], Gm[l2][c]);
-            Tl[a][c] = cmul(cmake(-taus[c].x, -taus[c].y), acc);
+          Tm[c * SW + c] = taus[c];
+#pragma unroll
+          for (int a = 0; a < SW; ++a) {
+            if (a < c) {
+              cplx acc = cmake(0.0, 0.0);
+#pragma unroll
+              for (int l2 = 0; l2 < SW; ++l2)
+                if (l2 >= a && l2 < c) cfma(acc, Tm[a * SW + l2], Gm[l2][c]);
+              Tm[a * SW + c] = cmul(cmake(-taus[c].x, -taus[c].y), acc);
+            }
           }
         }
-        for (int a = 0; a < SW; ++a)
-          for (int c = 0; c < SW; ++c) Tm[a * SW + c] = Tl[a][c];
       }
     }
     // 4. V columns out

@@ -47,14 +47,13 @@ __device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double
     for (int k = 0; k < K; ++k) red[warp * K + k] = v[k];
   }
   __syncthreads();
-  if (warp == 0) {
+  // second level: value k by warp k mod (number of warps), not all K of them one after the other by warp 0 (the same
+  // butterfly over the same numbers: same bits)
+  for (int k = warp; k < K; k += NTHR / 32) {
+    double x = lane < NTHR / 32 ? red[lane * K + k] : 0.0;
 #pragma unroll
-    for (int k = 0; k < K; ++k) {
-      double x = lane < NTHR / 32 ? red[lane * K + k] : 0.0;
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-      if (lane == 0) res[k] = x;
-    }
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    if (lane == 0) res[k] = x;
   }
   __syncthreads();
 #pragma unroll

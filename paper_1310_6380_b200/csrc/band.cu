@@ -24,7 +24,11 @@
 namespace bsk {
 
 namespace {
-constexpr int KS = 8;         // split-K factor of the Gram product [G | S] = V^H [V | Z] (one output tile per matrix)
+constexpr int KS = 8;         // largest split-K factor of the Gram product [G | S] = V^H [V | Z] (one output tile per matrix)
+// The factor actually used depends on the number of rows only (never on the batch: a matrix gets the same bits alone and
+// in a batch): a tall product needs the parallelism, a short one only pays for writing and re-reading the partials
+// (C4, m <= 226: 128 KB per matrix and panel, 20 GB per step with KS = 8).
+inline int ksplit_of(int m) { return m >= 1024 ? 8 : (m >= 512 ? 4 : (m >= 256 ? 2 : 1)); }
 
 // Householder QR of the m x b panel block of every matrix, one CTA per matrix.  The panel is processed in sub-panels
 // of SW = 4 columns held in shared memory: a sub-panel is factored there (no global round trips between its columns), its
@@ -299,7 +303,7 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
 // (R: running right-hand sides; row l of T is final at step l: T[l, j] = tau_l R[l, j], then R[i, j] -= G[i, l] T[l, j]
 // for i < l).  tau_l = 0 (H_l = I) gives a zero row and column, as the forward recurrence does.
 // SM per matrix: [G | S] (b x 2b, ld b) at 0; [M2; T] (2b x b, ld 2b) at 2 b^2; tau at 4 b^2.
-__global__ void __launch_bounds__(1024) wy_small_kernel(int b, BatchRef SM, int inner) {
+__global__ void __launch_bounds__(1024) wy_small_kernel(int b, BatchRef SM, int inner, int ks) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *T = reinterpret_cast<cplx *>(smem_raw);  // b x b, T[i + j*b]
   cplx *S = T + b * b;                           // b x b
@@ -314,7 +318,7 @@ __global__ void __launch_bounds__(1024) wy_small_kernel(int b, BatchRef SM, int 
   if (t < b) taus[t] = sm[(size_t)4 * b * b + t];
   for (int i = t; i < b * b; i += blockDim.x) {
     cplx gs = cmake(0.0, 0.0), ss = cmake(0.0, 0.0);
-    for (int k = 0; k < KS; ++k) {  // fixed order: deterministic
+    for (int k = 0; k < ks; ++k) {  // fixed order: deterministic
       gs = cadd(gs, part[(size_t)k * 2 * b * b + i]);
       ss = cadd(ss, part[(size_t)k * 2 * b * b + b * b + i]);
     }
@@ -358,7 +362,7 @@ __global__ void __launch_bounds__(1024) wy_small_kernel(int b, BatchRef SM, int 
 //   W2 = V1^H V2 = Gm[0:b, 0:b],  G = V2^H V2 = Gm[b:2b, 0:b],  W1 = X1^H V2 = Gm[2b:3b, 0:b],  S0 = V2^H Z0 = Gm[b:2b, 2b:3b],
 //   S = S0 - W2^H W1 - W1^H W2,  T2 as in wy_small_kernel,  M2 = -1/2 T2^H S T2,  Cf = [-W1 T2; M2; -W2 T2; T2].
 // SM per matrix: Cf at 0; tau at 4 b^2; partials at 4 b^2 + 64.
-__global__ void __launch_bounds__(1024) wy_pair_kernel(int b, BatchRef SM, int inner) {
+__global__ void __launch_bounds__(1024) wy_pair_kernel(int b, BatchRef SM, int inner, int ks) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cplx *T = reinterpret_cast<cplx *>(smem_raw);  // b x b, T[i + j*b]
   cplx *S = T + b * b;
@@ -375,7 +379,7 @@ __global__ void __launch_bounds__(1024) wy_pair_kernel(int b, BatchRef SM, int i
   if (t < b) taus[t] = sm[(size_t)4 * b * b + t];
   auto gm = [&](int r, int c) {  // fixed order over the k-splits: deterministic
     cplx a = cmake(0.0, 0.0);
-    for (int k = 0; k < KS; ++k) a = cadd(a, part[(size_t)k * b3 * b3 + r + (size_t)c * b3]);
+    for (int k = 0; k < ks; ++k) a = cadd(a, part[(size_t)k * b3 * b3 + r + (size_t)c * b3]);
     return a;
   };
   for (int i = t; i < b * b; i += blockDim.x) {
@@ -510,11 +514,11 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     const int r0 = c0 + b, m = n - r0;
     qr(c0, sv, sv2);
     gemm(KC_GEMM_HEMM, m, b, m, 0, 0, BS_GEMM_A_HERM_LOWER, trailing(r0), lda, slot(sv, r0), n, slot(sv2 + 1, r0), n, 1.0, 0.0);
-    gemm(KC_GEMM_WY, b, 2 * b, m, 1, 0, 0, slot(sv, r0), n, slot(sv2, r0), n, smG, b, 1.0, 0.0, KS, (long long)2 * b * b);
+    gemm(KC_GEMM_WY, b, 2 * b, m, 1, 0, 0, slot(sv, r0), n, slot(sv2, r0), n, smG, b, 1.0, 0.0, ksplit_of(m), (long long)2 * b * b);
     {
       KScope ks(KC_OTHER, 0.0, s);
       // few matrices: one thread per entry (latency); many: smaller CTAs, several per SM (throughput)
-      wy_small_kernel<<<nmat, nmat > 592 ? 256 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
+      wy_small_kernel<<<nmat, nmat > 592 ? 256 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner, ksplit_of(m));
       ++launches;
     }
     keep(c0, sv, (long long)2 * b * b + b, 2 * b);
@@ -546,10 +550,10 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     // Z0 = A22 V2 with the trailing matrix as it was before panel 1's update -> slot 3
     gemm(KC_GEMM_HEMM, m2, b, m2, 0, 0, BS_GEMM_A_HERM_LOWER, trailing(r1), lda, slot(1, r1), n, slot(3, r1), n, 1.0, 0.0);
     // Gm = [V1 V2 X1]^H [V2 X1 Z0]  (3b x 3b, split-K)
-    gemm(KC_GEMM_WY, 3 * b, 3 * b, m2, 1, 0, 0, slot(0, r1), n, slot(1, r1), n, smG, 3 * b, 1.0, 0.0, KS, (long long)9 * b * b);
+    gemm(KC_GEMM_WY, 3 * b, 3 * b, m2, 1, 0, 0, slot(0, r1), n, slot(1, r1), n, smG, 3 * b, 1.0, 0.0, ksplit_of(m2), (long long)9 * b * b);
     {
       KScope ks(KC_OTHER, 0.0, s);
-      wy_pair_kernel<<<nmat, nmat > 592 ? 256 : b * b, (6 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner);
+      wy_pair_kernel<<<nmat, nmat > 592 ? 256 : b * b, (6 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner, ksplit_of(m2));
       ++launches;
     }
     keep(c1, 1, (long long)3 * b, 4 * b);

@@ -47,6 +47,44 @@ __device__ __forceinline__ double warp_sum(double x) {  // butterfly: every lane
   for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
   return x;
 }
+__device__ __forceinline__ cplx shfl_xor_c(cplx v, int m) {
+  return make_double2(__shfl_xor_sync(0xffffffffu, v.x, m), __shfl_xor_sync(0xffffffffu, v.y, m));
+}
+// Transposed reduction of NV values per lane over a group of lanes (stride s, 2s, ...): at every stage a lane keeps
+// half of its values and receives the partner's partial sums of those, so the stages move NV/2, NV/4, ... values instead
+// of NV each, and the lane ends with the total of ONE value (index returned in `own`); when a single value is left the
+// remaining stages are plain butterflies.  A kept sum is own + partner, exactly what the butterfly `x += shfl_xor(x)`
+// forms in that lane, and a + b = b + a bit for bit: the totals are the butterfly's bits.
+template <int NV, int STAGES>
+__device__ __forceinline__ cplx reduce_transposed(cplx (&v)[NV], int bits, int stride, int &own) {
+  static_assert(NV == 1 || NV == 2 || NV == 4, "");
+  own = 0;
+  cplx a;
+  int st = 0;
+  if (NV == 4) {
+    const int b0 = bits & 1;
+    const cplx k0 = b0 ? v[1] : v[0], k1 = b0 ? v[3] : v[2], s0 = b0 ? v[0] : v[1], s1 = b0 ? v[2] : v[3];
+    v[0] = cadd(k0, shfl_xor_c(s0, stride));
+    v[1] = cadd(k1, shfl_xor_c(s1, stride));
+    own = b0;
+    const int b1 = (bits >> 1) & 1;
+    const cplx k = b1 ? v[1] : v[0], sd = b1 ? v[0] : v[1];
+    a = cadd(k, shfl_xor_c(sd, 2 * stride));
+    own += 2 * b1;
+    st = 2;
+  } else if (NV == 2) {
+    const int b0 = bits & 1;
+    const cplx k = b0 ? v[1] : v[0], sd = b0 ? v[0] : v[1];
+    a = cadd(k, shfl_xor_c(sd, stride));
+    own = b0;
+    st = 1;
+  } else {
+    a = v[0];
+  }
+#pragma unroll
+  for (; st < STAGES; ++st) a = cadd(a, shfl_xor_c(a, stride << st));
+  return a;
+}
 __device__ __forceinline__ void named_bar(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -141,32 +179,37 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
       }
     }
   }
-  // p = D v: partial row sums over this warp's columns, then over the four lanes of a row
+  // p = D v: partial row sums over this warp's columns, then over the four lanes of a row (transposed reduction: lane
+  // (g, t), t < TR, ends with the sum of row 8 t + g)
 #pragma unroll
   for (int rt = 0; rt < TR; ++rt) {
 #pragma unroll
     for (int ci = 0; ci < TCW; ++ci)
 #pragma unroll
       for (int j = 0; j < 2; ++j) cfma(acc[rt], cmake(tre[rt][ci][j], tim[rt][ci][j]), vc[ci][j]);
-#pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
-      acc[rt].x += __shfl_xor_sync(0xffffffffu, acc[rt].x, o);
-      acc[rt].y += __shfl_xor_sync(0xffffffffu, acc[rt].y, o);
-    }
-    if (t == 0) ts[C::O_P + rw * B + 8 * rt + g] = acc[rt];
+  }
+  {
+    int own;
+    const cplx a = reduce_transposed<TR, 2>(acc, t, 1, own);
+    if (t < TR) ts[C::O_P + rw * B + 8 * own + g] = a;
   }
   if (NW > 1) named_bar(bar_id, 32 * NW);
   else __syncwarp();
-  // lane l = row l: p = tau D v, w = p - tau/2 (p^H v) v   (every D warp computes the same bits)
-  const int l = lane < B ? lane : B - 1;
+  // lane l = row l: p = tau D v, w = p - tau/2 (p^H v) v   (every D warp computes the same bits).  For B < 32 the upper
+  // lanes mirror the lower ones, so the lane sums need log2(B) butterfly stages.
+  const int l = B < 32 ? (lane & (B - 1)) : lane;
   cplx p = ts[C::O_P + l];
 #pragma unroll
   for (int w2 = 1; w2 < NW; ++w2) p = cadd(p, ts[C::O_P + w2 * B + l]);
   p = cmul(tau, p);
   const cplx v = vb[l];
-  const bool in = lane < L;
-  const double sr = warp_sum(in ? p.x * v.x + p.y * v.y : 0.0);  // p^H v
-  const double si = warp_sum(in ? p.x * v.y - p.y * v.x : 0.0);
+  const bool in = l < L;
+  double sr = in ? p.x * v.x + p.y * v.y : 0.0, si = in ? p.x * v.y - p.y * v.x : 0.0;  // p^H v
+#pragma unroll
+  for (int o = (B < 32 ? B : 32) / 2; o > 0; o >>= 1) {
+    sr += __shfl_xor_sync(0xffffffffu, sr, o);
+    si += __shfl_xor_sync(0xffffffffu, si, o);
+  }
   const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
   cplx w = p;
   cfma(w, alpha, v);
@@ -239,33 +282,31 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
       }
     }
   }
-  // u = C v: partial row sums; C[:,0] goes along
+  // u = C v: partial row sums (transposed reduction over the four lanes of a row); C[:,0] goes along
 #pragma unroll
   for (int rt = 0; rt < TR; ++rt) {
 #pragma unroll
     for (int ci = 0; ci < TCW; ++ci)
 #pragma unroll
       for (int j = 0; j < 2; ++j) cfma(acc[rt], cmake(tre[rt][ci][j], tim[rt][ci][j]), vc[ci][j]);
-#pragma unroll
-    for (int o = 1; o <= 2; o <<= 1) {
-      acc[rt].x += __shfl_xor_sync(0xffffffffu, acc[rt].x, o);
-      acc[rt].y += __shfl_xor_sync(0xffffffffu, acc[rt].y, o);
-    }
-    if (t == 0) {
-      ts[C::O_U + rw * B + 8 * rt + g] = acc[rt];
-      if (rw == 0) ts[C::O_C0 + 8 * rt + g] = cmake(tre[rt][0][0], tim[rt][0][0]);
-    }
+    if (t == 0 && rw == 0) ts[C::O_C0 + 8 * rt + g] = cmake(tre[rt][0][0], tim[rt][0][0]);
   }
   asm volatile("bar.arrive %0, %1;\n" ::"r"(team_bar), "r"(C::TT) : "memory");  // releases the D warps of the team
+  {
+    int own;
+    const cplx a = reduce_transposed<TR, 2>(acc, t, 1, own);
+    if (t < TR) ts[C::O_U + rw * B + 8 * own + g] = a;
+  }
   if (NW > 1) named_bar(bar_id, 32 * NW);
   else __syncwarp();
   // lane l = row l of C: x = C[:,0] - tau u (conj(v[0]) = 1), then the reflector that annihilates x below its first entry.
   // zlarfg, branch-free: no reflector when the block has a single row (L2 <= 1) or x is already e_1-shaped.
-  const int l = lane < B ? lane : B - 1;
+  // For B < 32 the upper lanes mirror the lower ones, so the lane sums need log2(B) butterfly stages.
+  const int l = B < 32 ? (lane & (B - 1)) : lane;
   cplx u = ts[C::O_U + l];
 #pragma unroll
   for (int w2 = 1; w2 < NW; ++w2) u = cadd(u, ts[C::O_U + w2 * B + l]);
-  const bool in = lane < L2;
+  const bool in = l < L2;
   cplx tu = cmul(tau, u);
   tu.x = in ? tu.x : 0.0;
   tu.y = in ? tu.y : 0.0;
@@ -274,11 +315,11 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   x.y = in ? x.y : 0.0;
   // three lane reductions in one butterfly: |x[1:]|^2 and sum_{l>=1} conj(x_l) (tau u)_l, which gives
   // s = v2^H (tau u) = (tau u)_0 + conj(scale) sum_{l>=1} conj(x_l) (tau u)_l  without a second pass over the lanes
-  double ss = lane >= 1 ? x.x * x.x + x.y * x.y : 0.0;
-  double sdr = lane >= 1 ? x.x * tu.x + x.y * tu.y : 0.0;
-  double sdi = lane >= 1 ? x.x * tu.y - x.y * tu.x : 0.0;
+  double ss = l >= 1 ? x.x * x.x + x.y * x.y : 0.0;
+  double sdr = l >= 1 ? x.x * tu.x + x.y * tu.y : 0.0;
+  double sdi = l >= 1 ? x.x * tu.y - x.y * tu.x : 0.0;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
+  for (int o = (B < 32 ? B : 32) / 2; o > 0; o >>= 1) {
     ss += __shfl_xor_sync(0xffffffffu, ss, o);
     sdr += __shfl_xor_sync(0xffffffffu, sdr, o);
     sdi += __shfl_xor_sync(0xffffffffu, sdi, o);
@@ -297,8 +338,8 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   scale.x = trivial ? 0.0 : scale.x;
   scale.y = trivial ? 0.0 : scale.y;
   cplx v2 = cmul(x, scale);
-  v2.x = lane == 0 ? 1.0 : v2.x;
-  v2.y = lane == 0 ? 0.0 : v2.y;
+  v2.x = l == 0 ? 1.0 : v2.x;
+  v2.y = l == 0 ? 0.0 : v2.y;
   const cplx sv = cadd(tu0, cmulc(cmake(sdr, sdi), scale));  // (tau u)_0 + conj(scale) sum conj(x_l) (tau u)_l
   const double s_re = sv.x, s_im = sv.y;
   if (lane < B) {
@@ -307,32 +348,29 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   }
   if (lane == 0) *tau_next = tau2;
   __syncwarp();
-  // z0 = v2^H C over this warp's columns: column sums over the tile rows, then over the eight lanes of a column
-  cplx z[TCW][2];
+  // z0 = v2^H C over this warp's columns: column sums over the tile rows, then over the eight lanes of a column by a
+  // transposed reduction: lane (g, t), g < 2 TCW, ends with the sum of column 8 (rw TCW + g / 2) + 2 t + g % 2 and forms
+  // that column's entry of y alone
+  cplx z[2 * TCW];
 #pragma unroll
-  for (int ci = 0; ci < TCW; ++ci) z[ci][0] = z[ci][1] = cmake(0.0, 0.0);
+  for (int q = 0; q < 2 * TCW; ++q) z[q] = cmake(0.0, 0.0);
 #pragma unroll
   for (int rt = 0; rt < TR; ++rt) {
     const cplx vr = vnext[8 * rt + g];
 #pragma unroll
     for (int ci = 0; ci < TCW; ++ci)
 #pragma unroll
-      for (int j = 0; j < 2; ++j) cfmac(z[ci][j], vr, cmake(tre[rt][ci][j], tim[rt][ci][j]));
+      for (int j = 0; j < 2; ++j) cfmac(z[2 * ci + j], vr, cmake(tre[rt][ci][j], tim[rt][ci][j]));
   }
-#pragma unroll
-  for (int ci = 0; ci < TCW; ++ci)
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-#pragma unroll
-      for (int o = 4; o <= 16; o <<= 1) {
-        z[ci][j].x += __shfl_xor_sync(0xffffffffu, z[ci][j].x, o);
-        z[ci][j].y += __shfl_xor_sync(0xffffffffu, z[ci][j].y, o);
-      }
-      // y = tau2 conj(z0 - s conj(v)) = tau2 (conj(z0) - conj(s) v)
-      const cplx vcj = vc[ci][j];
-      const cplx q = cmake(z[ci][j].x - (s_re * vcj.x + s_im * vcj.y), -z[ci][j].y - (s_re * vcj.y - s_im * vcj.x));
-      if (g == 0) ts[C::O_Y + 8 * (rw * TCW + ci) + 2 * t + j] = cmul(tau2, q);
-    }
+  {
+    int own;
+    const cplx zs = reduce_transposed<2 * TCW, 3>(z, g, 4, own);
+    const int co = 8 * (rw * TCW + (own >> 1)) + 2 * t + (own & 1);
+    // y = tau2 conj(z0 - s conj(v)) = tau2 (conj(z0) - conj(s) v)
+    const cplx vcj = vb[co];
+    const cplx q = cmake(zs.x - (s_re * vcj.x + s_im * vcj.y), -zs.y - (s_re * vcj.y - s_im * vcj.x));
+    if (g < 2 * TCW) ts[C::O_Y + co] = cmul(tau2, q);
+  }
   __syncwarp();
   // C -= (tau u) v^H + v2 y^H   (a, b, c, d) = (tau u, v, v2, y)
   const cplx *tuv = ts + C::O_TU, *yv = ts + C::O_Y;

@@ -101,6 +101,25 @@ struct Cfg {
   static_assert(TC % NW == 0, "tile columns split over the role's warps");
 };
 
+// The norm of a reflector's vector and its reciprocal, and a reciprocal, without the IEEE square root and division: their
+// fix-up sequences are ~25 dependent instructions each on the chain of every step.  rsqrt is good to 1 ulp, the Newton
+// step makes s * rsqrt(s) a square root good to about 1 ulp, the two Newton steps on rcp.approx (2^-23) a reciprocal
+// good to about 1 ulp: H = I - tau v v^H stays unitary to a few ulp (tau, v and beta are formed from the same values),
+// which is all the backward stability of the chase needs.  The subnormal range is flushed (d < 2.3e-308).
+__device__ __forceinline__ void norm_and_inverse(double s, double &nrm, double &inv) {
+  inv = rsqrt(s);
+  nrm = s * inv;
+  nrm = fma(fma(-nrm, nrm, s), 0.5 * inv, nrm);
+}
+__device__ __forceinline__ double fast_rcp(double d) {
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;\n" : "=d"(x) : "d"(d));
+  double e = fma(-d, x, 1.0);
+  x = fma(x, e, x);
+  e = fma(-d, x, 1.0);
+  return fma(x, e, x);
+}
+
 // LAPACK zlarfg on a vector spread over the 32 lanes of a warp (x valid for l < len; other lanes must hold 0):
 // H = I - tau v v^H, H^H x = beta e_1, beta real, v[0] = 1.  Returns v in x.
 __device__ __forceinline__ void warp_larfg(cplx &x, int len, int l, cplx &tau, double &beta) {
@@ -112,9 +131,12 @@ __device__ __forceinline__ void warp_larfg(cplx &x, int len, int l, cplx &tau, d
     x = (l == 0) ? cmake(1.0, 0.0) : cmake(0.0, 0.0);
     return;
   }
-  beta = -copysign(sqrt(al.x * al.x + al.y * al.y + ss), al.x);
-  tau = cmake((beta - al.x) / beta, -al.y / beta);
-  const double dr = al.x - beta, di = al.y, den = 1.0 / (dr * dr + di * di);
+  double nrm, inrm;
+  norm_and_inverse(al.x * al.x + al.y * al.y + ss, nrm, inrm);
+  beta = -copysign(nrm, al.x);
+  const double ib = -copysign(inrm, al.x);
+  tau = cmake((beta - al.x) * ib, -al.y * ib);
+  const double dr = al.x - beta, di = al.y, den = fast_rcp(dr * dr + di * di);
   const cplx scale = cmake(dr * den, -di * den);
   if (l == 0) x = cmake(1.0, 0.0);
   else if (l < len) x = cmul(x, scale);
@@ -326,14 +348,15 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   }
   const cplx al = shfl_c(x, 0), tu0 = shfl_c(tu, 0);
   const bool norefl = L2 <= 1, trivial = norefl || (ss == 0.0 && al.y == 0.0);
-  const double nrm = sqrt(al.x * al.x + al.y * al.y + ss);
+  double nrm, inrm;
+  norm_and_inverse(al.x * al.x + al.y * al.y + ss, nrm, inrm);
   const double beta2 = trivial ? 1.0 : -copysign(nrm, al.x);
-  const double ib = 1.0 / beta2;
+  const double ib = trivial ? 1.0 : -copysign(inrm, al.x);
   cplx tau2 = cmake((beta2 - al.x) * ib, -al.y * ib);
   tau2.x = trivial ? 0.0 : tau2.x;
   tau2.y = trivial ? 0.0 : tau2.y;
   const double dr = al.x - beta2, di = al.y;
-  const double den = 1.0 / (dr * dr + di * di);
+  const double den = fast_rcp(dr * dr + di * di);
   cplx scale = cmake(dr * den, -di * den);
   scale.x = trivial ? 0.0 : scale.x;
   scale.y = trivial ? 0.0 : scale.y;

@@ -41,14 +41,37 @@ constexpr int SW = 4;  // sub-panel width
 template <int K, int NTHR>
 __device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double *res) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (K == 1) {
 #pragma unroll
-  for (int k = 0; k < K; ++k) {
+    for (int o = 16; o > 0; o >>= 1) v[0] += __shfl_xor_sync(0xffffffffu, v[0], o);
+    if (lane == 0) red[warp * K] = v[0];
+  } else {
+    // first level, transposed: at the stage with partner distance 16, 8, ... a lane keeps half of its values and receives
+    // the partner's partial sums of those (KP/2 + KP/4 + ... exchanges instead of 5 KP); a kept sum is own + partner, the
+    // butterfly's own operation in the same stage order, so the totals have the butterfly's bits.  Lane bit 4 - s chooses at
+    // stage s: the lane ends with value own = bit4 + 2 bit3 + ...
+    constexpr int KP = K <= 2 ? 2 : (K <= 4 ? 4 : (K <= 8 ? 8 : 16));
+    static_assert(K <= 16, "");
+    double w[KP];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
-  }
-  if (lane == 0) {
+    for (int k = 0; k < KP; ++k) w[k] = k < K ? v[k] : 0.0;
+    int own = 0;
 #pragma unroll
-    for (int k = 0; k < K; ++k) red[warp * K + k] = v[k];
+    for (int st = 0; st < 5; ++st) {
+      const int o = 16 >> st, cnt = KP >> (st + 1);
+      if (cnt >= 1) {
+        const int bit = (lane >> (4 - st)) & 1;
+#pragma unroll
+        for (int q = 0; q < cnt; ++q) {
+          const double keep = bit ? w[2 * q + 1] : w[2 * q], send = bit ? w[2 * q] : w[2 * q + 1];
+          w[q] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+        }
+        own += bit << st;
+      } else {
+        w[0] += __shfl_xor_sync(0xffffffffu, w[0], o);
+      }
+    }
+    if ((lane & (32 / KP - 1)) == 0 && own < K) red[warp * K + own] = w[0];
   }
   __syncthreads();
   // second level: value k by warp k mod (number of warps), not all K of them one after the other by warp 0 (the same

@@ -78,8 +78,9 @@ __device__ __forceinline__ void block_reduce(double (&v)[K], double *red, double
   // butterfly over the same numbers: same bits)
   for (int k = warp; k < K; k += NTHR / 32) {
     double x = lane < NTHR / 32 ? red[lane * K + k] : 0.0;
+    // (with W < 32 warps the stages at distance >= W add exact zeros to the lanes that matter: skipped, same bits)
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    for (int o = (NTHR / 32 < 32 ? NTHR / 32 : 32) / 2; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
     if (lane == 0) res[k] = x;
   }
   __syncthreads();
@@ -282,12 +283,32 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
 #pragma unroll
         for (int k = 0; k < SW; ++k) cfmac(d[k], sp[(size_t)k * m + i], x);
       }
+      {
+        // the 2 SW lane sums: transposed reduction (4 + 2 + 1 + 1 + 1 exchanges instead of 40; a kept sum is own + partner
+        // in the butterfly's stage order: same bits), then every total is broadcast from the lane that holds it
+        double w[2 * SW];
 #pragma unroll
-      for (int k = 0; k < SW; ++k) {
+        for (int k = 0; k < SW; ++k) { w[2 * k] = d[k].x; w[2 * k + 1] = d[k].y; }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          d[k].x += __shfl_xor_sync(0xffffffffu, d[k].x, o);
-          d[k].y += __shfl_xor_sync(0xffffffffu, d[k].y, o);
+        for (int st = 0; st < 5; ++st) {
+          const int o = 16 >> st, cnt = (2 * SW) >> (st + 1);
+          if (cnt >= 1) {
+            const int bit = (lane >> (4 - st)) & 1;
+#pragma unroll
+            for (int q = 0; q < cnt; ++q) {
+              const double keep = bit ? w[2 * q + 1] : w[2 * q], send = bit ? w[2 * q] : w[2 * q + 1];
+              w[q] = keep + __shfl_xor_sync(0xffffffffu, send, o);
+            }
+          } else {
+            w[0] += __shfl_xor_sync(0xffffffffu, w[0], o);
+          }
+        }
+        // value e = b0 + 2 b1 + 4 b2 lives in the lanes with bit 4 = b0, bit 3 = b1, bit 2 = b2
+#pragma unroll
+        for (int e = 0; e < 2 * SW; ++e) {
+          const int src = ((e & 1) << 4) | (((e >> 1) & 1) << 3) | (((e >> 2) & 1) << 2);
+          const double tot = __shfl_sync(0xffffffffu, w[0], src);
+          if (e & 1) d[e >> 1].y = tot; else d[e >> 1].x = tot;
         }
       }
       cplx gk[SW];  // g = T^H d

@@ -518,14 +518,18 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
   auto qr = [&](int c0, int s1, int s2) {
     const int m = n - (c0 + b);
     KScope ks(KC_PANEL, 0.0, s);
-    if (m > 640) {
-      const size_t smem = (size_t)SW * m * sizeof(cplx) + (32 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
-      panel_qr_kernel<1024><<<nmat, 1024, smem, s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
-    } else {
-      const size_t smem = (size_t)SW * m * sizeof(cplx) + (8 * 32 + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
-      if (nmat > 592) panel_qr_kernel<256, 4><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
-      else panel_qr_kernel<256, 2><<<nmat, 256, smem, s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
-    }
+    auto smem_of = [&](int nthr) {
+      return (size_t)SW * m * sizeof(cplx) + (nthr + 32) * sizeof(double) + (2 + SW * SW) * sizeof(cplx);
+    };
+    // The thread count depends on m only (it decides the summation order, i.e. the bits); the register budget (CTAs per SM)
+    // on the batch.  m <= 256: 128 threads (at most two rows per thread, four warps per block reduction) and twice as many
+    // CTAs per SM: C4 panel 15.2 -> 11.2 ms (64 threads: 10.5 ms there, but C2 1.22 -> 1.51 and C3 3.40 -> 3.68 ms; 128
+    // threads: 1.29 and 3.47).
+    if (m > 640) panel_qr_kernel<1024><<<nmat, 1024, smem_of(1024), s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
+    else if (m > 256 && nmat > 592) panel_qr_kernel<256, 4><<<nmat, 256, smem_of(256), s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
+    else if (m > 256) panel_qr_kernel<256, 2><<<nmat, 256, smem_of(256), s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
+    else if (nmat > 592) panel_qr_kernel<128, 8><<<nmat, 128, smem_of(128), s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
+    else panel_qr_kernel<128, 4><<<nmat, 128, smem_of(128), s>>>(n, lda, b, c0, A, VW, SM, inner, s1, s2);
     ++launches;
   };
   auto gemm = [&](int kclass, int M, int N, int K, int opA, int opB, int flags, BatchRef Ar, int la, BatchRef Br, int lb,

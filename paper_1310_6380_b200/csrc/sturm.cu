@@ -14,22 +14,36 @@ constexpr int ROUNDS = 24;   // 9^24 > 2^76
 // Number of eigenvalues < x = number of negative q_i = p_i / p_{i-1}, q_0 = d_0 - x, q_i = d_i - x - e_{i-1}^2 / q_{i-1}
 // (a zero pivot is replaced by a tiny negative one, the role of -pivmin in LAPACK dstebz).  Evaluated WITHOUT the division, whose latency (~100 cycles)
 // would serialise the recurrence: p_i = (d_i - x) p_{i-1} - e_{i-1}^2 p_{i-2}, a sign change between p_{i-1} and p_i
-// is a negative pivot.  The pair (p_{i-1}, p_i) is rescaled by a power of two whenever its exponent leaves [2^-400, 2^400]
-// (this does not change the ratio), so nothing overflows or underflows.
+// is a negative pivot.  The pair (p_{i-1}, p_i) is renormalised by the power of two that brings p_i into [1, 2) every
+// FOURTH step (an exact scaling of both, which changes no ratio and no sign): the chain of a step is then one DFMA and the
+// zero test, not DFMA -> exponent test -> multiply.  Between two renormalisations the pair may grow by ||T - x||^4 and
+// shrink by (2^-52 ||T - x||)^4, far inside the exponent range for any matrix this path produces.
+__device__ __forceinline__ void sturm_step(double di, double e2i, double x, double &p0, double &p1, int &cnt) {
+  double p2 = fma(di - x, p1, -(e2i * p0));
+  if (p2 == 0.0) p2 = -0x1p-200 * p1;  // q_i = -2^-200
+  cnt += (p2 < 0.0) != (p1 < 0.0);
+  p0 = p1;
+  p1 = p2;
+}
+__device__ __forceinline__ void sturm_renorm(double &p0, double &p1) {
+  const int ex = (__double2hiint(p1) >> 20) & 0x7ff;
+  const double sc = __hiloint2double((2046 - ex) << 20, 0);  // 2^(1023 - ex): p1 -> [1, 2)
+  p0 *= sc;
+  p1 *= sc;
+}
 __device__ __forceinline__ int sturm_count(const double *__restrict__ d, const double *__restrict__ e2, int n, double x) {
   double p0 = 1.0, p1 = d[0] - x;
   if (p1 == 0.0) p1 = -0x1p-200;  // zero pivot -> tiny negative pivot (relative 2^-200: far below rounding)
   int cnt = p1 < 0.0;
-  for (int i = 1; i < n; ++i) {
-    double p2 = fma(d[i] - x, p1, -(e2[i - 1] * p0));
-    if (p2 == 0.0) p2 = -0x1p-200 * p1;               // q_i = -2^-200 (|p1| >= 2^-453 after rescaling: no underflow)
-    cnt += (p2 < 0.0) != (p1 < 0.0);
-    const int ex = (__double2hiint(p2) >> 20) & 0x7ff;
-    double sc = 1.0;
-    if (ex > 1023 + 400) sc = 0x1p-400;
-    else if (ex < 1023 - 400) sc = 0x1p+400;
-    p0 = p1 * sc;
-    p1 = p2 * sc;
+  int i = 1;
+  for (; i + 3 < n; i += 4) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) sturm_step(d[i + u], e2[i + u - 1], x, p0, p1, cnt);
+    sturm_renorm(p0, p1);
+  }
+  for (; i < n; ++i) {
+    sturm_step(d[i], e2[i - 1], x, p0, p1, cnt);
+    sturm_renorm(p0, p1);
   }
   return cnt;
 }

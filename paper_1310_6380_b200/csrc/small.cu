@@ -74,9 +74,19 @@ __global__ void __launch_bounds__(ST) tridiag_small_kernel(int n, int lda, Batch
     if (ss == 0.0 && al.y == 0.0) {
       tau = cmake(0.0, 0.0); scale = cmake(0.0, 0.0); beta = al.x;
     } else {
-      beta = -copysign(sqrt(al.x * al.x + al.y * al.y + ss), al.x);
-      tau = cmake((beta - al.x) / beta, -al.y / beta);
-      const double dr = al.x - beta, di = al.y, den = 1.0 / (dr * dr + di * di);
+      // norm and reciprocals without the IEEE square root and divisions (as in chase.cu: rsqrt / rcp.approx + Newton
+      // steps, each good to about 1 ulp; tau, v and beta come from the same values, so H stays unitary to a few ulp)
+      const double s2 = al.x * al.x + al.y * al.y + ss, inrm = rsqrt(s2);
+      double nrm = s2 * inrm;
+      nrm = fma(fma(-nrm, nrm, s2), 0.5 * inrm, nrm);
+      beta = -copysign(nrm, al.x);
+      const double ib = -copysign(inrm, al.x);
+      tau = cmake((beta - al.x) * ib, -al.y * ib);
+      const double dr = al.x - beta, di = al.y, dd = dr * dr + di * di;
+      double den;
+      asm("rcp.approx.ftz.f64 %0, %1;\n" : "=d"(den) : "d"(dd));
+      den = fma(den, fma(-dd, den, 1.0), den);
+      den = fma(den, fma(-dd, den, 1.0), den);
       scale = cmake(dr * den, -di * den);
     }
     if (t == 0) { dg[j] = As[j * ld + j].x; eg[j] = beta; }
@@ -85,9 +95,20 @@ __global__ void __launch_bounds__(ST) tridiag_small_kernel(int n, int lda, Batch
     __syncthreads();
     // p = tau A22 v: thread (r, g) sums the columns c = g, g + 2, ... of its row
     {
-      cplx acc = cmake(0.0, 0.0);
-      if (r < m)
-        for (int c = g; c < m; c += 2) cfma(acc, As[(base + c) * ld + base + r], vs[c]);
+      // four independent partial sums: the row's dependent chain is m / 8 complex multiply-adds long instead of m / 2
+      cplx acc = cmake(0.0, 0.0), acc1 = cmake(0.0, 0.0), acc2 = cmake(0.0, 0.0), acc3 = cmake(0.0, 0.0);
+      if (r < m) {
+        const cplx *row = As + (size_t)base * ld + base + r;
+        int c = g;
+        for (; c + 6 < m; c += 8) {
+          cfma(acc, row[(size_t)c * ld], vs[c]);
+          cfma(acc1, row[(size_t)(c + 2) * ld], vs[c + 2]);
+          cfma(acc2, row[(size_t)(c + 4) * ld], vs[c + 4]);
+          cfma(acc3, row[(size_t)(c + 6) * ld], vs[c + 6]);
+        }
+        for (; c < m; c += 2) cfma(acc, row[(size_t)c * ld], vs[c]);
+        acc = cadd(cadd(acc, acc1), cadd(acc2, acc3));
+      }
       if (r < SNMAX) ps[g * SNMAX + r] = acc;
     }
     __syncthreads();

@@ -565,8 +565,9 @@ int launch_sy2sb(int n, int lda, int b, BatchRef A, BatchRef VW, BatchRef SM, Ba
     gemm(KC_GEMM_WY, b, 2 * b, m, 1, 0, 0, slot(sv, r0), n, slot(sv2, r0), n, smG, b, 1.0, 0.0, ksplit_of(m), (long long)2 * b * b);
     {
       KScope ks(KC_OTHER, 0.0, s);
-      // few matrices: one thread per entry (latency); many: smaller CTAs, several per SM (throughput)
-      wy_small_kernel<<<nmat, nmat > 592 ? 256 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner, ksplit_of(m));
+      // few matrices: one thread per entry (latency); many: smaller CTAs, several per SM (throughput; C4: 256 threads 3.98 ms of
+      // `other` per step, 128: 3.31, 64: 3.44, 32: 4.68).  Every entry is summed by one thread: the thread count changes no bit
+      wy_small_kernel<<<nmat, nmat > 592 ? 128 : b * b, (4 * b * b + b) * sizeof(cplx), s>>>(b, SM, inner, ksplit_of(m));
       ++launches;
     }
     keep(c0, sv, (long long)2 * b * b + b, 2 * b);

@@ -440,29 +440,41 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
 // Executed by all 2 NW warps of a team (role 0 = D warps, 1 = C warps).  State (i, k, J, L, finished) is identical in
 // every thread of the team.  Named barriers: 1 + team (whole team, only at k = 0), 5 + team / 9 + team (the D / C pair
 // of a B = 32 team; G <= 4 there), 15 (I/O warps).
+// The head of sweep i: the reflector that annihilates column i below the sub-diagonal (into the parity-0 buffers of the team
+// scratch); d[i], e[i] are final.  One warp.  Column i is final once sweep i - 1 has finished its step 0, i.e. one macro-step
+// before sweep i may start: a team that is idle then computes the head there (`head_done`), beside the steps of the
+// other teams, instead of at the start of its own step 0, where every second macro-step of the pipeline would wait for it.
+template <int B, int NW>
+__device__ __forceinline__ void sweep_head(const cplx *ring, int Wc, cplx *ts, int n, int i, int lane, double *dg, double *eg) {
+  using C = Cfg<B, NW>;
+  const int L = min(B, n - 1 - i);
+  const cplx *ci = ring + (size_t)(i % Wc) * C::LD;
+  cplx x = lane < L ? ci[1 + lane] : cmake(0.0, 0.0);
+  cplx tau0;
+  double beta;
+  warp_larfg(x, L, lane, tau0, beta);
+  if (lane < B) ts[C::O_V + lane] = x;
+  if (lane == 0) {
+    ts[C::O_TAU] = tau0;
+    eg[i] = beta;
+    dg[i] = ci[0].x;
+  }
+}
+
 template <int B, int NW>
 __device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, int i, int &k, int &J, int &sJ, int &L,
-                                          bool &finished, int role, int rw, int lane, int team, double *dg, double *eg) {
+                                          bool &finished, int role, int rw, int lane, int team, double *dg, double *eg,
+                                          bool &head_done) {
   using C = Cfg<B, NW>;
   const int par = k & 1;
   cplx *vb = ts + C::O_V + par * B, *vnext = ts + C::O_V + (par ^ 1) * B;
   if (k == 0) {
-    // the reflector that annihilates column i below the sub-diagonal; d[i], e[i] are final
     L = min(B, n - 1 - i);
-    if (role == 1 && rw == 0) {
-      const cplx *ci = ring + (size_t)(i % Wc) * C::LD;
-      cplx x = lane < L ? ci[1 + lane] : cmake(0.0, 0.0);
-      cplx tau0;
-      double beta;
-      warp_larfg(x, L, lane, tau0, beta);
-      if (lane < B) vb[lane] = x;
-      if (lane == 0) {
-        ts[C::O_TAU + par] = tau0;
-        eg[i] = beta;
-        dg[i] = ci[0].x;
-      }
+    if (!head_done) {  // (team-uniform)
+      if (role == 1 && rw == 0) sweep_head<B, NW>(ring, Wc, ts, n, i, lane, dg, eg);
+      named_bar(1 + team, C::TT);
     }
-    named_bar(1 + team, C::TT);
+    head_done = false;
   }
   const cplx tau = ts[C::O_TAU + par];
   const int Jn = J + L, L2 = min(B, n - Jn);
@@ -517,14 +529,18 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_resident_kernel(int n,
   __syncthreads();
   const int S = n >= 2 ? start[n - 2] + 1 : 0;  // the last sweep has a single step
   int i = 0, k = 0, J = 0, sJ = 0, L = 0, next_i = team;
-  bool finished = true;
+  bool finished = true, head_done = false;
   for (int s = 0; s < S; ++s) {
     if (finished && next_i <= n - 2 && start[next_i] == s) {
       i = next_i; k = 0; J = i + 1; sJ = J % Wc; L = 0; finished = false;
     }
     if (!finished) {
-      team_step<B, NW>(ring, Wc, ts, n, i, k, J, sJ, L, finished, role, rw, lane, team, dg, eg);
+      team_step<B, NW>(ring, Wc, ts, n, i, k, J, sJ, L, finished, role, rw, lane, team, dg, eg, head_done);
       if (finished) next_i += G;
+    } else if (next_i <= n - 2 && start[next_i] == s + 1) {
+      // idle now, the next sweep of this team starts at the next macro-step: its column is final, its head goes here
+      if (role == 1 && rw == 0) sweep_head<B, NW>(ring, Wc, ts, n, next_i, lane, dg, eg);
+      head_done = true;
     }
     __syncthreads();
   }
@@ -624,7 +640,7 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
     __syncthreads();
 
     int i = t0 + team, k = 0, J = i + 1, sJ = J % Wc, L = 0;
-    bool finished = is_io || team >= nvalid;
+    bool finished = is_io || team >= nvalid, head_done = false;
     const int nsteps0 = (n - 1 - t0 + B - 1) / B;
     const int S = nsteps0 + 2 * (nvalid - 1);
     for (int s = 0; s < S; ++s) {
@@ -662,7 +678,13 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
         io_load(whi, hi, io_tid, io_nt);
       }
       wlo = keep; whi = hi;
-      if (!finished && s >= 2 * team) team_step<B, NW>(ring, Wc, ts, n, i, k, J, sJ, L, finished, role, rw, lane, team, dg, eg);
+      if (!finished && s >= 2 * team) {
+        team_step<B, NW>(ring, Wc, ts, n, i, k, J, sJ, L, finished, role, rw, lane, team, dg, eg, head_done);
+      } else if (!finished && s == 2 * team - 1) {
+        // the sweep starts at the next macro-step: its column is final (the sweep before it has finished its step 0)
+        if (role == 1 && rw == 0) sweep_head<B, NW>(ring, Wc, ts, n, i, lane, dg, eg);
+        head_done = true;
+      }
       __syncthreads();
     }
     // the tail of the window goes back; the train is done

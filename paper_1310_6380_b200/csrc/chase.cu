@@ -32,7 +32,7 @@
 namespace bsk {
 
 namespace {
-constexpr int NIO = 4;  // I/O warps of the streamed variant
+constexpr int NIO = 2;  // I/O warps of the streamed variant (four left room for six teams of two warps; two for seven: C5 35.8 -> 34.5 ms, C3 6.29 -> 6.06)
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -576,7 +576,7 @@ __global__ void __launch_bounds__(Cfg<B, NW>::MAXT) chase_stream_kernel(int n, B
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int ncomp = G * C::TT;
   const bool is_io = tid >= ncomp;
-  const int io_tid = tid - ncomp, io_nt = NIO * 32;
+  const int io_tid = tid - ncomp, io_nt = (int)blockDim.x - ncomp;
   // warps [0, G NW): the D warps of teams 0 .. G-1, then the C warps (the issue arbiter favours the higher warp index:
   // the C half is the longer chain), then the I/O warps; every scheduler hosts warps of both roles
   const int role = warp >= G * NW ? 1 : 0, wr = warp - role * G * NW, team = wr / NW, rw = wr % NW;

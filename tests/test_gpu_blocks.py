@@ -291,6 +291,28 @@ def test_sturm_random_and_degenerate(bs):
         assert np.max(np.abs(got[b] - ref)) <= 1e-14 * n * max(1.0, np.max(np.abs(ref)))
 
 
+@pytest.mark.parametrize("scale", [1e-60, 1.0, 1e12, 1e60])
+@pytest.mark.parametrize("n", [5, 98, 1023, 1922])
+def test_sturm_scaled_matrices(bs, n, scale):
+    """The Sturm recurrence is renormalised by an exact power of two every fourth step (S7): matrices
+    whose entries sit at 1e-60 .. 1e60 make the unscaled pair grow or shrink by hundreds of orders of magnitude over n steps
+    (lengths with every remainder modulo four).  The eigenvalues must scale with the matrix, to rounding."""
+    import torch
+    rng = np.random.default_rng(n)
+    dn = rng.normal(size=(2, n)) * scale
+    en = rng.normal(size=(2, n)) * scale
+    dn[1] = np.abs(dn[1]) + 3.0 * scale   # second matrix: diagonally dominant, positive definite
+    nev = min(n, 18)
+    d, e = torch.from_numpy(dn).cuda(), torch.from_numpy(en).cuda()
+    lam = torch.zeros(2, nev, dtype=torch.float64, device="cuda")
+    bs.bs_sturm(n, d, e, nev, lam, 2)
+    got = lam.cpu().numpy()
+    for b in range(2):
+        T = np.diag(dn[b] / scale) + np.diag(en[b, :n - 1] / scale, 1) + np.diag(en[b, :n - 1] / scale, -1)
+        ref = np.linalg.eigvalsh(T)
+        assert np.max(np.abs(got[b] / scale - ref[:nev])) <= 1e-14 * n * max(1.0, np.max(np.abs(ref)))
+
+
 def test_error_paths(bs):
     c = wl.random_small_cell(1, 2)
     comp = bs.bs_isotropic_plane_strain(c.E, c.nu)

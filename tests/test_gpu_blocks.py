@@ -196,6 +196,28 @@ def test_zhetrd_eigenvalues(bs, n, nb, algo):
         assert np.max(np.abs(lt - la)) <= 1e-13 * n * np.max(np.abs(la))
 
 
+@pytest.mark.parametrize("scale", [1e-100, 1e100])
+@pytest.mark.parametrize("n,nb,algo", [(98, 16, 0), (300, 16, 0), (300, 16, 2), (300, 8, 0), (500, 16, 0)])
+def test_zhetrd_scaled_matrices(bs, n, nb, algo, scale):
+    """The reflectors of the chase and of the small-matrix kernel take their norm from rsqrt and their reciprocals from
+    rcp.approx + Newton steps (chase item (7)): matrices at 1e-100 and 1e100 must give the scaled
+    eigenvalues to the usual backward error (squares of the entries stay far inside the exponent range)."""
+    import torch
+    rng = np.random.default_rng(7 * n + nb)
+    G = rand_c(rng, n, n)
+    A = G + G.conj().T
+    dA = to_dev(A * scale)[None].contiguous()
+    d = torch.zeros(1, n, dtype=torch.float64, device="cuda")
+    e = torch.zeros(1, n, dtype=torch.float64, device="cuda")
+    scratch = torch.zeros(bs.bs_zhetrd_scratch_elems(n, nb), dtype=torch.complex128, device="cuda")
+    bs.bs_zhetrd(n, dA, n, n * n, d, e, scratch, nb, algo, 1)
+    torch.cuda.synchronize()
+    dd, ee = d[0].cpu().numpy() / scale, e[0].cpu().numpy()[:n - 1] / scale
+    T = np.diag(dd) + np.diag(ee, 1) + np.diag(ee, -1)
+    la = np.linalg.eigvalsh(A)
+    assert np.max(np.abs(np.linalg.eigvalsh(T) - la)) <= 1e-13 * n * np.max(np.abs(la))
+
+
 @pytest.mark.parametrize("n,nb,batch", [(242, 16, 1500), (242, 8, 1500), (338, 16, 900), (242, 32, 600)])
 def test_zhetrd_forced_streaming_large_batch(bs, n, nb, batch):
     """BS_TRIDIAG_TWO_STAGE_STREAMED runs stage 2 through the ring of three sweeps with several CTAs per SM (the I/O

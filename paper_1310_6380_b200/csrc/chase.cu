@@ -159,7 +159,8 @@ __device__ __forceinline__ double frag_cols(const cplx *b, const cplx *d, int id
 // ---------------------------------------------------------------------------------------------- the D half of a step
 // D <- H^H D H on the L x L Hermitian block at (J, J); v, tau of the step are in the team scratch.  Warp rw of the NW
 // D warps owns the tile columns ctg(rw, .) (all tile rows); tiles strictly above the diagonal are only read.
-template <int B, int NW>
+// FULL: the block is complete (L = B): every mask below is true and is compiled out (team-uniform choice, same bits).
+template <int B, int NW, bool FULL>
 __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, const cplx *vb, cplx tau, int L, int rw,
                                        int lane, int bar_id) {
   using C = Cfg<B, NW>;
@@ -195,7 +196,7 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
         const int r = 8 * rt + g;
         const bool low = r >= c;
         const cplx a = ring[low ? cs + r : rs[rt] + c];  // lower part as stored, upper part mirrored
-        const bool ok = r < L && c < L;
+        const bool ok = FULL || (r < L && c < L);
         tre[rt][ci][j] = ok ? a.x : 0.0;
         tim[rt][ci][j] = (ok && r != c) ? (low ? a.y : -a.y) : 0.0;
       }
@@ -225,7 +226,7 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
   for (int w2 = 1; w2 < NW; ++w2) p = cadd(p, ts[C::O_P + w2 * B + l]);
   p = cmul(tau, p);
   const cplx v = vb[l];
-  const bool in = l < L;
+  const bool in = FULL || l < L;
   double sr = in ? p.x * v.x + p.y * v.y : 0.0, si = in ? p.x * v.y - p.y * v.x : 0.0;  // p^H v
 #pragma unroll
   for (int o = (B < 32 ? B : 32) / 2; o > 0; o >>= 1) {
@@ -265,7 +266,7 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
 #pragma unroll
       for (int rt = 0; rt < TR; ++rt) {
         const int r = 8 * rt + g;
-        if (r >= c && r < L) ring[cs + r] = cmake(tre[rt][ci][j], r == c ? 0.0 : tim[rt][ci][j]);
+        if (r >= c && (FULL || r < L)) ring[cs + r] = cmake(tre[rt][ci][j], r == c ? 0.0 : tim[rt][ci][j]);
       }
     }
   }
@@ -274,7 +275,8 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
 // ---------------------------------------------------------------------------------------------- the C half of a step
 // C <- H2^H (C H) on the L2 x L block below D; produces the next reflector (v2 -> vnext, tau2 -> *tau_next).  Warp rw of
 // the NW C warps owns the tile columns rw TCW .. (rw + 1) TCW - 1 (all tile rows).
-template <int B, int NW>
+// FULL: both blocks are complete (L = L2 = B): the masks are compiled out.
+template <int B, int NW, bool FULL>
 __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, const cplx *vb, cplx *vnext, cplx *tau_next,
                                        cplx tau, int L, int L2, int rw, int lane, int bar_id, int team_bar) {
   using C = Cfg<B, NW>;
@@ -292,13 +294,13 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
       const int c = 8 * (rw * TCW + ci) + 2 * t + j;
       int sl = sJ + c;
       sl -= sl >= Wc ? Wc : 0;
-      const int cs = sl * LD + (c < L ? L - c : 0);  // (a masked column reads its own first entries)
+      const int cs = sl * LD + ((FULL || c < L) ? L - c : 0);  // (a masked column reads its own first entries)
       vc[ci][j] = vb[c];
 #pragma unroll
       for (int rt = 0; rt < TR; ++rt) {
         const int r = 8 * rt + g;
         cplx a = ring[cs + r];
-        const bool ok = r < L2 && c < L;
+        const bool ok = FULL || (r < L2 && c < L);
         tre[rt][ci][j] = ok ? a.x : 0.0;
         tim[rt][ci][j] = ok ? a.y : 0.0;
       }
@@ -328,7 +330,7 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   cplx u = ts[C::O_U + l];
 #pragma unroll
   for (int w2 = 1; w2 < NW; ++w2) u = cadd(u, ts[C::O_U + w2 * B + l]);
-  const bool in = l < L2;
+  const bool in = FULL || l < L2;
   cplx tu = cmul(tau, u);
   tu.x = in ? tu.x : 0.0;
   tu.y = in ? tu.y : 0.0;
@@ -430,7 +432,7 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
 #pragma unroll
       for (int rt = 0; rt < TR; ++rt) {
         const int r = 8 * rt + g;
-        if (r < L2 && c < L) ring[cs + r] = cmake(tre[rt][ci][j], tim[rt][ci][j]);
+        if (FULL || (r < L2 && c < L)) ring[cs + r] = cmake(tre[rt][ci][j], tim[rt][ci][j]);
       }
     }
   }
@@ -481,9 +483,13 @@ __device__ __forceinline__ void team_step(cplx *ring, int Wc, cplx *ts, int n, i
   if (role == 0) {
     // the C warps (the longer chain of the step) load their tiles first: the D warps wait until those are in registers
     if (L2 > 0) named_bar(1 + team, C::TT);
-    step_D<B, NW>(ring, Wc, sJ, ts, vb, tau, L, rw, lane, 5 + team);
+    if (L == B) step_D<B, NW, true>(ring, Wc, sJ, ts, vb, tau, L, rw, lane, 5 + team);
+    else step_D<B, NW, false>(ring, Wc, sJ, ts, vb, tau, L, rw, lane, 5 + team);
   } else if (L2 > 0) {
-    step_C<B, NW>(ring, Wc, sJ, ts, vb, vnext, ts + C::O_TAU + (par ^ 1), tau, L, L2, rw, lane, 9 + team, 1 + team);
+    if (L == B && L2 == B)
+      step_C<B, NW, true>(ring, Wc, sJ, ts, vb, vnext, ts + C::O_TAU + (par ^ 1), tau, L, L2, rw, lane, 9 + team, 1 + team);
+    else
+      step_C<B, NW, false>(ring, Wc, sJ, ts, vb, vnext, ts + C::O_TAU + (par ^ 1), tau, L, L2, rw, lane, 9 + team, 1 + team);
   }
   if (L2 <= 0) {
     finished = true;

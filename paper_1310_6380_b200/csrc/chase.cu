@@ -101,6 +101,17 @@ struct Cfg {
   static_assert(TC % NW == 0, "tile columns split over the role's warps");
 };
 
+// Complex products and sums of products with EXPLICIT fused multiply-adds: this file is compiled without implicit contraction
+// (so that the copies of a step inlined into different kernels round identically); explicit fma() calls are DFMAs in every
+// copy, one instruction and one rounding instead of a DMUL and a DADD.
+__device__ __forceinline__ cplx cmul_f(cplx a, cplx b) {
+  return make_double2(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ cplx cmulc_f(cplx a, cplx b) {  // a * conj(b)
+  return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -(a.x * b.y)));
+}
+__device__ __forceinline__ double sumsq_f(double a, double b) { return fma(a, a, b * b); }
+
 // The norm of a reflector's vector and its reciprocal, and a reciprocal, without the IEEE square root and division: their
 // fix-up sequences are ~25 dependent instructions each on the chain of every step.  rsqrt is good to 1 ulp, the Newton
 // step makes s * rsqrt(s) a square root good to about 1 ulp, the two Newton steps on rcp.approx (2^-23) a reciprocal
@@ -123,7 +134,7 @@ __device__ __forceinline__ double fast_rcp(double d) {
 // LAPACK zlarfg on a vector spread over the 32 lanes of a warp (x valid for l < len; other lanes must hold 0):
 // H = I - tau v v^H, H^H x = beta e_1, beta real, v[0] = 1.  Returns v in x.
 __device__ __forceinline__ void warp_larfg(cplx &x, int len, int l, cplx &tau, double &beta) {
-  const double ss = warp_sum((l >= 1 && l < len) ? x.x * x.x + x.y * x.y : 0.0);
+  const double ss = warp_sum((l >= 1 && l < len) ? sumsq_f(x.x, x.y) : 0.0);
   const cplx al = shfl_c(x, 0);
   if (ss == 0.0 && al.y == 0.0) {
     tau = cmake(0.0, 0.0);
@@ -132,14 +143,14 @@ __device__ __forceinline__ void warp_larfg(cplx &x, int len, int l, cplx &tau, d
     return;
   }
   double nrm, inrm;
-  norm_and_inverse(al.x * al.x + al.y * al.y + ss, nrm, inrm);
+  norm_and_inverse(sumsq_f(al.x, al.y) + ss, nrm, inrm);
   beta = -copysign(nrm, al.x);
   const double ib = -copysign(inrm, al.x);
   tau = cmake((beta - al.x) * ib, -al.y * ib);
-  const double dr = al.x - beta, di = al.y, den = fast_rcp(dr * dr + di * di);
+  const double dr = al.x - beta, di = al.y, den = fast_rcp(sumsq_f(dr, di));
   const cplx scale = cmake(dr * den, -di * den);
   if (l == 0) x = cmake(1.0, 0.0);
-  else if (l < len) x = cmul(x, scale);
+  else if (l < len) x = cmul_f(x, scale);
   else x = cmake(0.0, 0.0);
 }
 
@@ -224,16 +235,16 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
   cplx p = ts[C::O_P + l];
 #pragma unroll
   for (int w2 = 1; w2 < NW; ++w2) p = cadd(p, ts[C::O_P + w2 * B + l]);
-  p = cmul(tau, p);
+  p = cmul_f(tau, p);
   const cplx v = vb[l];
   const bool in = FULL || l < L;
-  double sr = in ? p.x * v.x + p.y * v.y : 0.0, si = in ? p.x * v.y - p.y * v.x : 0.0;  // p^H v
+  double sr = in ? fma(p.x, v.x, p.y * v.y) : 0.0, si = in ? fma(p.x, v.y, -(p.y * v.x)) : 0.0;  // p^H v
 #pragma unroll
   for (int o = (B < 32 ? B : 32) / 2; o > 0; o >>= 1) {
     sr += __shfl_xor_sync(0xffffffffu, sr, o);
     si += __shfl_xor_sync(0xffffffffu, si, o);
   }
-  const cplx alpha = cmul(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
+  const cplx alpha = cmul_f(cmake(-0.5 * tau.x, -0.5 * tau.y), cmake(sr, si));
   cplx w = p;
   cfma(w, alpha, v);
   if (lane < B) ts[C::O_W + lane] = in ? w : cmake(0.0, 0.0);
@@ -331,7 +342,7 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
 #pragma unroll
   for (int w2 = 1; w2 < NW; ++w2) u = cadd(u, ts[C::O_U + w2 * B + l]);
   const bool in = FULL || l < L2;
-  cplx tu = cmul(tau, u);
+  cplx tu = cmul_f(tau, u);
   tu.x = in ? tu.x : 0.0;
   tu.y = in ? tu.y : 0.0;
   cplx x = csub(ts[C::O_C0 + l], tu);
@@ -339,9 +350,9 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   x.y = in ? x.y : 0.0;
   // three lane reductions in one butterfly: |x[1:]|^2 and sum_{l>=1} conj(x_l) (tau u)_l, which gives
   // s = v2^H (tau u) = (tau u)_0 + conj(scale) sum_{l>=1} conj(x_l) (tau u)_l  without a second pass over the lanes
-  double ss = l >= 1 ? x.x * x.x + x.y * x.y : 0.0;
-  double sdr = l >= 1 ? x.x * tu.x + x.y * tu.y : 0.0;
-  double sdi = l >= 1 ? x.x * tu.y - x.y * tu.x : 0.0;
+  double ss = l >= 1 ? sumsq_f(x.x, x.y) : 0.0;
+  double sdr = l >= 1 ? fma(x.x, tu.x, x.y * tu.y) : 0.0;
+  double sdi = l >= 1 ? fma(x.x, tu.y, -(x.y * tu.x)) : 0.0;
 #pragma unroll
   for (int o = (B < 32 ? B : 32) / 2; o > 0; o >>= 1) {
     ss += __shfl_xor_sync(0xffffffffu, ss, o);
@@ -351,21 +362,21 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
   const cplx al = shfl_c(x, 0), tu0 = shfl_c(tu, 0);
   const bool norefl = L2 <= 1, trivial = norefl || (ss == 0.0 && al.y == 0.0);
   double nrm, inrm;
-  norm_and_inverse(al.x * al.x + al.y * al.y + ss, nrm, inrm);
+  norm_and_inverse(sumsq_f(al.x, al.y) + ss, nrm, inrm);
   const double beta2 = trivial ? 1.0 : -copysign(nrm, al.x);
   const double ib = trivial ? 1.0 : -copysign(inrm, al.x);
   cplx tau2 = cmake((beta2 - al.x) * ib, -al.y * ib);
   tau2.x = trivial ? 0.0 : tau2.x;
   tau2.y = trivial ? 0.0 : tau2.y;
   const double dr = al.x - beta2, di = al.y;
-  const double den = fast_rcp(dr * dr + di * di);
+  const double den = fast_rcp(sumsq_f(dr, di));
   cplx scale = cmake(dr * den, -di * den);
   scale.x = trivial ? 0.0 : scale.x;
   scale.y = trivial ? 0.0 : scale.y;
-  cplx v2 = cmul(x, scale);
+  cplx v2 = cmul_f(x, scale);
   v2.x = l == 0 ? 1.0 : v2.x;
   v2.y = l == 0 ? 0.0 : v2.y;
-  const cplx sv = cadd(tu0, cmulc(cmake(sdr, sdi), scale));  // (tau u)_0 + conj(scale) sum conj(x_l) (tau u)_l
+  const cplx sv = cadd(tu0, cmulc_f(cmake(sdr, sdi), scale));  // (tau u)_0 + conj(scale) sum conj(x_l) (tau u)_l
   const double s_re = sv.x, s_im = sv.y;
   if (lane < B) {
     ts[C::O_TU + lane] = tu;
@@ -393,8 +404,8 @@ __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, con
     const int co = 8 * (rw * TCW + (own >> 1)) + 2 * t + (own & 1);
     // y = tau2 conj(z0 - s conj(v)) = tau2 (conj(z0) - conj(s) v)
     const cplx vcj = vb[co];
-    const cplx q = cmake(zs.x - (s_re * vcj.x + s_im * vcj.y), -zs.y - (s_re * vcj.y - s_im * vcj.x));
-    if (g < 2 * TCW) ts[C::O_Y + co] = cmul(tau2, q);
+    const cplx q = cmake(zs.x - fma(s_re, vcj.x, s_im * vcj.y), -zs.y - fma(s_re, vcj.y, -(s_im * vcj.x)));
+    if (g < 2 * TCW) ts[C::O_Y + co] = cmul_f(tau2, q);
   }
   __syncwarp();
   // C -= (tau u) v^H + v2 y^H   (a, b, c, d) = (tau u, v, v2, y)

@@ -172,8 +172,9 @@ __device__ __forceinline__ double frag_cols(const cplx *b, const cplx *d, int id
 // D warps owns the tile columns ctg(rw, .) (all tile rows); tiles strictly above the diagonal are only read.
 // FULL: the block is complete (L = B): every mask below is true and is compiled out (team-uniform choice, same bits).
 template <int B, int NW, bool FULL>
-__device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, const cplx *vb, cplx tau, int L, int rw,
+__device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, const cplx *vb, cplx tau, int L, int rw_,
                                        int lane, int bar_id) {
+  const int rw = NW == 1 ? 0 : rw_;  // (one warp per half: a compile-time zero, the tile positions below become constants)
   using C = Cfg<B, NW>;
   constexpr int LD = C::LD, TR = C::TR, TCW = C::TCW;
   const int g = lane >> 2, t = lane & 3;
@@ -289,7 +290,8 @@ __device__ __forceinline__ void step_D(cplx *ring, int Wc, int sJ, cplx *ts, con
 // FULL: both blocks are complete (L = L2 = B): the masks are compiled out.
 template <int B, int NW, bool FULL>
 __device__ __forceinline__ void step_C(cplx *ring, int Wc, int sJ, cplx *ts, const cplx *vb, cplx *vnext, cplx *tau_next,
-                                       cplx tau, int L, int L2, int rw, int lane, int bar_id, int team_bar) {
+                                       cplx tau, int L, int L2, int rw_, int lane, int bar_id, int team_bar) {
+  const int rw = NW == 1 ? 0 : rw_;
   using C = Cfg<B, NW>;
   constexpr int LD = C::LD, TR = C::TR, TCW = C::TCW;
   const int g = lane >> 2, t = lane & 3;

@@ -147,9 +147,19 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
         if (ss == 0.0 && al.y == 0.0) {
           tau = cmake(0.0, 0.0); scale = cmake(0.0, 0.0); beta = al.x;
         } else {
-          beta = -copysign(sqrt(al.x * al.x + al.y * al.y + ss), al.x);
-          tau = cmake((beta - al.x) / beta, -al.y / beta);
-          const double dr = al.x - beta, di = al.y, den = 1.0 / (dr * dr + di * di);
+          // norm and reciprocals by rsqrt / rcp.approx + Newton steps (each good to about 1 ulp) instead of the IEEE square
+          // root and three divisions: the whole CTA waits for this thread at the next barrier, once per column
+          const double s2 = al.x * al.x + al.y * al.y + ss, inrm = rsqrt(s2);
+          double nrm = s2 * inrm;
+          nrm = fma(fma(-nrm, nrm, s2), 0.5 * inrm, nrm);
+          beta = -copysign(nrm, al.x);
+          const double ib = -copysign(inrm, al.x);
+          tau = cmake((beta - al.x) * ib, -al.y * ib);
+          const double dr = al.x - beta, di = al.y, dd = dr * dr + di * di;
+          double den;
+          asm("rcp.approx.ftz.f64 %0, %1;\n" : "=d"(den) : "d"(dd));
+          den = fma(den, fma(-dd, den, 1.0), den);
+          den = fma(den, fma(-dd, den, 1.0), den);
           scale = cmake(dr * den, -di * den);
         }
         scal[0] = tau; scal[1] = scale;

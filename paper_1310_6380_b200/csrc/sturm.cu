@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
   extern __shared__ double sm[];
   double *d = sm, *e2 = sm + n;
   __shared__ double s_lo, s_hi;
-  __shared__ int cnts[ST];
+  __shared__ __align__(8) int cnts[ST];
   const int z = blockIdx.x, t = threadIdx.x;
   dg += (size_t)z * n;
   eg += (size_t)z * n;
@@ -63,17 +63,30 @@ __global__ void __launch_bounds__(ST) sturm_kernel(int n, const double *__restri
     e2[i] = (i + 1 < n) ? eg[i] * eg[i] : 0.0;
   }
   __syncthreads();
-  if (t == 0) {  // Gershgorin bounds (n <= 2048: serial is fine next to the bisection itself)
+  {
+    // Gershgorin bounds: every thread takes rows t, t + nthr, ...; minimum and maximum over the CTA (exact, whatever the
+    // order).  (One thread looping over all n rows, two square roots each, was a tenth of the kernel at n = 1922.)
     double lo = d[0], hi = d[0];
-    for (int i = 0; i < n; ++i) {
+    for (int i = t; i < n; i += nthr) {
       const double l = i > 0 ? sqrt(e2[i - 1]) : 0.0, r = i + 1 < n ? sqrt(e2[i]) : 0.0;
       lo = fmin(lo, d[i] - l - r);
       hi = fmax(hi, d[i] + l + r);
     }
-    const double nrm = fmax(fabs(lo), fabs(hi));
-    lo -= 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
-    hi += 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
-    s_lo = lo; s_hi = hi;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+      hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+    }
+    double *red = reinterpret_cast<double *>(cnts);  // (cnts is not in use yet: ST ints = ST / 2 doubles >= 2 per warp)
+    if ((t & 31) == 0) { red[2 * (t >> 5)] = lo; red[2 * (t >> 5) + 1] = hi; }
+    __syncthreads();
+    if (t == 0) {
+      for (int w = 1; w < (nthr + 31) / 32; ++w) { lo = fmin(lo, red[2 * w]); hi = fmax(hi, red[2 * w + 1]); }
+      const double nrm = fmax(fabs(lo), fabs(hi));
+      lo -= 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
+      hi += 2.0 * nrm * 2.3e-16 * n + 2.0 * 2.3e-308;
+      s_lo = lo; s_hi = hi;
+    }
   }
   __syncthreads();
   const int grp = t / G, sub = t % G;

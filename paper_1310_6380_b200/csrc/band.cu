@@ -112,10 +112,9 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
 
   for (int js = 0; js < b; js += SW) {
     // 1. sub-panel -> shared memory
-    for (int q = t; q < SW * m; q += NTHR) {
-      const int jj = q / m, i = q % m;
-      sp[q] = Ag[(size_t)(r0 + i) + (size_t)(c0 + js + jj) * lda];
-    }
+#pragma unroll
+    for (int jj = 0; jj < SW; ++jj)  // (column by column: no integer division per element)
+      for (int i = t; i < m; i += NTHR) sp[(size_t)jj * m + i] = Ag[(size_t)(r0 + i) + (size_t)(c0 + js + jj) * lda];
     __syncthreads();
     cplx taus[SW];
     double nxt = -1.0;  // partial sum of |x|^2 below the pivot of the next column, gathered while it is updated
@@ -260,12 +259,13 @@ __global__ void __launch_bounds__(NTHR, MINB) panel_qr_kernel(int n, int lda, in
       }
     }
     // 4. V columns out
-    for (int q = t; q < SW * m; q += NTHR) {
-      const int jj = q / m, i = q % m;
-      const cplx v = sp[q];
-      V1[(size_t)(js + jj) * n + r0 + i] = v;
-      V2[(size_t)(js + jj) * n + r0 + i] = v;
-    }
+#pragma unroll
+    for (int jj = 0; jj < SW; ++jj)
+      for (int i = t; i < m; i += NTHR) {
+        const cplx v = sp[(size_t)jj * m + i];
+        V1[(size_t)(js + jj) * n + r0 + i] = v;
+        V2[(size_t)(js + jj) * n + r0 + i] = v;
+      }
     __syncthreads();  // Tm visible
     // 5. remaining panel columns: x <- x - V T^H (V^H x), one warp per column, rows >= js
     cplx Tr[SW][SW];

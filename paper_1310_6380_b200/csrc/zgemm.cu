@@ -512,6 +512,7 @@ void launch_zgemm(const GemmDesc &g, cudaStream_t s) {
   if (g.flags & BS_GEMM_A_HERM_LOWER) { launch_one<0, 0, 1>(g, s); return; }  // requires opA == opB == 0, K == M
   if (g.opA == 0 && g.opB == 0) launch_one<0, 0, 0>(g, s);
   else if (g.opA == 0 && g.opB == 1) launch_one<0, 1, 0>(g, s);
+  else if (g.opA == 1 && g.opB == 0 && g.M <= 48 && g.M % 32 != 0 && g.flags == 0) launch_one<1, 0, 0, 16, 32, 64>(g, s);  // Gram products of the band reduction (M = 16, 48): 16-row tiles waste no half tile
   else if (g.opA == 1 && g.opB == 0) launch_one<1, 0, 0>(g, s);
   else launch_one<1, 1, 0>(g, s);
 }
